@@ -1,0 +1,152 @@
+/*
+ * vlasov.h -- C ABI of the B200-native Strang semi-Lagrangian Vlasov step.
+ *
+ * Method: T. M. Rocha Filho, "Solving the Vlasov equation for one-dimensional models with long range
+ * interactions on a GPU", arXiv 1206.3229.  Citations below are PAPER.md line numbers.
+ *
+ * The library advances the one-particle distribution f(theta, p) on an equally spaced grid
+ * (section 3) stored as ONE flat row-major array  f[j * Ntheta + i],  i the position index
+ * (fastest), j the momentum index (L115), resident in GPU memory for the whole run (L115), by the time-split
+ * steps (1)-(4) of section 3 (L71-L87, eqs (9)-(12)):
+ *     f_I (x,p) = f(x - p dt/2, p);  F_I = mean-field force of f_I;  f_II(x,p) = f_I(x, p - F_I(x) dt);
+ *     f(t+dt)   = f_II(x - p dt/2, p),
+ * every value at the foot of a characteristic taken from the cubic spline of eqs (13)-(14) (L89-L98) whose
+ * second derivatives are the eighth-order centred difference of eq (16) (L106-L111).
+ *
+ * Conventions common to all calls
+ *   - every function returns 0 on success or a negative VLASOV_E* code; no exception crosses the ABI;
+ *     vlasov_last_error() gives a static, thread-local, human-readable message for the last failure;
+ *   - one singleton context per process; calls are not thread-safe;
+ *   - "host" pointers are ordinary CPU memory (pinned or pageable), "device" pointers are CUDA global memory
+ *     of the current device; the library never frees memory it was handed through vlasov_attach;
+ *   - all work is enqueued on the attached CUDA stream (default: the legacy default stream); only
+ *     vlasov_moments, vlasov_download, vlasov_history, vlasov_get_vector and vlasov_sync block the host;
+ *   - there is no CPU fallback: without a CUDA device vlasov_init fails with VLASOV_ECUDA.
+ *   - grid nodes: x_i = x_min + i (x_max - x_min)/Ntheta, i = 0..Ntheta-1 (right end excluded), same for p.
+ */
+#ifndef VLASOV_B200_H
+#define VLASOV_B200_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* error codes */
+#define VLASOV_OK 0
+#define VLASOV_EINVAL (-1)   /* bad argument or call order                       */
+#define VLASOV_ENOTINIT (-2) /* vlasov_init has not been called                  */
+#define VLASOV_ECUDA (-3)    /* a CUDA call failed; sticky until vlasov_init     */
+#define VLASOV_ENOMEM (-4)   /* allocation failed / attached workspace too small */
+
+/* model: which pair potential defines the mean-field force, section 2 */
+#define VLASOV_MODEL_FREE 0  /* F = 0 (free streaming; tests)                                    */
+#define VLASOV_MODEL_HMF 1   /* eq (3); force by the two moments of eqs (7)-(8) L56-L63      */
+#define VLASOV_MODEL_RING 2  /* eq (2), softened; direct circulant sum over theta        */
+#define VLASOV_MODEL_SHEET 3 /* eq (4), V = |x - x'|; prefix sum of the density          */
+
+/* keys of vlasov_set_param */
+#define VLASOV_KEY_EPS 1       /* ring softening epsilon of eq (2); default 0.01                            */
+#define VLASOV_KEY_PRECISION 2 /* storage precision of f: 64 (default) or 32; arithmetic of sums is fp64    */
+#define VLASOV_KEY_BC_X 3      /* 0 periodic (paper, L113; default for FREE/HMF/RING), 1 zero extension     */
+#define VLASOV_KEY_BC_P 4      /* 0 periodic (paper, L113), 1 zero extension "f = 0 beyond" (default)       */
+#define VLASOV_KEY_HISTORY 5   /* 1: vlasov_step records the 8 moments after every step (no a6 fusion)      */
+#define VLASOV_KEY_FUSE 6      /* 1 (default): consecutive half theta-shifts of steps k, k+1 run as one pass */
+
+/* sub-steps for vlasov_substep (parity tests of single stages; same kernels as vlasov_step) */
+#define VLASOV_SUB_THETA_HALF 0  /* eq (9)/(12): f(x - p dt/2, p), also leaves the column sums for the force */
+#define VLASOV_SUB_FORCE 1       /* eq (10): density + force of the CURRENT f (runs its own density pass)    */
+#define VLASOV_SUB_P_FULL 2      /* eq (11): f(x, p - F dt) with the force vector currently stored           */
+#define VLASOV_SUB_THETA_TWICE 3 /* two half shifts in one pass (the fused a5 o a1 kernel)                   */
+
+/* vectors for vlasov_get_vector / vlasov_set_vector (Ntheta doubles each) */
+#define VLASOV_VEC_RHO 0   /* density rho_i = dp sum_j f_ij used by the last force evaluation */
+#define VLASOV_VEC_FORCE 1 /* force F_i used by (or set for) the next momentum shift           */
+
+/*
+ * Create the singleton context (frees a previous one).
+ *   model   VLASOV_MODEL_*
+ *   grid    {Ntheta, Np}  (host), each >= 1
+ *   domain  {x_min, x_max, p_min, p_max} (host), half-open intervals
+ *   dt      time step of one full Strang step
+ * Computes once: per-row integer shift and the ten interpolation weights of the theta half shift
+ * (p_j and dt never change), sin/cos tables of the nodes (L210), ring force/potential tables.
+ * Boundary defaults follow BASELINE.json: x periodic (zero extension for SHEET), p zero extension.
+ * f is zero until vlasov_upload.  Errors: EINVAL (arguments), ECUDA (no device / CUDA failure), ENOMEM.
+ */
+int vlasov_init(int model, const int grid[2], const double domain[4], double dt);
+
+/* Change a parameter (VLASOV_KEY_*) after vlasov_init and before the first upload/attach/step. */
+int vlasov_set_param(int key, double value);
+
+/* Bytes of ONE copy of f (Ntheta*Np*sizeof(element)) and of the work buffer vlasov_attach expects
+ * (second copy of f for the out-of-place passes + per-band column sums).  0 if not initialised. */
+size_t vlasov_state_bytes(void);
+size_t vlasov_workspace_bytes(void);
+
+/*
+ * Hand the library caller-owned device memory and a stream (all three stay owned by the caller):
+ *   f_dev       device, vlasov_state_bytes() bytes, row-major [Np][Ntheta]; its content is taken as f(t)
+ *   work_dev    device, >= vlasov_workspace_bytes() bytes, 256-byte aligned, content irrelevant
+ *   cuda_stream a cudaStream_t cast to void* (NULL = legacy default stream)
+ * If vlasov_attach is never called the library allocates both buffers itself at the first upload.
+ * After a step the current f lives in EITHER f_dev or the first vlasov_state_bytes() of work_dev (the passes
+ * ping-pong); vlasov_state_ptr tells which.  Errors: EINVAL, ENOMEM (work_bytes too small).
+ */
+int vlasov_attach(void* f_dev, void* work_dev, size_t work_bytes, void* cuda_stream);
+
+/* Device pointer of the current f (one of the two buffers above). */
+int vlasov_state_ptr(void** f_dev_out);
+
+/* Host -> device copy of a full state (row-major [Np][Ntheta], element type per PRECISION); sets t = 0.
+ * Device -> host copy of the current state (blocks until done).  Together: checkpoint / resume. */
+int vlasov_upload(const void* f_host);
+int vlasov_download(void* f_host);
+
+/*
+ * Enqueue n >= 1 Strang steps (asynchronous).  The state afterwards is f(t0 + n dt) as n single steps give
+ * it: theta(dt/2), [force, p(dt), theta(dt/2) theta(dt/2)] x (n-1), force, p(dt), theta(dt/2), where the
+ * two adjacent half shifts are evaluated one after the other inside one kernel (unless FUSE = 0 or
+ * HISTORY = 1).  Errors: EINVAL (n <= 0), ENOTINIT, ECUDA.
+ */
+int vlasov_step(int n);
+
+/* One stage on its own (VLASOV_SUB_*); used by the parity tests.  Does not advance t. */
+int vlasov_substep(int which);
+
+/* Copy a device vector (VLASOV_VEC_*) of Ntheta doubles to / from host memory (blocking). */
+int vlasov_get_vector(int which, double* host_out);
+int vlasov_set_vector(int which, const double* host_in);
+
+/*
+ * out (host, 8 doubles) = {t, mass, P, K, U, M_x, M_y, E = K + U} of the current state, rectangle rule:
+ *   mass = dx dp sum f, P = dx dp sum p f, K = dx dp sum p^2/2 f, (M_x, M_y) eq (8),
+ *   U = (1/2) int rho phi:  HMF (mass^2 - M_x^2 - M_y^2)/2;  ring  phi = dtheta sum_m V(m dtheta) rho_{i-m};
+ *   sheet  phi = dx sum_k |x_i - x_k| rho_k;  FREE 0.
+ * Runs one extra read pass over f; blocks until done.
+ */
+int vlasov_moments(double out[8]);
+
+/* With HISTORY = 1: copy the records {t, mass, P, K, U, M_x, M_y, E} written after each of the steps of
+ * the LAST vlasov_step call into out (host, 8*max_steps doubles); returns the number of records copied
+ * (>= 0) or a negative code. */
+int vlasov_history(double* out, int max_steps);
+
+/* Block until everything enqueued so far has finished. */
+int vlasov_sync(void);
+
+/* Number of kernels the library has launched since vlasov_init (for bench.py's gpu_launches). */
+int vlasov_launch_count(unsigned long long* out);
+
+/* Fill out[0..n) (host) with implementation facts for reports: {SM count, theta-kernel CTAs, p-kernel CTAs,
+ * bands, warps per theta CTA (2-shift), warps per theta CTA (1-shift)}; returns how many were written. */
+int vlasov_info(double* out, int n);
+
+void vlasov_free(void);
+const char* vlasov_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* VLASOV_B200_H */

@@ -1,0 +1,278 @@
+"""ctypes binding of ``csrc/libvlasov_b200.so`` (the C ABI of include/vlasov.h).
+
+Argument marshalling only: every step of the path runs in the CUDA kernels behind the ABI.  The module-level
+functions carry the C names (``vlasov_init`` ...); ``Vlasov`` is a convenience handle that also owns the torch
+tensors used as device memory (torch = device memory + stream, nothing else).
+
+There is no CPU fallback: importing works without a GPU (so that the symbol table can be checked), but every
+call that needs the device raises ``VlasovError`` if the library is missing or CUDA is unavailable.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import numpy as np
+
+from . import build as _build
+
+MODEL_FREE, MODEL_HMF, MODEL_RING, MODEL_SHEET = 0, 1, 2, 3
+KEY_EPS, KEY_PRECISION, KEY_BC_X, KEY_BC_P, KEY_HISTORY, KEY_FUSE = 1, 2, 3, 4, 5, 6
+KEY_TUNE_NW1, KEY_TUNE_NW2, KEY_TUNE_BANDS, KEY_TUNE_PSEG, KEY_TUNE_PTX = 101, 102, 103, 104, 105
+SUB_THETA_HALF, SUB_FORCE, SUB_P_FULL, SUB_THETA_TWICE = 0, 1, 2, 3
+VEC_RHO, VEC_FORCE = 0, 1
+OK, EINVAL, ENOTINIT, ECUDA, ENOMEM = 0, -1, -2, -3, -4
+
+EXPORTS = (
+    "vlasov_init", "vlasov_set_param", "vlasov_state_bytes", "vlasov_workspace_bytes", "vlasov_attach",
+    "vlasov_state_ptr", "vlasov_upload", "vlasov_download", "vlasov_step", "vlasov_substep",
+    "vlasov_get_vector", "vlasov_set_vector", "vlasov_moments", "vlasov_history", "vlasov_sync",
+    "vlasov_launch_count", "vlasov_info", "vlasov_free", "vlasov_last_error",
+)
+
+
+class VlasovError(RuntimeError):
+    def __init__(self, code: int, what: str, msg: str):
+        super().__init__("%s failed with code %d: %s" % (what, code, msg))
+        self.code = code
+
+
+_lib = None
+_dp = ctypes.POINTER(ctypes.c_double)
+
+
+def library_path() -> str:
+    return _build.LIB
+
+
+def load(build_if_missing: bool = True):
+    """dlopen the CUDA library (building it with nvcc if it is missing or stale)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = _build.LIB
+    if build_if_missing:
+        try:
+            path = _build.build_library()
+        except Exception as exc:  # stale but present is still loadable; missing is fatal
+            if not os.path.exists(path):
+                raise VlasovError(ECUDA, "load", "CUDA library missing and nvcc build failed: %s" % exc)
+    if not os.path.exists(path):
+        raise VlasovError(ECUDA, "load", "%s not found (no CPU fallback exists)" % path)
+    lib = ctypes.CDLL(path)
+    vp, ci, cd, sz = ctypes.c_void_p, ctypes.c_int, ctypes.c_double, ctypes.c_size_t
+    sig = {
+        "vlasov_init": (ci, [ci, ctypes.POINTER(ci), _dp, cd]),
+        "vlasov_set_param": (ci, [ci, cd]),
+        "vlasov_state_bytes": (sz, []),
+        "vlasov_workspace_bytes": (sz, []),
+        "vlasov_attach": (ci, [vp, vp, sz, vp]),
+        "vlasov_state_ptr": (ci, [ctypes.POINTER(vp)]),
+        "vlasov_upload": (ci, [vp]),
+        "vlasov_download": (ci, [vp]),
+        "vlasov_step": (ci, [ci]),
+        "vlasov_substep": (ci, [ci]),
+        "vlasov_get_vector": (ci, [ci, _dp]),
+        "vlasov_set_vector": (ci, [ci, _dp]),
+        "vlasov_moments": (ci, [_dp]),
+        "vlasov_history": (ci, [_dp, ci]),
+        "vlasov_sync": (ci, []),
+        "vlasov_launch_count": (ci, [ctypes.POINTER(ctypes.c_ulonglong)]),
+        "vlasov_info": (ci, [_dp, ci]),
+        "vlasov_free": (None, []),
+        "vlasov_last_error": (ctypes.c_char_p, []),
+    }
+    for name, (res, args) in sig.items():
+        fn = getattr(lib, name)
+        fn.restype = res
+        fn.argtypes = args
+    _lib = lib
+    return lib
+
+
+def _chk(rc: int, what: str) -> int:
+    if rc < 0:
+        raise VlasovError(rc, what, (load().vlasov_last_error() or b"").decode())
+    return rc
+
+
+# ---- the C names ------------------------------------------------------------------------------------------
+
+def vlasov_init(model: int, grid, domain, dt: float) -> None:
+    g = (ctypes.c_int * 2)(int(grid[0]), int(grid[1]))
+    d = (ctypes.c_double * 4)(*[float(x) for x in domain])
+    _chk(load().vlasov_init(int(model), g, d, float(dt)), "vlasov_init")
+
+
+def vlasov_set_param(key: int, value: float) -> None:
+    _chk(load().vlasov_set_param(int(key), float(value)), "vlasov_set_param")
+
+
+def vlasov_state_bytes() -> int:
+    return int(load().vlasov_state_bytes())
+
+
+def vlasov_workspace_bytes() -> int:
+    return int(load().vlasov_workspace_bytes())
+
+
+def vlasov_attach(f_dev_ptr: int, work_dev_ptr: int, work_bytes: int, cuda_stream: int) -> None:
+    _chk(load().vlasov_attach(ctypes.c_void_p(f_dev_ptr), ctypes.c_void_p(work_dev_ptr), int(work_bytes),
+                              ctypes.c_void_p(cuda_stream)), "vlasov_attach")
+
+
+def vlasov_state_ptr() -> int:
+    out = ctypes.c_void_p()
+    _chk(load().vlasov_state_ptr(ctypes.byref(out)), "vlasov_state_ptr")
+    return int(out.value or 0)
+
+
+def vlasov_upload(f_host: np.ndarray) -> None:
+    assert f_host.flags["C_CONTIGUOUS"]
+    _chk(load().vlasov_upload(ctypes.c_void_p(f_host.ctypes.data)), "vlasov_upload")
+
+
+def vlasov_upload_ptr(host_ptr: int) -> None:
+    _chk(load().vlasov_upload(ctypes.c_void_p(host_ptr)), "vlasov_upload")
+
+
+def vlasov_download(f_host: np.ndarray) -> None:
+    assert f_host.flags["C_CONTIGUOUS"] and f_host.flags["WRITEABLE"]
+    _chk(load().vlasov_download(ctypes.c_void_p(f_host.ctypes.data)), "vlasov_download")
+
+
+def vlasov_download_ptr(host_ptr: int) -> None:
+    _chk(load().vlasov_download(ctypes.c_void_p(host_ptr)), "vlasov_download")
+
+
+def vlasov_step(n: int = 1) -> None:
+    _chk(load().vlasov_step(int(n)), "vlasov_step")
+
+
+def vlasov_substep(which: int) -> None:
+    _chk(load().vlasov_substep(int(which)), "vlasov_substep")
+
+
+def vlasov_get_vector(which: int, n: int) -> np.ndarray:
+    out = np.empty(n, dtype=np.float64)
+    _chk(load().vlasov_get_vector(int(which), out.ctypes.data_as(_dp)), "vlasov_get_vector")
+    return out
+
+
+def vlasov_set_vector(which: int, v) -> None:
+    v = np.ascontiguousarray(v, dtype=np.float64)
+    _chk(load().vlasov_set_vector(int(which), v.ctypes.data_as(_dp)), "vlasov_set_vector")
+
+
+def vlasov_moments() -> np.ndarray:
+    out = np.empty(8, dtype=np.float64)
+    _chk(load().vlasov_moments(out.ctypes.data_as(_dp)), "vlasov_moments")
+    return out
+
+
+def vlasov_history(max_steps: int) -> np.ndarray:
+    out = np.empty((max(int(max_steps), 1), 8), dtype=np.float64)
+    n = _chk(load().vlasov_history(out.ctypes.data_as(_dp), int(max_steps)), "vlasov_history")
+    return out[:n]
+
+
+def vlasov_sync() -> None:
+    _chk(load().vlasov_sync(), "vlasov_sync")
+
+
+def vlasov_launch_count() -> int:
+    out = ctypes.c_ulonglong(0)
+    _chk(load().vlasov_launch_count(ctypes.byref(out)), "vlasov_launch_count")
+    return int(out.value)
+
+
+def vlasov_info() -> dict:
+    buf = np.zeros(16, dtype=np.float64)
+    n = _chk(load().vlasov_info(buf.ctypes.data_as(_dp), 16), "vlasov_info")
+    names = ["sm_count", "theta2_ctas", "p_ctas", "theta2_bands", "theta2_warps", "theta1_warps", "theta1_ctas",
+             "p_seg_len", "p_threads"]
+    return {k: int(buf[i]) for i, k in enumerate(names[:n])}
+
+
+def vlasov_free() -> None:
+    load().vlasov_free()
+
+
+# ---- convenience handle -----------------------------------------------------------------------------------
+
+class Vlasov:
+    """Singleton solver handle.  ``f`` arrays are [Np, Ntheta], theta fastest.
+
+    Device memory comes from torch (``torch.empty`` on ``cuda``) and is handed over with ``vlasov_attach``
+    together with torch's current stream; nothing else of torch is used.
+    """
+
+    def __init__(self, model: int, grid, domain, dt: float, precision: int = 64, device: str = "cuda:0",
+                 attach: bool = True, **params):
+        import torch
+
+        if not torch.cuda.is_available():
+            raise VlasovError(ECUDA, "Vlasov", "no CUDA device: this library has no CPU fallback")
+        self.torch = torch
+        self.device = torch.device(device)
+        torch.cuda.set_device(self.device)
+        self.ntheta, self.np_ = int(grid[0]), int(grid[1])
+        self.dtype = np.float64 if precision == 64 else np.float32
+        vlasov_init(model, grid, domain, dt)
+        if precision != 64:
+            vlasov_set_param(KEY_PRECISION, precision)
+        keys = {"eps": KEY_EPS, "bc_x": KEY_BC_X, "bc_p": KEY_BC_P, "history": KEY_HISTORY, "fuse": KEY_FUSE,
+                "tune_nw1": KEY_TUNE_NW1, "tune_nw2": KEY_TUNE_NW2, "tune_bands": KEY_TUNE_BANDS,
+                "tune_pseg": KEY_TUNE_PSEG, "tune_ptx": KEY_TUNE_PTX}
+        for k, v in params.items():
+            vlasov_set_param(keys[k], float(v))
+        self.f_dev = self.work_dev = None
+        if attach:
+            tdt = torch.float64 if precision == 64 else torch.float32
+            self.f_dev = torch.zeros((self.np_, self.ntheta), dtype=tdt, device=self.device)
+            self.work_dev = torch.empty(vlasov_workspace_bytes() + 256, dtype=torch.uint8, device=self.device)
+            wp = (self.work_dev.data_ptr() + 255) & ~255
+            self.stream = torch.cuda.current_stream(self.device)
+            vlasov_attach(self.f_dev.data_ptr(), wp, vlasov_workspace_bytes(), self.stream.cuda_stream)
+
+    def upload(self, f) -> None:
+        f = np.ascontiguousarray(f, dtype=self.dtype)
+        assert f.shape == (self.np_, self.ntheta)
+        vlasov_upload(f)
+        vlasov_sync()  # f may be a temporary: do not let it die under the asynchronous copy
+
+    def download(self) -> np.ndarray:
+        out = np.empty((self.np_, self.ntheta), dtype=self.dtype)
+        vlasov_download(out)
+        return out
+
+    def step(self, n: int = 1) -> None:
+        vlasov_step(n)
+
+    def substep(self, which: int) -> None:
+        vlasov_substep(which)
+
+    def density(self) -> np.ndarray:
+        return vlasov_get_vector(VEC_RHO, self.ntheta)
+
+    def force(self) -> np.ndarray:
+        return vlasov_get_vector(VEC_FORCE, self.ntheta)
+
+    def set_force(self, F) -> None:
+        vlasov_set_vector(VEC_FORCE, F)
+
+    def moments(self) -> np.ndarray:
+        return vlasov_moments()
+
+    def history(self, n: int) -> np.ndarray:
+        return vlasov_history(n)
+
+    def sync(self) -> None:
+        vlasov_sync()
+
+    def info(self) -> dict:
+        return vlasov_info()
+
+    def close(self) -> None:
+        vlasov_free()
+        self.f_dev = self.work_dev = None

@@ -1,0 +1,673 @@
+// vlasov_api.cu -- host side of the C ABI declared in include/vlasov.h.
+//
+// Singleton context, tables computed once on the host (PAPER.md L210 stores sin/cos of the nodes once; the
+// per-row shift of the theta half step is constant for the whole run because p_j and dt never change),
+// launch sequencing of one Strang step (L71-L87):
+//     theta(dt/2) -> rho -> F -> p(dt) -> theta(dt/2)
+// with the trailing and leading half shifts of consecutive steps merged into one pass (a6).
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include <vector>
+
+#include "../../include/vlasov.h"
+#include "vlasov_kernels.cuh"
+
+namespace {
+
+constexpr int R_THETA = 9;       // consecutive outputs per lane in the theta kernel (odd: bank-conflict-free)
+constexpr int KEY_TUNE_NW1 = 101, KEY_TUNE_NW2 = 102, KEY_TUNE_BANDS = 103, KEY_TUNE_PSEG = 104,
+              KEY_TUNE_PTX = 105;
+
+thread_local char g_err[512] = "";
+
+struct Ctx {
+    bool ready = false, prepared = false, cuda_failed = false;
+    int model = 0, ntheta = 0, np = 0;
+    double xmin = 0, xmax = 0, pmin = 0, pmax = 0, dt = 0, eps = 0.01, t = 0;
+    int bc_x = 0, bc_p = 1, prec = 64;
+    bool history = false, fuse = true;
+    cudaStream_t stream = nullptr;
+    int sm_count = 148;
+
+    void* f[2] = {nullptr, nullptr};  // ping-pong copies of the state
+    int cur = 0;
+    bool own_f = false, own_work = false, attached = false;
+    void* work = nullptr;
+    double* colpart = nullptr;  // inside work
+    int cp_bands = 0;
+
+    // small library-owned device buffers
+    int* srow = nullptr;
+    double *wrow = nullptr, *cos_t = nullptr, *sin_t = nullptr, *ringK = nullptr, *ringV = nullptr;
+    double *rho = nullptr, *force = nullptr, *rho_m = nullptr, *phi = nullptr, *mpart = nullptr, *pkpart = nullptr,
+           *mom_dev = nullptr, *hist = nullptr;
+    int hist_cap = 0, hist_count = 0;
+
+    // launch configuration
+    int nw[3] = {0, 6, 6};         // warps per theta CTA for NSTAGE = 1, 2
+    int nchunks[3] = {0, 0, 0};
+    int nbands[3] = {0, 0, 0}, rpb[3] = {0, 0, 0};
+    int mbands = 0, mrpb = 0;      // moments pass
+    int p_tx = 128, p_seg = 0, p_nseg = 0;
+    int tune_nw1 = 0, tune_nw2 = 0, tune_bands = 0, tune_pseg = 0, tune_ptx = 0;
+    unsigned long long launches = 0;
+};
+
+Ctx G;
+
+int fail(int code, const char* fmt, const char* a = "") {
+    snprintf(g_err, sizeof(g_err), fmt, a);
+    return code;
+}
+
+#define CU(call)                                                                                 \
+    do {                                                                                         \
+        cudaError_t e_ = (call);                                                                 \
+        if (e_ != cudaSuccess) {                                                                 \
+            G.cuda_failed = true;                                                                \
+            snprintf(g_err, sizeof(g_err), "%s failed: %s (%s:%d)", #call, cudaGetErrorString(e_), \
+                     __FILE__, __LINE__);                                                        \
+            return VLASOV_ECUDA;                                                                 \
+        }                                                                                        \
+    } while (0)
+
+#define LAUNCH_CHECK()                 \
+    do {                               \
+        G.launches++;                  \
+        CU(cudaGetLastError());        \
+    } while (0)
+
+size_t elem_bytes() { return G.prec == 32 ? 4 : 8; }
+size_t state_bytes() { return (size_t)G.ntheta * (size_t)G.np * elem_bytes(); }
+size_t round256(size_t b) { return (b + 255) & ~(size_t)255; }
+int cdiv(int a, int b) { return (a + b - 1) / b; }
+
+void free_small() {
+    void* ptrs[] = {G.srow, G.wrow, G.cos_t, G.sin_t, G.ringK, G.ringV, G.rho, G.force, G.rho_m,
+                    G.phi,  G.mpart, G.pkpart, G.mom_dev, G.hist};
+    for (void* p : ptrs)
+        if (p) cudaFree(p);
+    G.srow = nullptr;
+    G.wrow = G.cos_t = G.sin_t = G.ringK = G.ringV = G.rho = G.force = G.rho_m = G.phi = G.mpart = G.pkpart =
+        G.mom_dev = G.hist = nullptr;
+    G.hist_cap = G.hist_count = 0;
+}
+
+void free_big() {
+    if (G.own_f && G.f[0]) cudaFree(G.f[0]);
+    if (G.own_work && G.work) cudaFree(G.work);
+    G.f[0] = G.f[1] = G.work = nullptr;
+    G.colpart = nullptr;
+    G.own_f = G.own_work = G.attached = false;
+    G.cur = 0;
+}
+
+template <typename T, int NSTAGE>
+size_t theta_smem_bytes(int nw) {
+    constexpr int LANES = (NSTAGE == 2) ? 31 : 32;
+    const int chunk = nw * LANES * R_THETA;
+    const int lenA = chunk + 9 * NSTAGE;
+    return (size_t)(((lenA + 1) & ~1) + chunk) * sizeof(T);
+}
+
+// choose warps per CTA so that the ragged last chunk wastes little; bands so that one wave fills the GPU
+template <typename T, int NSTAGE>
+int configure_theta(int tune_nw) {
+    constexpr int LANES = (NSTAGE == 2) ? 31 : 32;
+    const int tile = LANES * R_THETA;
+    const int tiles = cdiv(G.ntheta, tile);
+    int nw = 0;
+    if (tune_nw > 0) {
+        nw = tune_nw;
+    } else {
+        int best_nw = 1, best_waste = 1 << 30;
+        for (int c = 8; c >= 1; --c) {
+            const int waste = cdiv(tiles, c) * c - tiles;
+            if (waste * 25 <= tiles) {  // <= 4 %
+                nw = c;
+                break;
+            }
+            if (waste < best_waste) {
+                best_waste = waste;
+                best_nw = c;
+            }
+        }
+        if (nw == 0) nw = best_nw;
+    }
+    if (nw > 12) nw = 12;
+    G.nw[NSTAGE] = nw;
+    G.nchunks[NSTAGE] = cdiv(tiles, nw);
+    auto kern = vl::theta_sweep_kernel<T, NSTAGE, R_THETA>;
+    const size_t smem = theta_smem_bytes<T, NSTAGE>(nw);
+    CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    int occ = 1;
+    CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, nw * 32, smem));
+    if (occ < 1) occ = 1;
+    int bands = G.tune_bands > 0 ? G.tune_bands : (G.sm_count * occ) / G.nchunks[NSTAGE];
+    if (bands < 1) bands = 1;
+    if (bands > G.np) bands = G.np;
+    G.rpb[NSTAGE] = cdiv(G.np, bands);
+    G.nbands[NSTAGE] = cdiv(G.np, G.rpb[NSTAGE]);
+    return VLASOV_OK;
+}
+
+template <typename T>
+int configure_all() {
+    int rc;
+    if ((rc = configure_theta<T, 1>(G.tune_nw1)) != 0) return rc;
+    if ((rc = configure_theta<T, 2>(G.tune_nw2)) != 0) return rc;
+    // p shift: 128 adjacent columns per CTA; segments so that a bit more than one wave of CTAs exists
+    G.p_tx = G.tune_ptx > 0 ? G.tune_ptx : 128;
+    if (G.p_tx > 256) G.p_tx = 256;
+    int occ = 1;
+    CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, vl::p_sweep_kernel<T>, G.p_tx, 0));
+    if (occ < 1) occ = 1;
+    const int colblocks = cdiv(G.ntheta, G.p_tx);
+    int nseg = cdiv(G.sm_count * occ, colblocks);
+    if (nseg < 1) nseg = 1;
+    int seg = G.tune_pseg > 0 ? G.tune_pseg : cdiv(G.np, nseg);
+    if (seg < 40 && G.tune_pseg <= 0) seg = 40;  // keep the 9-row halo re-read below ~20 %
+    if (seg > G.np) seg = G.np;
+    G.p_seg = seg;
+    G.p_nseg = cdiv(G.np, seg);
+    // moments pass
+    G.mbands = cdiv(G.sm_count * 8, cdiv(G.ntheta, 256));
+    if (G.mbands > G.np) G.mbands = G.np;
+    if (G.mbands < 1) G.mbands = 1;
+    G.mrpb = cdiv(G.np, G.mbands);
+    G.mbands = cdiv(G.np, G.mrpb);
+    return VLASOV_OK;
+}
+
+int max_bands_bound() {
+    // upper bound of every band count configure_all() can pick: one band per slot of the GPU, or per row
+    int b = G.sm_count * 32;
+    if (G.tune_bands > b) b = G.tune_bands;
+    if (b > G.np) b = G.np;
+    return b < 1 ? 1 : b;
+}
+
+size_t workspace_bytes() {
+    return round256(state_bytes()) + round256((size_t)max_bands_bound() * G.ntheta * sizeof(double));
+}
+
+int prepare() {
+    if (G.prepared) return VLASOV_OK;
+    const int nt = G.ntheta, np = G.np;
+    const double dx = (G.xmax - G.xmin) / (double)nt, dp = (G.pmax - G.pmin) / (double)np;
+    const double tau = 0.5 * G.dt;
+
+    // per-row shift of one half step: displacement p_j tau (eq (9)), u = -disp/dx cells
+    std::vector<int> srow(np);
+    std::vector<double> wrow((size_t)np * 10);
+    for (int j = 0; j < np; ++j) {
+        const double p = G.pmin + (double)j * dp;
+        const double disp = p * tau;
+        double sf, a;
+        vl::split_shift(-disp / dx, &sf, &a);
+        if (G.bc_x == vl::BC_PERIODIC) {
+            sf = fmod(sf, (double)nt);
+        } else {
+            const double lim = (double)nt + 64.0;
+            sf = fmin(fmax(sf, -lim), lim);
+        }
+        srow[j] = (int)sf;
+        vl::spline_fd8_weights(a, &wrow[(size_t)j * 10]);
+    }
+    std::vector<double> ct(nt), st(nt);
+    for (int i = 0; i < nt; ++i) {
+        const double th = G.xmin + (double)i * dx;
+        ct[i] = cos(th);
+        st[i] = sin(th);
+    }
+    CU(cudaMalloc(&G.srow, sizeof(int) * np));
+    CU(cudaMalloc(&G.wrow, sizeof(double) * np * 10));
+    CU(cudaMalloc(&G.cos_t, sizeof(double) * nt));
+    CU(cudaMalloc(&G.sin_t, sizeof(double) * nt));
+    CU(cudaMemcpy(G.srow, srow.data(), sizeof(int) * np, cudaMemcpyHostToDevice));
+    CU(cudaMemcpy(G.wrow, wrow.data(), sizeof(double) * np * 10, cudaMemcpyHostToDevice));
+    CU(cudaMemcpy(G.cos_t, ct.data(), sizeof(double) * nt, cudaMemcpyHostToDevice));
+    CU(cudaMemcpy(G.sin_t, st.data(), sizeof(double) * nt, cudaMemcpyHostToDevice));
+    if (G.model == VLASOV_MODEL_RING) {
+        // eq (2) (L33-L35): V(x) = -1/(sqrt2 sqrt(1 - cos x + eps)); K = -dV/dx; 1 - cos x = 2 sin^2(x/2)
+        std::vector<double> K(nt), V(nt);
+        for (int m = 0; m < nt; ++m) {
+            const double x = (double)m * dx;
+            const double h = sin(0.5 * x);
+            const double q = 2.0 * h * h + G.eps;
+            V[m] = -1.0 / (sqrt(2.0) * sqrt(q));
+            K[m] = (m == 0) ? 0.0 : -sin(x) / (2.0 * sqrt(2.0) * q * sqrt(q));
+        }
+        CU(cudaMalloc(&G.ringK, sizeof(double) * nt));
+        CU(cudaMalloc(&G.ringV, sizeof(double) * nt));
+        CU(cudaMemcpy(G.ringK, K.data(), sizeof(double) * nt, cudaMemcpyHostToDevice));
+        CU(cudaMemcpy(G.ringV, V.data(), sizeof(double) * nt, cudaMemcpyHostToDevice));
+    }
+    CU(cudaMalloc(&G.rho, sizeof(double) * nt));
+    CU(cudaMalloc(&G.force, sizeof(double) * nt));
+    CU(cudaMalloc(&G.rho_m, sizeof(double) * nt));
+    CU(cudaMalloc(&G.phi, sizeof(double) * nt));
+    CU(cudaMemset(G.rho, 0, sizeof(double) * nt));
+    CU(cudaMemset(G.force, 0, sizeof(double) * nt));
+    CU(cudaMalloc(&G.mpart, sizeof(double) * 2 * cdiv(nt, 256)));
+    CU(cudaMalloc(&G.mom_dev, sizeof(double) * 8));
+
+    int rc = (G.prec == 32) ? configure_all<float>() : configure_all<double>();
+    if (rc != 0) return rc;
+    CU(cudaMalloc(&G.pkpart, sizeof(double) * 2 * (size_t)G.mbands * cdiv(nt, 256)));
+    G.cp_bands = max_bands_bound();
+    G.prepared = true;
+    return VLASOV_OK;
+}
+
+int ensure_buffers() {
+    int rc = prepare();
+    if (rc != 0) return rc;
+    if (G.f[0] != nullptr) return VLASOV_OK;
+    // never attached: the library owns both copies
+    CU(cudaMalloc(&G.f[0], round256(state_bytes())));
+    G.own_f = true;
+    CU(cudaMalloc(&G.work, workspace_bytes()));
+    G.own_work = true;
+    G.f[1] = G.work;
+    G.colpart = reinterpret_cast<double*>(static_cast<char*>(G.work) + round256(state_bytes()));
+    CU(cudaMemsetAsync(G.f[0], 0, state_bytes(), G.stream));
+    G.cur = 0;
+    return VLASOV_OK;
+}
+
+// ---- launches -----------------------------------------------------------------------------------
+
+template <typename T, int NSTAGE>
+int launch_theta(bool want_colsums) {
+    vl::ThetaArgs<T> a;
+    a.fin = static_cast<const T*>(G.f[G.cur]);
+    a.fout = static_cast<T*>(G.f[G.cur ^ 1]);
+    a.srow = G.srow;
+    a.wrow = G.wrow;
+    a.colpart = want_colsums ? G.colpart : nullptr;
+    a.ntheta = G.ntheta;
+    a.np = G.np;
+    a.bc_x = G.bc_x;
+    a.rows_per_band = G.rpb[NSTAGE];
+    const int nw = G.nw[NSTAGE];
+    dim3 grid(G.nchunks[NSTAGE], G.nbands[NSTAGE]);
+    vl::theta_sweep_kernel<T, NSTAGE, R_THETA>
+        <<<grid, nw * 32, theta_smem_bytes<T, NSTAGE>(nw), G.stream>>>(a);
+    LAUNCH_CHECK();
+    G.cur ^= 1;
+    return VLASOV_OK;
+}
+
+int theta_pass(int nstage, bool want_colsums) {
+    if (G.prec == 32)
+        return nstage == 2 ? launch_theta<float, 2>(want_colsums) : launch_theta<float, 1>(want_colsums);
+    return nstage == 2 ? launch_theta<double, 2>(want_colsums) : launch_theta<double, 1>(want_colsums);
+}
+
+template <typename T>
+int launch_p() {
+    vl::PArgs<T> a;
+    a.fin = static_cast<const T*>(G.f[G.cur]);
+    a.fout = static_cast<T*>(G.f[G.cur ^ 1]);
+    a.force = G.force;
+    a.ntheta = G.ntheta;
+    a.np = G.np;
+    a.bc_p = G.bc_p;
+    a.seg_len = G.p_seg;
+    a.dt = G.dt;
+    a.dp = (G.pmax - G.pmin) / (double)G.np;
+    dim3 grid(cdiv(G.ntheta, G.p_tx), G.p_nseg);
+    vl::p_sweep_kernel<T><<<grid, G.p_tx, 0, G.stream>>>(a);
+    LAUNCH_CHECK();
+    G.cur ^= 1;
+    return VLASOV_OK;
+}
+
+int p_pass() { return G.prec == 32 ? launch_p<float>() : launch_p<double>(); }
+
+// rho (and for HMF the moment partials) from the column sums left in colpart by `bands` bands
+int rho_from_colpart(int bands, double* rho_out, bool hmf_partials) {
+    const double dp = (G.pmax - G.pmin) / (double)G.np;
+    vl::rho_reduce_kernel<<<cdiv(G.ntheta, 256), 256, 0, G.stream>>>(
+        G.colpart, bands, G.ntheta, dp, rho_out, G.cos_t, G.sin_t, hmf_partials ? G.mpart : nullptr);
+    LAUNCH_CHECK();
+    return VLASOV_OK;
+}
+
+int force_from_rho() {
+    const int nt = G.ntheta;
+    const double dx = (G.xmax - G.xmin) / (double)nt;
+    switch (G.model) {
+        case VLASOV_MODEL_HMF:
+            vl::force_hmf_kernel<<<cdiv(nt, 256), 256, 0, G.stream>>>(G.mpart, cdiv(nt, 256), dx, G.cos_t, G.sin_t,
+                                                                      nt, G.force, nullptr);
+            break;
+        case VLASOV_MODEL_RING:
+            vl::ring_convolve_kernel<<<cdiv(nt, 256), 256, 0, G.stream>>>(G.ringK, G.rho, nt, dx, G.force);
+            break;
+        case VLASOV_MODEL_SHEET:
+            vl::sheet_scan_kernel<<<1, 1024, 0, G.stream>>>(G.rho, nt, dx, 0, G.force);
+            break;
+        default:
+            vl::fill_zero_kernel<<<cdiv(nt, 256), 256, 0, G.stream>>>(G.force, nt);
+            break;
+    }
+    LAUNCH_CHECK();
+    return VLASOV_OK;
+}
+
+template <typename T>
+int launch_moments_pass() {
+    const double dp = (G.pmax - G.pmin) / (double)G.np;
+    dim3 grid(cdiv(G.ntheta, 256), G.mbands);
+    vl::moments_pass_kernel<T><<<grid, 256, 0, G.stream>>>(static_cast<const T*>(G.f[G.cur]), G.ntheta, G.np,
+                                                           G.mrpb, G.pmin, dp, G.colpart, G.pkpart);
+    LAUNCH_CHECK();
+    return VLASOV_OK;
+}
+
+int moments_pass() { return G.prec == 32 ? launch_moments_pass<float>() : launch_moments_pass<double>(); }
+
+int moments_async(double* dev_out8) {
+    int rc;
+    const int nt = G.ntheta;
+    const double dx = (G.xmax - G.xmin) / (double)nt, dp = (G.pmax - G.pmin) / (double)G.np;
+    if ((rc = moments_pass()) != 0) return rc;
+    if ((rc = rho_from_colpart(G.mbands, G.rho_m, false)) != 0) return rc;
+    const double* phi = nullptr;
+    if (G.model == VLASOV_MODEL_RING) {
+        vl::ring_convolve_kernel<<<cdiv(nt, 256), 256, 0, G.stream>>>(G.ringV, G.rho_m, nt, dx, G.phi);
+        LAUNCH_CHECK();
+        phi = G.phi;
+    } else if (G.model == VLASOV_MODEL_SHEET) {
+        vl::sheet_scan_kernel<<<1, 1024, 0, G.stream>>>(G.rho_m, nt, dx, 1, G.phi);
+        LAUNCH_CHECK();
+        phi = G.phi;
+    }
+    vl::moments_final_kernel<<<1, 1024, 0, G.stream>>>(G.rho_m, phi, nt, G.pkpart, G.mbands * cdiv(nt, 256), G.cos_t,
+                                                       G.sin_t, dx, dp, G.model, G.t, dev_out8);
+    LAUNCH_CHECK();
+    return VLASOV_OK;
+}
+
+int check_ready() {
+    if (!G.ready) return fail(VLASOV_ENOTINIT, "vlasov_init has not been called");
+    if (G.cuda_failed) return VLASOV_ECUDA;
+    return VLASOV_OK;
+}
+
+}  // namespace
+
+// ---- exported -----------------------------------------------------------------------------------
+
+extern "C" {
+
+const char* vlasov_last_error(void) { return g_err; }
+
+void vlasov_free(void) {
+    if (G.ready) cudaStreamSynchronize(G.stream);
+    free_small();
+    free_big();
+    G = Ctx();
+}
+
+int vlasov_init(int model, const int grid[2], const double domain[4], double dt) {
+    if (model < 0 || model > 3 || !grid || !domain) return fail(VLASOV_EINVAL, "vlasov_init: bad model or null argument");
+    if (grid[0] < 1 || grid[1] < 1) return fail(VLASOV_EINVAL, "vlasov_init: grid sizes must be >= 1");
+    if (!(domain[1] > domain[0]) || !(domain[3] > domain[2]) || !isfinite(dt))
+        return fail(VLASOV_EINVAL, "vlasov_init: empty domain or non-finite dt");
+    if ((double)grid[0] * (double)grid[1] > 4.0e9) return fail(VLASOV_EINVAL, "vlasov_init: grid too large");
+    vlasov_free();
+    int dev = 0, count = 0;
+    if (cudaGetDeviceCount(&count) != cudaSuccess || count < 1) {
+        cudaGetLastError();
+        return fail(VLASOV_ECUDA, "vlasov_init: no CUDA device (there is no CPU fallback)");
+    }
+    CU(cudaGetDevice(&dev));
+    CU(cudaDeviceGetAttribute(&G.sm_count, cudaDevAttrMultiProcessorCount, dev));
+    G.model = model;
+    G.ntheta = grid[0];
+    G.np = grid[1];
+    G.xmin = domain[0];
+    G.xmax = domain[1];
+    G.pmin = domain[2];
+    G.pmax = domain[3];
+    G.dt = dt;
+    G.bc_x = (model == VLASOV_MODEL_SHEET) ? vl::BC_ZERO : vl::BC_PERIODIC;
+    G.bc_p = vl::BC_ZERO;
+    G.ready = true;
+    g_err[0] = 0;
+    return VLASOV_OK;
+}
+
+int vlasov_set_param(int key, double value) {
+    int rc = check_ready();
+    if (rc != 0) return rc;
+    if (G.prepared) return fail(VLASOV_EINVAL, "vlasov_set_param: must precede attach/upload/step");
+    switch (key) {
+        case VLASOV_KEY_EPS:
+            if (!(value > 0.0)) return fail(VLASOV_EINVAL, "EPS must be > 0");
+            G.eps = value;
+            break;
+        case VLASOV_KEY_PRECISION:
+            if (value != 64.0 && value != 32.0) return fail(VLASOV_EINVAL, "PRECISION must be 64 or 32");
+            G.prec = (int)value;
+            break;
+        case VLASOV_KEY_BC_X:
+            if (value != 0.0 && value != 1.0) return fail(VLASOV_EINVAL, "BC_X must be 0 or 1");
+            G.bc_x = (int)value;
+            break;
+        case VLASOV_KEY_BC_P:
+            if (value != 0.0 && value != 1.0) return fail(VLASOV_EINVAL, "BC_P must be 0 or 1");
+            G.bc_p = (int)value;
+            break;
+        case VLASOV_KEY_HISTORY: G.history = (value != 0.0); break;
+        case VLASOV_KEY_FUSE: G.fuse = (value != 0.0); break;
+        case KEY_TUNE_NW1: G.tune_nw1 = (int)value; break;
+        case KEY_TUNE_NW2: G.tune_nw2 = (int)value; break;
+        case KEY_TUNE_BANDS: G.tune_bands = (int)value; break;
+        case KEY_TUNE_PSEG: G.tune_pseg = (int)value; break;
+        case KEY_TUNE_PTX: G.tune_ptx = (int)value; break;
+        default: return fail(VLASOV_EINVAL, "vlasov_set_param: unknown key");
+    }
+    return VLASOV_OK;
+}
+
+size_t vlasov_state_bytes(void) { return G.ready ? state_bytes() : 0; }
+size_t vlasov_workspace_bytes(void) { return G.ready ? workspace_bytes() : 0; }
+
+int vlasov_attach(void* f_dev, void* work_dev, size_t work_bytes, void* cuda_stream) {
+    int rc = check_ready();
+    if (rc != 0) return rc;
+    if (!f_dev || !work_dev) return fail(VLASOV_EINVAL, "vlasov_attach: null buffer");
+    if (((uintptr_t)f_dev & 15) || ((uintptr_t)work_dev & 255))
+        return fail(VLASOV_EINVAL, "vlasov_attach: f_dev must be 16-byte and work_dev 256-byte aligned");
+    if (work_bytes < workspace_bytes()) return fail(VLASOV_ENOMEM, "vlasov_attach: work buffer too small");
+    G.stream = static_cast<cudaStream_t>(cuda_stream);
+    if ((rc = prepare()) != 0) return rc;
+    free_big();
+    G.f[0] = f_dev;
+    G.work = work_dev;
+    G.f[1] = work_dev;
+    G.colpart = reinterpret_cast<double*>(static_cast<char*>(work_dev) + round256(state_bytes()));
+    G.cur = 0;
+    G.attached = true;
+    return VLASOV_OK;
+}
+
+int vlasov_state_ptr(void** out) {
+    int rc = check_ready();
+    if (rc != 0) return rc;
+    if (!out) return fail(VLASOV_EINVAL, "vlasov_state_ptr: null");
+    if ((rc = ensure_buffers()) != 0) return rc;
+    *out = G.f[G.cur];
+    return VLASOV_OK;
+}
+
+int vlasov_upload(const void* f_host) {
+    int rc = check_ready();
+    if (rc != 0) return rc;
+    if (!f_host) return fail(VLASOV_EINVAL, "vlasov_upload: null");
+    if ((rc = ensure_buffers()) != 0) return rc;
+    G.cur = 0;
+    CU(cudaMemcpyAsync(G.f[0], f_host, state_bytes(), cudaMemcpyHostToDevice, G.stream));
+    G.t = 0.0;
+    return VLASOV_OK;
+}
+
+int vlasov_download(void* f_host) {
+    int rc = check_ready();
+    if (rc != 0) return rc;
+    if (!f_host) return fail(VLASOV_EINVAL, "vlasov_download: null");
+    if ((rc = ensure_buffers()) != 0) return rc;
+    CU(cudaMemcpyAsync(f_host, G.f[G.cur], state_bytes(), cudaMemcpyDeviceToHost, G.stream));
+    CU(cudaStreamSynchronize(G.stream));
+    return VLASOV_OK;
+}
+
+int vlasov_sync(void) {
+    int rc = check_ready();
+    if (rc != 0) return rc;
+    CU(cudaStreamSynchronize(G.stream));
+    return VLASOV_OK;
+}
+
+int vlasov_step(int n) {
+    int rc = check_ready();
+    if (rc != 0) return rc;
+    if (n <= 0) return fail(VLASOV_EINVAL, "vlasov_step: n must be >= 1");
+    if ((rc = ensure_buffers()) != 0) return rc;
+    const bool hmf = (G.model == VLASOV_MODEL_HMF);
+    if (G.history) {
+        if (G.hist_cap < n) {
+            if (G.hist) CU(cudaFree(G.hist));
+            G.hist = nullptr;
+            CU(cudaMalloc(&G.hist, sizeof(double) * 8 * (size_t)n));
+            G.hist_cap = n;
+        }
+        G.hist_count = 0;
+    }
+    const bool fused = G.fuse && !G.history;
+    if (fused) {
+        if ((rc = theta_pass(1, true)) != 0) return rc;                       // eq (9)
+        for (int k = 0; k < n; ++k) {
+            if ((rc = rho_from_colpart(G.nbands[k == 0 ? 1 : 2], G.rho, hmf)) != 0) return rc;
+            if ((rc = force_from_rho()) != 0) return rc;                      // eq (10)
+            if ((rc = p_pass()) != 0) return rc;                              // eq (11)
+            if (k + 1 < n) {
+                if ((rc = theta_pass(2, true)) != 0) return rc;               // eq (12) of step k, eq (9) of k+1
+            } else {
+                if ((rc = theta_pass(1, false)) != 0) return rc;              // eq (12)
+            }
+        }
+        G.t += (double)n * G.dt;
+    } else {
+        for (int k = 0; k < n; ++k) {
+            if ((rc = theta_pass(1, true)) != 0) return rc;
+            if ((rc = rho_from_colpart(G.nbands[1], G.rho, hmf)) != 0) return rc;
+            if ((rc = force_from_rho()) != 0) return rc;
+            if ((rc = p_pass()) != 0) return rc;
+            if ((rc = theta_pass(1, false)) != 0) return rc;
+            G.t += G.dt;
+            if (G.history) {
+                if ((rc = moments_async(G.hist + 8 * (size_t)k)) != 0) return rc;
+                G.hist_count = k + 1;
+            }
+        }
+    }
+    return VLASOV_OK;
+}
+
+int vlasov_substep(int which) {
+    int rc = check_ready();
+    if (rc != 0) return rc;
+    if ((rc = ensure_buffers()) != 0) return rc;
+    switch (which) {
+        case VLASOV_SUB_THETA_HALF: return theta_pass(1, true);
+        case VLASOV_SUB_THETA_TWICE: return theta_pass(2, true);
+        case VLASOV_SUB_FORCE:
+            if ((rc = moments_pass()) != 0) return rc;
+            if ((rc = rho_from_colpart(G.mbands, G.rho, G.model == VLASOV_MODEL_HMF)) != 0) return rc;
+            return force_from_rho();
+        case VLASOV_SUB_P_FULL: return p_pass();
+        default: return fail(VLASOV_EINVAL, "vlasov_substep: unknown stage");
+    }
+}
+
+int vlasov_get_vector(int which, double* host_out) {
+    int rc = check_ready();
+    if (rc != 0) return rc;
+    if (!host_out || (which != VLASOV_VEC_RHO && which != VLASOV_VEC_FORCE))
+        return fail(VLASOV_EINVAL, "vlasov_get_vector: bad argument");
+    if ((rc = ensure_buffers()) != 0) return rc;
+    const double* src = which == VLASOV_VEC_RHO ? G.rho : G.force;
+    CU(cudaMemcpyAsync(host_out, src, sizeof(double) * G.ntheta, cudaMemcpyDeviceToHost, G.stream));
+    CU(cudaStreamSynchronize(G.stream));
+    return VLASOV_OK;
+}
+
+int vlasov_set_vector(int which, const double* host_in) {
+    int rc = check_ready();
+    if (rc != 0) return rc;
+    if (!host_in || which != VLASOV_VEC_FORCE) return fail(VLASOV_EINVAL, "vlasov_set_vector: only FORCE can be set");
+    if ((rc = ensure_buffers()) != 0) return rc;
+    CU(cudaMemcpyAsync(G.force, host_in, sizeof(double) * G.ntheta, cudaMemcpyHostToDevice, G.stream));
+    CU(cudaStreamSynchronize(G.stream));
+    return VLASOV_OK;
+}
+
+int vlasov_moments(double out[8]) {
+    int rc = check_ready();
+    if (rc != 0) return rc;
+    if (!out) return fail(VLASOV_EINVAL, "vlasov_moments: null");
+    if ((rc = ensure_buffers()) != 0) return rc;
+    if ((rc = moments_async(G.mom_dev)) != 0) return rc;
+    CU(cudaMemcpyAsync(out, G.mom_dev, sizeof(double) * 8, cudaMemcpyDeviceToHost, G.stream));
+    CU(cudaStreamSynchronize(G.stream));
+    return VLASOV_OK;
+}
+
+int vlasov_history(double* out, int max_steps) {
+    int rc = check_ready();
+    if (rc != 0) return rc;
+    if (!out || max_steps < 0) return fail(VLASOV_EINVAL, "vlasov_history: bad argument");
+    const int n = G.hist_count < max_steps ? G.hist_count : max_steps;
+    if (n > 0) {
+        CU(cudaMemcpyAsync(out, G.hist, sizeof(double) * 8 * (size_t)n, cudaMemcpyDeviceToHost, G.stream));
+        CU(cudaStreamSynchronize(G.stream));
+    }
+    return n;
+}
+
+int vlasov_launch_count(unsigned long long* out) {
+    if (!out) return fail(VLASOV_EINVAL, "vlasov_launch_count: null");
+    *out = G.launches;
+    return VLASOV_OK;
+}
+
+int vlasov_info(double* out, int n) {
+    int rc = check_ready();
+    if (rc != 0) return rc;
+    if (!out || n < 0) return fail(VLASOV_EINVAL, "vlasov_info: bad argument");
+    if ((rc = prepare()) != 0) return rc;
+    const double v[] = {(double)G.sm_count,
+                        (double)G.nchunks[2] * G.nbands[2],
+                        (double)cdiv(G.ntheta, G.p_tx) * G.p_nseg,
+                        (double)G.nbands[2],
+                        (double)G.nw[2],
+                        (double)G.nw[1],
+                        (double)G.nchunks[1] * G.nbands[1],
+                        (double)G.p_seg,
+                        (double)G.p_tx};
+    const int m = (int)(sizeof(v) / sizeof(v[0]));
+    const int k = n < m ? n : m;
+    for (int q = 0; q < k; ++q) out[q] = v[q];
+    return k;
+}
+
+}  // extern "C"

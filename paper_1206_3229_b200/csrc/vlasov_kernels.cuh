@@ -1,0 +1,605 @@
+// vlasov_kernels.cuh -- CUDA kernels (sm_100a) of the Strang semi-Lagrangian Vlasov step.
+//
+// Method: arXiv 1206.3229.  One shift of a grid line by a constant displacement evaluates the
+// cubic spline of eqs (13)-(14) (L89-L98) with f'' from the 9-point difference of eq (16) (L106-L111).
+// Substituting (16) into (13) the h^2 cancels and the value at the foot becomes a 10-tap filter
+//     f_new[i] = sum_{m=-4}^{5} w_m(a) f[i + s + m],
+//     w_m = [m==0](1-a) + [m==1] a + (A c_m + B c_{m-1})/6,  A = (1-a)^3-(1-a),  B = a^3-a,
+// with s the integer part and a in [0,1) the fractional part of -displacement/h.  The weights depend only on
+// the line (row for the theta shift, column for the p shift), never on the position along it.
+//
+// Layout (L115): f[j*Ntheta + i], theta contiguous.  No transposes (the paper's steps (i), (iii), L117-L119,
+// are not needed): the theta shift runs along the contiguous axis through shared memory, the p shift lets
+// adjacent threads own adjacent columns and march down p with a register window.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace vl {
+
+enum { BC_PERIODIC = 0, BC_ZERO = 1 };
+
+// eq (16), divided by 6 (the 1/6 of gamma, delta in eq (14)); index m+4, m = -4..4
+__host__ __device__ inline double c16_over_6(int m) {
+    switch (m < 0 ? -m : m) {
+        case 0: return (-205.0 / 72.0) / 6.0;
+        case 1: return (8.0 / 5.0) / 6.0;
+        case 2: return (-1.0 / 5.0) / 6.0;
+        case 3: return (8.0 / 315.0) / 6.0;
+        case 4: return (-1.0 / 560.0) / 6.0;
+        default: return 0.0;
+    }
+}
+
+// ten filter weights for fraction a; w[mm] multiplies f[k + mm - 4]
+__host__ __device__ inline void spline_fd8_weights(double a, double w[10]) {
+    const double al = 1.0 - a;
+    const double A = al * (al * al - 1.0);  // alpha^3 - alpha
+    const double B = a * (a * a - 1.0);     // beta^3 - beta
+#pragma unroll
+    for (int mm = 0; mm < 10; ++mm) {
+        const int m = mm - 4;
+        double v = A * c16_over_6(m) + B * c16_over_6(m - 1);
+        if (m == 0) v += al;
+        if (m == 1) v += a;
+        w[mm] = v;
+    }
+}
+
+// split u = -displacement/h into integer cell shift and fraction in [0,1)
+__host__ __device__ inline void split_shift(double u, double* s_out, double* a_out) {
+    double sf = floor(u);
+    double a = u - sf;
+    if (a >= 1.0) {  // u = -tiny: floor = -1 and u + 1 rounds to 1
+        sf += 1.0;
+        a = 0.0;
+    }
+    *s_out = sf;
+    *a_out = a;
+}
+
+__device__ __forceinline__ int wrap_index(int k, int n) {
+    int r = k % n;
+    return r < 0 ? r + n : r;
+}
+
+// ------------------------------------------------------------------------------------------------
+// theta shift (rows, contiguous axis).  NSTAGE = 1: one half shift (eq (9) or (12)).  NSTAGE = 2: the
+// half shift that ends step k followed by the one that opens step k+1, same row, same (s, w), the
+// intermediate row kept in registers (halo exchanged with warp shuffles).
+//
+// A CTA owns a chunk of NW warp tiles of one row and walks down a band of rows, so that each thread owns
+// the same R consecutive COLUMNS for every row of the band and can keep their column sums (the density
+// partials, eq (10)) in registers.  Each lane reads its R+9 window from shared memory with lane stride R
+// (R odd: conflict-free for 8-byte words) and produces R consecutive values with R*10 FMAs.
+// ------------------------------------------------------------------------------------------------
+template <typename T>
+struct ThetaArgs {
+    const T* fin;
+    T* fout;
+    const int* srow;      // [Np] integer cell shift of one half step
+    const double* wrow;   // [Np][10] weights of one half step
+    double* colpart;      // [nbands][Ntheta] column sums of the OUTPUT over the band's rows (may be null)
+    int ntheta, np, bc_x, rows_per_band;
+};
+
+template <typename T, int NSTAGE, int R>
+__global__ void __launch_bounds__(384) theta_sweep_kernel(const ThetaArgs<T> arg) {
+    constexpr int LANES = (NSTAGE == 2) ? 31 : 32;  // lanes that own outputs
+    constexpr int TILE = LANES * R;                 // outputs per warp
+    constexpr int HALO = 9 * NSTAGE;
+    constexpr int KPRE = R + 1;                     // >= ceil((NW*TILE + HALO) / (32*NW))
+
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, NW = blockDim.x >> 5;
+    const int chunk = NW * TILE;
+    const int lenA = chunk + HALO;
+    T* A = reinterpret_cast<T*>(smem_raw);
+    T* O = A + ((lenA + 1) & ~1);
+
+    const int ntheta = arg.ntheta;
+    const int c0 = blockIdx.x * chunk;
+    const int j0 = blockIdx.y * arg.rows_per_band;
+    const int j1 = min(arg.np, j0 + arg.rows_per_band);
+    const int myq = warp * TILE + lane * R;
+    const int i0 = c0 + myq;
+    const bool owner = (lane < LANES);
+    const bool periodic = (arg.bc_x == BC_PERIODIC);
+
+    double csum[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) csum[r] = 0.0;
+
+    T pre[KPRE];
+    auto prefetch = [&](int j) {
+        const int S = NSTAGE * arg.srow[j];
+        const T* __restrict__ row = arg.fin + (size_t)j * ntheta;
+        int base = c0 + S - 4 * NSTAGE;
+        if (periodic) base = wrap_index(base, ntheta);
+#pragma unroll
+        for (int k = 0; k < KPRE; ++k) {
+            const int q = tid + k * blockDim.x;
+            T v = T(0);
+            if (q < lenA) {
+                int src = base + q;
+                if (periodic) {
+                    while (src >= ntheta) src -= ntheta;
+                    v = __ldg(row + src);
+                } else if ((unsigned)src < (unsigned)ntheta) {
+                    v = __ldg(row + src);
+                }
+            }
+            pre[k] = v;
+        }
+    };
+    auto stash = [&]() {
+#pragma unroll
+        for (int k = 0; k < KPRE; ++k) {
+            const int q = tid + k * blockDim.x;
+            if (q < lenA) A[q] = pre[k];
+        }
+    };
+
+    if (j0 < j1) {
+        prefetch(j0);
+        stash();
+    }
+    __syncthreads();
+
+    for (int j = j0; j < j1; ++j) {
+        if (j + 1 < j1) prefetch(j + 1);  // global loads of the next row fly during this row's arithmetic
+
+        T w[10];
+        {
+            const double* __restrict__ wr = arg.wrow + (size_t)j * 10;
+#pragma unroll
+            for (int m = 0; m < 10; ++m) w[m] = (T)__ldg(wr + m);
+        }
+        T v[R + 9];
+#pragma unroll
+        for (int k = 0; k < R + 9; ++k) v[k] = A[myq + k];
+
+        T g[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            T acc = w[0] * v[r];
+#pragma unroll
+            for (int m = 1; m < 10; ++m) acc = fma(w[m], v[r + m], acc);
+            g[r] = acc;
+        }
+
+        T out[R];
+        if (NSTAGE == 2) {
+            if (!periodic) {  // the intermediate row is zero outside [0, Ntheta) (two separate cropped shifts)
+                const int x0 = i0 + arg.srow[j] - 4;
+#pragma unroll
+                for (int r = 0; r < R; ++r)
+                    if ((unsigned)(x0 + r) >= (unsigned)ntheta) g[r] = T(0);
+            }
+            T h[R + 9];
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                h[r] = g[r];
+                h[R + r] = __shfl_down_sync(0xffffffffu, g[r], 1);
+            }
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                T acc = w[0] * h[r];
+#pragma unroll
+                for (int m = 1; m < 10; ++m) acc = fma(w[m], h[r + m], acc);
+                out[r] = acc;
+            }
+        } else {
+#pragma unroll
+            for (int r = 0; r < R; ++r) out[r] = g[r];
+        }
+
+        if (owner) {
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                O[myq + r] = out[r];
+                csum[r] += (double)out[r];
+            }
+        }
+        __syncthreads();  // O complete, all reads of A done
+
+        {
+            T* __restrict__ orow = arg.fout + (size_t)j * ntheta;
+            const int lim = min(chunk, ntheta - c0);
+            for (int q = tid; q < lim; q += blockDim.x) orow[c0 + q] = O[q];
+        }
+        if (j + 1 < j1) stash();
+        __syncthreads();
+    }
+
+    if (arg.colpart != nullptr && owner) {
+        double* __restrict__ cp = arg.colpart + (size_t)blockIdx.y * ntheta;
+#pragma unroll
+        for (int r = 0; r < R; ++r)
+            if (i0 + r < ntheta) cp[i0 + r] = csum[r];
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// p shift (columns, strided axis), eq (11): f_II(x_i, p_j) = f_I(x_i, p_j - F_i dt).
+// One thread = one column x one segment of rows.  Adjacent lanes own adjacent columns, so every load and
+// store of a warp is one contiguous 256-byte piece of a row: coalesced without any transpose.  The ten
+// taps live in a register window that slides down the column: one new load and ten FMAs per output.
+// ------------------------------------------------------------------------------------------------
+template <typename T>
+struct PArgs {
+    const T* fin;
+    T* fout;
+    const double* force;  // [Ntheta]
+    int ntheta, np, bc_p, seg_len;
+    double dt, dp;
+};
+
+template <typename T>
+__device__ __forceinline__ T load_row(const T* __restrict__ col, int r, int np, size_t pitch, bool periodic) {
+    if (periodic) {
+        if (r >= np) r -= np;  // callers keep r in [0, 2 np)
+        return __ldg(col + (size_t)r * pitch);
+    }
+    return ((unsigned)r < (unsigned)np) ? __ldg(col + (size_t)r * pitch) : T(0);
+}
+
+template <typename T>
+__global__ void __launch_bounds__(256) p_sweep_kernel(const PArgs<T> arg) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= arg.ntheta) return;
+    const int np = arg.np;
+    const int j0 = blockIdx.y * arg.seg_len;
+    const int j1 = min(np, j0 + arg.seg_len);
+    if (j0 >= j1) return;
+    const bool periodic = (arg.bc_p == BC_PERIODIC);
+    const size_t pitch = (size_t)arg.ntheta;
+
+    // foot of the characteristic: u = -(F dt)/dp cells  (D18)
+    double sf, a;
+    split_shift(-(arg.force[i] * arg.dt) / arg.dp, &sf, &a);
+    int s;
+    if (periodic) {
+        sf = fmod(sf, (double)np);
+        s = (int)sf;
+        if (s < 0) s += np;  // s in [0, np)
+    } else {
+        const double lim = (double)np + 64.0;
+        s = (int)fmin(fmax(sf, -lim), lim);
+    }
+    double wd[10];
+    spline_fd8_weights(a, wd);
+    T w[10];
+#pragma unroll
+    for (int m = 0; m < 10; ++m) w[m] = (T)wd[m];
+
+    const T* __restrict__ col = arg.fin + i;
+    T* __restrict__ ocol = arg.fout + i;
+
+    // row index of tap mm for output j is j + s + mm - 4.  In periodic mode keep an offset in [0, np).
+    int rbase = j0 + s - 4;
+    if (periodic) rbase = wrap_index(rbase, np);
+
+    T v[10];
+#pragma unroll
+    for (int k = 0; k < 9; ++k) {
+        int r = rbase + k;
+        if (periodic && r >= np) r -= np;
+        v[k] = load_row(col, r, np, pitch, periodic);
+    }
+    v[9] = T(0);
+    int rnext = rbase + 9;  // row of the next new tap
+    if (periodic) rnext = rnext % np;
+
+    T nv[10];
+    auto fetch = [&](int jb) {  // the ten new taps of outputs jb .. jb+9
+#pragma unroll
+        for (int k = 0; k < 10; ++k) {
+            int r = rnext + k;
+            nv[k] = (jb + k < j1) ? load_row(col, r, np, pitch, periodic) : T(0);
+        }
+        rnext += 10;
+        if (periodic && rnext >= np) rnext -= np;
+    };
+
+    fetch(j0);
+    for (int jb = j0; jb < j1; jb += 10) {
+        T cur[10];
+#pragma unroll
+        for (int k = 0; k < 10; ++k) cur[k] = nv[k];
+        if (jb + 10 < j1) fetch(jb + 10);  // loads of the next ten rows fly during these 100 FMAs
+#pragma unroll
+        for (int k = 0; k < 10; ++k) {
+            v[(k + 9) % 10] = cur[k];
+            T acc = w[0] * v[k % 10];
+#pragma unroll
+            for (int m = 1; m < 10; ++m) acc = fma(w[m], v[(k + m) % 10], acc);
+            if (jb + k < j1) ocol[(size_t)(jb + k) * pitch] = acc;
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// density and forces (eq (10); per model eqs (2), (4), (7)-(8))
+// ------------------------------------------------------------------------------------------------
+template <int NT>
+__device__ __forceinline__ double block_sum(double v, double* red /* NT/32 doubles */) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    __syncthreads();
+    if (lane == 0) red[warp] = v;
+    __syncthreads();
+    double t = 0.0;
+    if (warp == 0) {
+        t = (lane < NT / 32) ? red[lane] : 0.0;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) t += __shfl_down_sync(0xffffffffu, t, o);
+    }
+    return t;  // valid in thread 0
+}
+
+// rho_i = dp * sum_b colpart[b][i];  for HMF also per-block partial sums of cos(theta_i) rho_i, sin(theta_i) rho_i
+__global__ void __launch_bounds__(256) rho_reduce_kernel(const double* __restrict__ colpart, int nbands, int ntheta,
+                                                         double dp, double* __restrict__ rho,
+                                                         const double* __restrict__ cos_t,
+                                                         const double* __restrict__ sin_t,
+                                                         double* __restrict__ mpart /* [gridDim.x][2] */) {
+    __shared__ double red[8];
+    const int i = blockIdx.x * 256 + threadIdx.x;
+    double acc = 0.0;
+    if (i < ntheta) {
+        double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
+        int b = 0;
+        for (; b + 4 <= nbands; b += 4) {
+            a0 += colpart[(size_t)(b + 0) * ntheta + i];
+            a1 += colpart[(size_t)(b + 1) * ntheta + i];
+            a2 += colpart[(size_t)(b + 2) * ntheta + i];
+            a3 += colpart[(size_t)(b + 3) * ntheta + i];
+        }
+        for (; b < nbands; ++b) a0 += colpart[(size_t)b * ntheta + i];
+        acc = ((a0 + a1) + (a2 + a3)) * dp;
+        rho[i] = acc;
+    }
+    if (mpart != nullptr) {
+        const double c = (i < ntheta) ? cos_t[i] * acc : 0.0;
+        const double s = (i < ntheta) ? sin_t[i] * acc : 0.0;
+        const double cs = block_sum<256>(c, red);
+        const double ss = block_sum<256>(s, red);
+        if (threadIdx.x == 0) {
+            mpart[2 * blockIdx.x + 0] = cs;
+            mpart[2 * blockIdx.x + 1] = ss;
+        }
+    }
+}
+
+// HMF, eqs (7)-(8) (L56-L63): F_i = -M_x sin(theta_i) + M_y cos(theta_i)
+__global__ void __launch_bounds__(256) force_hmf_kernel(const double* __restrict__ mpart, int nparts, double dtheta,
+                                                        const double* __restrict__ cos_t,
+                                                        const double* __restrict__ sin_t, int ntheta,
+                                                        double* __restrict__ force, double* __restrict__ mxy) {
+    double mx = 0.0, my = 0.0;
+    for (int b = 0; b < nparts; ++b) {  // same order in every thread: deterministic, identical M everywhere
+        mx += mpart[2 * b + 0];
+        my += mpart[2 * b + 1];
+    }
+    mx *= dtheta;
+    my *= dtheta;
+    const int i = blockIdx.x * 256 + threadIdx.x;
+    if (i < ntheta) force[i] = -sin_t[i] * mx + cos_t[i] * my;
+    if (mxy != nullptr && blockIdx.x == 0 && threadIdx.x == 0) {
+        mxy[0] = mx;
+        mxy[1] = my;
+    }
+}
+
+// ring, eq (2) (L33-L35), reading D9: out_i = scale * sum_{m=0}^{N-1} tab[m] rho[(i - m) mod N].
+// Used with tab = K (force) and tab = V (potential, for the energy).  The table tile and the matching
+// window of rho are staged in shared memory; every thread owns one i.
+constexpr int RING_TM = 1024;
+__global__ void __launch_bounds__(256) ring_convolve_kernel(const double* __restrict__ tab,
+                                                            const double* __restrict__ rho, int n, double scale,
+                                                            double* __restrict__ out) {
+    __shared__ double sK[RING_TM];
+    __shared__ double sR[RING_TM + 256];
+    const int ib = blockIdx.x * 256;
+    const int i = ib + threadIdx.x;
+    double acc0 = 0.0, acc1 = 0.0;
+    for (int m0 = 0; m0 < n; m0 += RING_TM) {
+        const int tm = min(RING_TM, n - m0);
+        __syncthreads();
+        for (int q = threadIdx.x; q < tm; q += 256) sK[q] = tab[m0 + q];
+        // sR[q] = rho[(ib - m0 - (tm-1) + q) mod n], q in [0, tm + 255)
+        const int lo = wrap_index(ib - m0 - (tm - 1), n);
+        for (int q = threadIdx.x; q < tm + 255; q += 256) sR[q] = rho[(lo + q) % n];
+        __syncthreads();
+        // rho index i - m  ->  sR[(i - ib) + (tm-1) - (m - m0)]
+        const int off = threadIdx.x + tm - 1;
+        int mm = 0;
+        for (; mm + 2 <= tm; mm += 2) {
+            acc0 = fma(sK[mm], sR[off - mm], acc0);
+            acc1 = fma(sK[mm + 1], sR[off - mm - 1], acc1);
+        }
+        if (mm < tm) acc0 = fma(sK[mm], sR[off - mm], acc0);
+    }
+    if (i < n) out[i] = (acc0 + acc1) * scale;
+}
+
+// sheet, eq (4) (L41-L45), reading D11: F_i = -dx (sum_{k<i} rho_k - sum_{k>i} rho_k) = -dx (2 C_i + rho_i - S)
+// with C the exclusive prefix sum and S the total.  One CTA of 1024 threads scans the whole vector.
+// With mode = 1 writes instead the potential phi_i = dx sum_k |x_i - x_k| rho_k (for the energy):
+// phi_i = dx * dxnode * (i (2 C_i - S + rho_i) ... ) evaluated from the two prefix sums of rho_k and k rho_k.
+__global__ void __launch_bounds__(1024) sheet_scan_kernel(const double* __restrict__ rho, int n, double dx, int mode,
+                                                          double* __restrict__ out) {
+    __shared__ double wsum0[32], wsum1[32];
+    __shared__ double carry0, carry1, tot0, tot1;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    // pass 1: totals S0 = sum rho_k, S1 = sum k rho_k
+    {
+        double a0 = 0.0, a1 = 0.0;
+        for (int k = threadIdx.x; k < n; k += 1024) {
+            a0 += rho[k];
+            a1 += (double)k * rho[k];
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            a0 += __shfl_down_sync(0xffffffffu, a0, o);
+            a1 += __shfl_down_sync(0xffffffffu, a1, o);
+        }
+        if (lane == 0) {
+            wsum0[warp] = a0;
+            wsum1[warp] = a1;
+        }
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            double t0 = 0.0, t1 = 0.0;
+            for (int q = 0; q < 32; ++q) {
+                t0 += wsum0[q];
+                t1 += wsum1[q];
+            }
+            tot0 = t0;
+            tot1 = t1;
+            carry0 = 0.0;
+            carry1 = 0.0;
+        }
+        __syncthreads();
+    }
+    // pass 2: chunked inclusive scan with carry
+    for (int base = 0; base < n; base += 1024) {
+        const int k = base + threadIdx.x;
+        const double r = (k < n) ? rho[k] : 0.0;
+        double x0 = r, x1 = (double)k * r;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const double y0 = __shfl_up_sync(0xffffffffu, x0, o);
+            const double y1 = __shfl_up_sync(0xffffffffu, x1, o);
+            if (lane >= o) {
+                x0 += y0;
+                x1 += y1;
+            }
+        }
+        __syncthreads();
+        if (lane == 31) {
+            wsum0[warp] = x0;
+            wsum1[warp] = x1;
+        }
+        __syncthreads();
+        if (warp == 0) {
+            double z0 = wsum0[lane], z1 = wsum1[lane];
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const double y0 = __shfl_up_sync(0xffffffffu, z0, o);
+                const double y1 = __shfl_up_sync(0xffffffffu, z1, o);
+                if (lane >= o) {
+                    z0 += y0;
+                    z1 += y1;
+                }
+            }
+            wsum0[lane] = z0;
+            wsum1[lane] = z1;
+        }
+        __syncthreads();
+        const double inc0 = carry0 + (warp > 0 ? wsum0[warp - 1] : 0.0) + x0;  // inclusive prefix of rho
+        const double inc1 = carry1 + (warp > 0 ? wsum1[warp - 1] : 0.0) + x1;  // inclusive prefix of k rho
+        if (k < n) {
+            const double C0 = inc0 - r;                  // sum_{q<k} rho_q
+            const double C1 = inc1 - (double)k * r;      // sum_{q<k} q rho_q
+            if (mode == 0) {
+                out[k] = -dx * (2.0 * C0 + r - tot0);
+            } else {
+                // sum_q |k - q| rho_q = k C0 - C1 + (S1 - C1 - k r) - k (S0 - C0 - r)
+                const double right0 = tot0 - C0 - r, right1 = tot1 - C1 - (double)k * r;
+                out[k] = dx * dx * (((double)k * C0 - C1) + (right1 - (double)k * right0));
+            }
+        }
+        __syncthreads();
+        if (threadIdx.x == 1023) {
+            carry0 = inc0;
+            carry1 = inc1;
+        }
+        __syncthreads();
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// moments (a7): one read pass over f.  Each thread owns one column over a band of rows.
+// ------------------------------------------------------------------------------------------------
+template <typename T>
+__global__ void __launch_bounds__(256) moments_pass_kernel(const T* __restrict__ f, int ntheta, int np,
+                                                           int rows_per_band, double pmin, double dp,
+                                                           double* __restrict__ colpart /* [bands][ntheta] */,
+                                                           double* __restrict__ pk_part /* [blocks][2] */) {
+    __shared__ double red[8];
+    const int i = blockIdx.x * 256 + threadIdx.x;
+    const int j0 = blockIdx.y * rows_per_band, j1 = min(np, j0 + rows_per_band);
+    double c0 = 0.0, c1 = 0.0, c2 = 0.0;
+    if (i < ntheta) {
+        for (int j = j0; j < j1; ++j) {
+            const double v = (double)f[(size_t)j * ntheta + i];
+            const double p = pmin + (double)j * dp;
+            c0 += v;
+            c1 = fma(p, v, c1);
+            c2 = fma(0.5 * p * p, v, c2);
+        }
+        colpart[(size_t)blockIdx.y * ntheta + i] = c0;
+    }
+    const double s1 = block_sum<256>(c1, red);
+    const double s2 = block_sum<256>(c2, red);
+    if (threadIdx.x == 0) {
+        const int b = blockIdx.y * gridDim.x + blockIdx.x;
+        pk_part[2 * b + 0] = s1;
+        pk_part[2 * b + 1] = s2;
+    }
+}
+
+// final: one CTA.  rho must already hold dp * column sums; phi (ring / sheet potential) may be null.
+// out = {t, mass, P, K, U, Mx, My, E}
+__global__ void __launch_bounds__(1024) moments_final_kernel(const double* __restrict__ rho,
+                                                             const double* __restrict__ phi, int ntheta,
+                                                             const double* __restrict__ pk_part, int nparts,
+                                                             const double* __restrict__ cos_t,
+                                                             const double* __restrict__ sin_t, double dtheta,
+                                                             double dp, int model, double t,
+                                                             double* __restrict__ out) {
+    __shared__ double red[32];
+    double m = 0.0, cx = 0.0, sx = 0.0, u = 0.0, pp = 0.0, kk = 0.0;
+    for (int i = threadIdx.x; i < ntheta; i += 1024) {
+        const double r = rho[i];
+        m += r;
+        cx = fma(cos_t[i], r, cx);
+        sx = fma(sin_t[i], r, sx);
+        if (phi != nullptr) u = fma(r, phi[i], u);
+    }
+    for (int b = threadIdx.x; b < nparts; b += 1024) {
+        pp += pk_part[2 * b + 0];
+        kk += pk_part[2 * b + 1];
+    }
+    const double M = block_sum<1024>(m, red);
+    const double CX = block_sum<1024>(cx, red);
+    const double SX = block_sum<1024>(sx, red);
+    const double UU = block_sum<1024>(u, red);
+    const double PP = block_sum<1024>(pp, red);
+    const double KK = block_sum<1024>(kk, red);
+    if (threadIdx.x == 0) {
+        const double mass = M * dtheta, Mx = CX * dtheta, My = SX * dtheta;
+        const double P = PP * dtheta * dp, K = KK * dtheta * dp;
+        double U = 0.0;
+        if (model == 1) U = 0.5 * (mass * mass - Mx * Mx - My * My);
+        else if (model == 2 || model == 3) U = 0.5 * UU * dtheta;
+        out[0] = t;
+        out[1] = mass;
+        out[2] = P;
+        out[3] = K;
+        out[4] = U;
+        out[5] = Mx;
+        out[6] = My;
+        out[7] = K + U;
+    }
+}
+
+__global__ void fill_zero_kernel(double* __restrict__ p, int n) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) p[i] = 0.0;
+}
+
+}  // namespace vl

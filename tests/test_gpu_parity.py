@@ -1,0 +1,213 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle, element by element.
+
+Tolerances (north_star): fp64 max|df| <= 1e-10 max|f| after 100 steps, moments to 1e-10.
+"""
+from __future__ import annotations
+
+import math
+
+import numpy as np
+import pytest
+
+from oracle import BC_PERIODIC, BC_ZERO, MODEL_FREE, MODEL_HMF, MODEL_RING, MODEL_SHEET, Oracle
+from paper_1206_3229_b200 import binding as vb
+from paper_1206_3229_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+PI = math.pi
+TOL = 1e-10
+
+
+def rel_err(a, b):
+    den = float(np.max(np.abs(b)))
+    return float(np.max(np.abs(a - b))) / (den if den > 0.0 else 1.0)
+
+
+def smooth_state(nt, npp, dom, seed=1):
+    rng = np.random.default_rng(seed)
+    th = inputs.nodes(dom[0], dom[1], nt)
+    p = inputs.nodes(dom[2], dom[3], npp)
+    f = np.exp(-0.5 * (p[:, None] / 0.8) ** 2) * (1 + 0.4 * np.cos(th[None, :] - 0.3) + 0.1 * np.sin(3 * th[None, :]))
+    return f + 1e-3 * rng.random((npp, nt))
+
+
+def pair(model, grid, dom, dt, f0, threads=8, gpu_params=None, **params):
+    o = Oracle(model, grid, dom, dt, threads=threads, **params)
+    o.upload(f0)
+    g = vb.Vlasov(model, grid, dom, dt, **params, **(gpu_params or {}))
+    g.upload(f0)
+    return o, g
+
+
+# ----------------------------------------------------------------------------- single stages (T1)
+GRIDS = [(64, 48), (279, 33), (280, 65), (1000, 37), (2233, 20), (31, 9), (1, 5), (7, 1)]
+
+
+@pytest.mark.parametrize("grid", GRIDS)
+@pytest.mark.parametrize("bc_x", [BC_PERIODIC, BC_ZERO])
+@pytest.mark.parametrize("dt", [0.1, -0.37, 9.0, 0.0])
+def test_theta_half_sweep(grid, bc_x, dt):
+    dom = (-PI, PI, -4.0, 4.0)
+    f0 = smooth_state(grid[0], grid[1], dom)
+    o, g = pair(MODEL_FREE, grid, dom, dt, f0, bc_x=bc_x)
+    o.theta_sweep(0.5 * dt)
+    g.substep(vb.SUB_THETA_HALF)
+    assert rel_err(g.download(), o.download()) < 1e-13
+    g.close()
+
+
+@pytest.mark.parametrize("grid", GRIDS)
+@pytest.mark.parametrize("bc_x", [BC_PERIODIC, BC_ZERO])
+@pytest.mark.parametrize("dt", [0.1, -0.37, 9.0])
+def test_theta_twice_fused_equals_two_oracle_half_sweeps(grid, bc_x, dt):
+    dom = (-PI, PI, -4.0, 4.0)
+    f0 = smooth_state(grid[0], grid[1], dom, seed=2)
+    o, g = pair(MODEL_FREE, grid, dom, dt, f0, bc_x=bc_x)
+    o.theta_sweep(0.5 * dt)
+    o.theta_sweep(0.5 * dt)
+    g.substep(vb.SUB_THETA_TWICE)
+    assert rel_err(g.download(), o.download()) < 1e-13
+    g.close()
+
+
+@pytest.mark.parametrize("grid", [(64, 48), (130, 257), (33, 1000), (200, 10), (5, 3), (300, 41)])
+@pytest.mark.parametrize("bc_p", [BC_ZERO, BC_PERIODIC])
+@pytest.mark.parametrize("amp", [0.5, 30.0, 2000.0])
+def test_p_sweep_with_given_force(grid, bc_p, amp):
+    dom = (-PI, PI, -4.0, 4.0)
+    f0 = smooth_state(grid[0], grid[1], dom, seed=3)
+    th = inputs.nodes(dom[0], dom[1], grid[0])
+    F = amp * np.sin(2 * th + 0.1) + 0.3 * amp
+    o, g = pair(MODEL_FREE, grid, dom, 0.1, f0, bc_p=bc_p)
+    o.p_sweep(0.1, force=F)
+    g.set_force(F)
+    g.substep(vb.SUB_P_FULL)
+    assert rel_err(g.download(), o.download()) < 1e-13
+    g.close()
+
+
+@pytest.mark.parametrize("model,dom", [(MODEL_HMF, (-PI, PI, -4.0, 4.0)), (MODEL_RING, (-PI, PI, -3.0, 3.0)),
+                                       (MODEL_SHEET, (-10.0, 10.0, -4.0, 4.0)), (MODEL_FREE, (-PI, PI, -4.0, 4.0))])
+@pytest.mark.parametrize("grid", [(64, 48), (300, 129), (1500, 40), (2048, 64)])
+def test_density_force_and_moments(model, dom, grid):
+    f0 = smooth_state(grid[0], grid[1], dom, seed=4)
+    o, g = pair(model, grid, dom, 0.05, f0)
+    g.substep(vb.SUB_FORCE)
+    rho_o, F_o = o.density(), o.force()
+    assert np.max(np.abs(g.density() - rho_o)) <= 1e-13 * np.max(np.abs(rho_o))
+    assert np.max(np.abs(g.force() - F_o)) <= 1e-12 * max(np.max(np.abs(F_o)), 1e-300)
+    mo, mg = o.moments(), g.moments()
+    assert np.max(np.abs(mg - mo)) <= 1e-12 * np.max(np.abs(mo))
+    g.close()
+
+
+def test_density_after_theta_sweep_epilogue():
+    """The column sums the theta kernel leaves behind feed the force of the step (eq (10) uses f_I)."""
+    c = inputs.config("cfg1", ntheta=300, npts=200)
+    o, g = pair(c["model"], c["grid"], c["domain"], c["dt"], c["f0"])
+    o.theta_sweep(0.5 * c["dt"])
+    F_o = o.force()
+    g.step(1)
+    assert np.max(np.abs(g.force() - F_o)) <= 1e-12 * np.max(np.abs(F_o))
+    assert np.max(np.abs(g.density() - o.density())) <= 1e-13 * np.max(o.density())
+    g.close()
+
+
+# ----------------------------------------------------------------------------- full steps (T2, T3)
+CASES = [
+    ("cfg1", dict()),                        # the real cfg 1: 256 x 256, 100 steps
+    ("cfg2", dict(ntheta=256, npts=320)),
+    ("cfg3", dict(ntheta=320, npts=256)),
+    ("cfg4", dict(ntheta=512, npts=300)),
+    ("cfg5", dict(ntheta=600, npts=280)),
+]
+
+
+@pytest.mark.parametrize("name,kw", CASES)
+@pytest.mark.parametrize("fuse", [1, 0])
+def test_100_steps_match_oracle(name, kw, fuse):
+    c = inputs.config(name, **kw)
+    o, g = pair(c["model"], c["grid"], c["domain"], c["dt"], c["f0"], gpu_params=dict(fuse=fuse), **c["params"])
+    o.step(100)
+    g.step(100)
+    fo, fg = o.download(), g.download()
+    assert rel_err(fg, fo) <= TOL
+    mo, mg = o.moments(), g.moments()
+    assert np.max(np.abs(mg - mo)) <= TOL * max(1.0, np.max(np.abs(mo)))
+    assert mg[0] == pytest.approx(100 * c["dt"])
+    g.close()
+
+
+def test_history_records_every_step_and_matches_oracle():
+    c = inputs.config("cfg1", n=128)
+    o, g = pair(c["model"], c["grid"], c["domain"], c["dt"], c["f0"], gpu_params=dict(history=1))
+    g.step(20)
+    h = g.history(20)
+    assert h.shape == (20, 8)
+    for k in range(20):
+        o.step(1)
+        mo = o.moments()
+        assert np.max(np.abs(h[k] - mo)) <= TOL * max(1.0, np.max(np.abs(mo))), k
+    g.close()
+
+
+def test_fused_multi_step_equals_single_steps():
+    """P18: step(5) == 5 x step(1) (same kernels' arithmetic; the intermediate row is rounded to fp64 in both)."""
+    c = inputs.config("cfg5", ntheta=700, npts=260)
+    g = vb.Vlasov(c["model"], c["grid"], c["domain"], c["dt"])
+    g.upload(c["f0"])
+    g.step(5)
+    a = g.download()
+    g.close()
+    g = vb.Vlasov(c["model"], c["grid"], c["domain"], c["dt"])
+    g.upload(c["f0"])
+    for _ in range(5):
+        g.step(1)
+    b = g.download()
+    g.close()
+    assert np.array_equal(a, b)
+
+
+def test_library_owned_buffers_and_checkpoint_roundtrip():
+    c = inputs.config("cfg1", n=96)
+    g = vb.Vlasov(c["model"], c["grid"], c["domain"], c["dt"], attach=False)
+    g.upload(c["f0"])
+    assert np.array_equal(g.download(), c["f0"])
+    g.step(3)
+    ck = g.download()
+    g.step(2)
+    ref = g.download()
+    g.close()
+    g = vb.Vlasov(c["model"], c["grid"], c["domain"], c["dt"])
+    g.upload(ck)
+    g.step(2)
+    assert np.array_equal(g.download(), ref)
+    g.close()
+
+
+def test_errors():
+    with pytest.raises(vb.VlasovError):
+        vb.vlasov_init(9, (8, 8), (-1, 1, -1, 1), 0.1)
+    with pytest.raises(vb.VlasovError):
+        vb.vlasov_init(1, (8, 8), (1, -1, -1, 1), 0.1)
+    vb.vlasov_free()
+    with pytest.raises(vb.VlasovError) as e:
+        vb.vlasov_step(1)
+    assert e.value.code == vb.ENOTINIT
+    vb.vlasov_init(1, (8, 8), (-1, 1, -1, 1), 0.1)
+    with pytest.raises(vb.VlasovError) as e:
+        vb.vlasov_step(0)
+    assert e.value.code == vb.EINVAL
+    vb.vlasov_free()
+
+
+def test_fp32_path_matches_oracle_to_1e_4():
+    c = inputs.config("cfg5", ntheta=600, npts=280)
+    o = Oracle(c["model"], c["grid"], c["domain"], c["dt"], threads=8)
+    o.upload(c["f0"])
+    o.step(100)
+    g = vb.Vlasov(c["model"], c["grid"], c["domain"], c["dt"], precision=32)
+    g.upload(c["f0"])
+    g.step(100)
+    assert rel_err(g.download().astype(np.float64), o.download()) <= 1e-4
+    g.close()

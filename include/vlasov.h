@@ -53,6 +53,7 @@ extern "C" {
 #define VLASOV_KEY_BC_P 4      /* 0 periodic (paper, L113), 1 zero extension "f = 0 beyond" (default)       */
 #define VLASOV_KEY_HISTORY 5   /* 1: vlasov_step records the 8 moments after every step (no a6 fusion)      */
 #define VLASOV_KEY_FUSE 6      /* 1 (default): consecutive half theta-shifts of steps k, k+1 run as one pass */
+#define VLASOV_KEY_PROFILE 7   /* 1: bracket every sweep launch of vlasov_step with CUDA events (any time)   */
 
 /* sub-steps for vlasov_substep (parity tests of single stages; same kernels as vlasov_step) */
 #define VLASOV_SUB_THETA_HALF 0  /* eq (9)/(12): f(x - p dt/2, p), also leaves the column sums for the force */
@@ -138,6 +139,11 @@ int vlasov_sync(void);
 
 /* Number of kernels the library has launched since vlasov_init (for bench.py's gpu_launches). */
 int vlasov_launch_count(unsigned long long* out);
+
+/* With PROFILE = 1: out (host) = {ms, launches} summed over the launches recorded since the last call, for
+ * the kernel classes {theta x1, theta x2 (fused), p, density+force}; CUDA-event times on the launch stream.
+ * Blocks until the stream is idle; resets the records. */
+int vlasov_kernel_times(double out[8]);
 
 /* Fill out[0..n) (host) with implementation facts for reports: {SM count, theta-kernel CTAs, p-kernel CTAs,
  * bands, warps per theta CTA (2-shift), warps per theta CTA (1-shift)}; returns how many were written. */

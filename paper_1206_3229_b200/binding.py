@@ -17,7 +17,7 @@ import numpy as np
 from . import build as _build
 
 MODEL_FREE, MODEL_HMF, MODEL_RING, MODEL_SHEET = 0, 1, 2, 3
-KEY_EPS, KEY_PRECISION, KEY_BC_X, KEY_BC_P, KEY_HISTORY, KEY_FUSE = 1, 2, 3, 4, 5, 6
+KEY_EPS, KEY_PRECISION, KEY_BC_X, KEY_BC_P, KEY_HISTORY, KEY_FUSE, KEY_PROFILE = 1, 2, 3, 4, 5, 6, 7
 KEY_TUNE_NW1, KEY_TUNE_NW2, KEY_TUNE_BANDS, KEY_TUNE_PSEG, KEY_TUNE_PTX = 101, 102, 103, 104, 105
 SUB_THETA_HALF, SUB_FORCE, SUB_P_FULL, SUB_THETA_TWICE = 0, 1, 2, 3
 VEC_RHO, VEC_FORCE = 0, 1
@@ -27,7 +27,7 @@ EXPORTS = (
     "vlasov_init", "vlasov_set_param", "vlasov_state_bytes", "vlasov_workspace_bytes", "vlasov_attach",
     "vlasov_state_ptr", "vlasov_upload", "vlasov_download", "vlasov_step", "vlasov_substep",
     "vlasov_get_vector", "vlasov_set_vector", "vlasov_moments", "vlasov_history", "vlasov_sync",
-    "vlasov_launch_count", "vlasov_info", "vlasov_free", "vlasov_last_error",
+    "vlasov_launch_count", "vlasov_kernel_times", "vlasov_info", "vlasov_free", "vlasov_last_error",
 )
 
 
@@ -79,6 +79,7 @@ def load(build_if_missing: bool = True):
         "vlasov_sync": (ci, []),
         "vlasov_launch_count": (ci, [ctypes.POINTER(ctypes.c_ulonglong)]),
         "vlasov_info": (ci, [_dp, ci]),
+        "vlasov_kernel_times": (ci, [_dp]),
         "vlasov_free": (None, []),
         "vlasov_last_error": (ctypes.c_char_p, []),
     }
@@ -186,6 +187,13 @@ def vlasov_launch_count() -> int:
     return int(out.value)
 
 
+def vlasov_kernel_times() -> dict:
+    buf = np.zeros(8, dtype=np.float64)
+    _chk(load().vlasov_kernel_times(buf.ctypes.data_as(_dp)), "vlasov_kernel_times")
+    names = ["theta1", "theta2", "p", "force"]
+    return {k: {"ms": float(buf[2 * i]), "launches": int(buf[2 * i + 1])} for i, k in enumerate(names)}
+
+
 def vlasov_info() -> dict:
     buf = np.zeros(16, dtype=np.float64)
     n = _chk(load().vlasov_info(buf.ctypes.data_as(_dp), 16), "vlasov_info")
@@ -221,7 +229,7 @@ class Vlasov:
         vlasov_init(model, grid, domain, dt)
         if precision != 64:
             vlasov_set_param(KEY_PRECISION, precision)
-        keys = {"eps": KEY_EPS, "bc_x": KEY_BC_X, "bc_p": KEY_BC_P, "history": KEY_HISTORY, "fuse": KEY_FUSE,
+        keys = {"eps": KEY_EPS, "bc_x": KEY_BC_X, "bc_p": KEY_BC_P, "history": KEY_HISTORY, "fuse": KEY_FUSE, "profile": KEY_PROFILE,
                 "tune_nw1": KEY_TUNE_NW1, "tune_nw2": KEY_TUNE_NW2, "tune_bands": KEY_TUNE_BANDS,
                 "tune_pseg": KEY_TUNE_PSEG, "tune_ptx": KEY_TUNE_PTX}
         for k, v in params.items():

@@ -55,9 +55,38 @@ struct Ctx {
     int p_tx = 128, p_seg = 0, p_nseg = 0;
     int tune_nw1 = 0, tune_nw2 = 0, tune_bands = 0, tune_pseg = 0, tune_ptx = 0;
     unsigned long long launches = 0;
+
+    // optional per-kernel timing with CUDA events on the launch stream (KEY_PROFILE)
+    bool profile = false;
+    std::vector<cudaEvent_t> ev[4][2];  // class: 0 theta x1, 1 theta x2, 2 p, 3 rho+force
+    size_t ev_used[4] = {0, 0, 0, 0};
 };
 
 Ctx G;
+constexpr size_t EV_CAP = 2048;
+
+void prof_begin(int cls) {
+    if (!G.profile || G.ev_used[cls] >= EV_CAP) return;
+    if (G.ev[cls][0].size() <= G.ev_used[cls]) {
+        cudaEvent_t a, b;
+        if (cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&b) != cudaSuccess) return;
+        G.ev[cls][0].push_back(a);
+        G.ev[cls][1].push_back(b);
+    }
+    cudaEventRecord(G.ev[cls][0][G.ev_used[cls]], G.stream);
+}
+void prof_end(int cls) {
+    if (!G.profile || G.ev_used[cls] >= EV_CAP || G.ev[cls][1].size() <= G.ev_used[cls]) return;
+    cudaEventRecord(G.ev[cls][1][G.ev_used[cls]], G.stream);
+    G.ev_used[cls]++;
+}
+void prof_free() {
+    for (int c = 0; c < 4; ++c)
+        for (int k = 0; k < 2; ++k) {
+            for (cudaEvent_t e : G.ev[c][k]) cudaEventDestroy(e);
+            G.ev[c][k].clear();
+        }
+}
 
 int fail(int code, const char* fmt, const char* a = "") {
     snprintf(g_err, sizeof(g_err), fmt, a);
@@ -296,8 +325,10 @@ int launch_theta(bool want_colsums) {
     a.rows_per_band = G.rpb[NSTAGE];
     const int nw = G.nw[NSTAGE];
     dim3 grid(G.nchunks[NSTAGE], G.nbands[NSTAGE]);
+    prof_begin(NSTAGE - 1);
     vl::theta_sweep_kernel<T, NSTAGE, R_THETA>
         <<<grid, nw * 32, theta_smem_bytes<T, NSTAGE>(nw), G.stream>>>(a);
+    prof_end(NSTAGE - 1);
     LAUNCH_CHECK();
     G.cur ^= 1;
     return VLASOV_OK;
@@ -322,7 +353,9 @@ int launch_p() {
     a.dt = G.dt;
     a.dp = (G.pmax - G.pmin) / (double)G.np;
     dim3 grid(cdiv(G.ntheta, G.p_tx), G.p_nseg);
+    prof_begin(2);
     vl::p_sweep_kernel<T><<<grid, G.p_tx, 0, G.stream>>>(a);
+    prof_end(2);
     LAUNCH_CHECK();
     G.cur ^= 1;
     return VLASOV_OK;
@@ -411,6 +444,7 @@ const char* vlasov_last_error(void) { return g_err; }
 
 void vlasov_free(void) {
     if (G.ready) cudaStreamSynchronize(G.stream);
+    prof_free();
     free_small();
     free_big();
     G = Ctx();
@@ -448,6 +482,10 @@ int vlasov_init(int model, const int grid[2], const double domain[4], double dt)
 int vlasov_set_param(int key, double value) {
     int rc = check_ready();
     if (rc != 0) return rc;
+    if (key == VLASOV_KEY_PROFILE) {
+        G.profile = (value != 0.0);
+        return VLASOV_OK;
+    }
     if (G.prepared) return fail(VLASOV_EINVAL, "vlasov_set_param: must precede attach/upload/step");
     switch (key) {
         case VLASOV_KEY_EPS:
@@ -468,6 +506,7 @@ int vlasov_set_param(int key, double value) {
             break;
         case VLASOV_KEY_HISTORY: G.history = (value != 0.0); break;
         case VLASOV_KEY_FUSE: G.fuse = (value != 0.0); break;
+        case VLASOV_KEY_PROFILE: G.profile = (value != 0.0); break;
         case KEY_TUNE_NW1: G.tune_nw1 = (int)value; break;
         case KEY_TUNE_NW2: G.tune_nw2 = (int)value; break;
         case KEY_TUNE_BANDS: G.tune_bands = (int)value; break;
@@ -556,8 +595,10 @@ int vlasov_step(int n) {
     if (fused) {
         if ((rc = theta_pass(1, true)) != 0) return rc;                       // eq (9)
         for (int k = 0; k < n; ++k) {
+            prof_begin(3);
             if ((rc = rho_from_colpart(G.nbands[k == 0 ? 1 : 2], G.rho, hmf)) != 0) return rc;
             if ((rc = force_from_rho()) != 0) return rc;                      // eq (10)
+            prof_end(3);
             if ((rc = p_pass()) != 0) return rc;                              // eq (11)
             if (k + 1 < n) {
                 if ((rc = theta_pass(2, true)) != 0) return rc;               // eq (12) of step k, eq (9) of k+1
@@ -647,6 +688,25 @@ int vlasov_history(double* out, int max_steps) {
 int vlasov_launch_count(unsigned long long* out) {
     if (!out) return fail(VLASOV_EINVAL, "vlasov_launch_count: null");
     *out = G.launches;
+    return VLASOV_OK;
+}
+
+int vlasov_kernel_times(double out[8]) {
+    int rc = check_ready();
+    if (rc != 0) return rc;
+    if (!out) return fail(VLASOV_EINVAL, "vlasov_kernel_times: null");
+    CU(cudaStreamSynchronize(G.stream));
+    for (int c = 0; c < 4; ++c) {
+        double total = 0.0;
+        for (size_t k = 0; k < G.ev_used[c]; ++k) {
+            float ms = 0.f;
+            CU(cudaEventElapsedTime(&ms, G.ev[c][0][k], G.ev[c][1][k]));
+            total += (double)ms;
+        }
+        out[2 * c + 0] = total;
+        out[2 * c + 1] = (double)G.ev_used[c];
+        G.ev_used[c] = 0;
+    }
     return VLASOV_OK;
 }
 

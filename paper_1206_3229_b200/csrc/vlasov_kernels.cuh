@@ -238,7 +238,7 @@ struct PArgs {
 template <typename T>
 __device__ __forceinline__ T load_row(const T* __restrict__ col, int r, int np, size_t pitch, bool periodic) {
     if (periodic) {
-        if (r >= np) r -= np;  // callers keep r in [0, 2 np)
+        while (r >= np) r -= np;  // callers keep r >= 0; np may be smaller than the ten-tap window
         return __ldg(col + (size_t)r * pitch);
     }
     return ((unsigned)r < (unsigned)np) ? __ldg(col + (size_t)r * pitch) : T(0);
@@ -283,9 +283,7 @@ __global__ void __launch_bounds__(256) p_sweep_kernel(const PArgs<T> arg) {
     T v[10];
 #pragma unroll
     for (int k = 0; k < 9; ++k) {
-        int r = rbase + k;
-        if (periodic && r >= np) r -= np;
-        v[k] = load_row(col, r, np, pitch, periodic);
+        v[k] = load_row(col, rbase + k, np, pitch, periodic);
     }
     v[9] = T(0);
     int rnext = rbase + 9;  // row of the next new tap
@@ -299,7 +297,7 @@ __global__ void __launch_bounds__(256) p_sweep_kernel(const PArgs<T> arg) {
             nv[k] = (jb + k < j1) ? load_row(col, r, np, pitch, periodic) : T(0);
         }
         rnext += 10;
-        if (periodic && rnext >= np) rnext -= np;
+        if (periodic) rnext %= np;
     };
 
     fetch(j0);

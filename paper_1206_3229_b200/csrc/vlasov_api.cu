@@ -15,12 +15,16 @@
 
 #include "../../include/vlasov.h"
 #include "vlasov_kernels.cuh"
+#include "vlasov_theta_bulk.cuh"
 
 namespace {
 
 constexpr int R_THETA = 9;       // consecutive outputs per lane in the theta kernel (odd: bank-conflict-free)
+constexpr int TB_NS = 3;         // rows in flight per warp in the bulk-copy theta kernel
+constexpr int TB_WARPS = 4;      // warps per CTA (independent pipelines)
+constexpr int TB_MINB = 3;       // CTAs per SM the register budget is set for
 constexpr int KEY_TUNE_NW1 = 101, KEY_TUNE_NW2 = 102, KEY_TUNE_BANDS = 103, KEY_TUNE_PSEG = 104,
-              KEY_TUNE_PTX = 105;
+              KEY_TUNE_PTX = 105, KEY_TUNE_GENERIC = 106;
 
 thread_local char g_err[512] = "";
 
@@ -51,9 +55,13 @@ struct Ctx {
     int nw[3] = {0, 6, 6};         // warps per theta CTA for NSTAGE = 1, 2
     int nchunks[3] = {0, 0, 0};
     int nbands[3] = {0, 0, 0}, rpb[3] = {0, 0, 0};
+    bool theta_bulk = false;       // rows are multiples of 16 bytes: bulk-copy kernel (else the generic one)
+    vl::ThetaBulkGrid bgrid[3] = {};
+    int bctas[3] = {0, 0, 0};
     int mbands = 0, mrpb = 0;      // moments pass
     int p_tx = 128, p_seg = 0, p_nseg = 0;
     int tune_nw1 = 0, tune_nw2 = 0, tune_bands = 0, tune_pseg = 0, tune_ptx = 0;
+    bool force_generic = false;    // KEY_TUNE_GENERIC: use the generic theta kernel even when rows are aligned
     unsigned long long launches = 0;
 
     // optional per-kernel timing with CUDA events on the launch stream (KEY_PROFILE)
@@ -170,7 +178,7 @@ int configure_theta(int tune_nw) {
     if (nw > 12) nw = 12;
     G.nw[NSTAGE] = nw;
     G.nchunks[NSTAGE] = cdiv(tiles, nw);
-    auto kern = vl::theta_sweep_kernel<T, NSTAGE, R_THETA>;
+    auto kern = vl::theta_sweep_generic_kernel<T, NSTAGE, R_THETA>;
     const size_t smem = theta_smem_bytes<T, NSTAGE>(nw);
     CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int occ = 1;
@@ -184,11 +192,40 @@ int configure_theta(int tune_nw) {
     return VLASOV_OK;
 }
 
+// bulk-copy kernel: every warp is a pipeline over (band of rows) x (chunk of columns); one wave of warps
+template <typename T, int NSTAGE>
+int configure_theta_bulk() {
+    using C = vl::ThetaBulk<T, NSTAGE, R_THETA, TB_NS, TB_WARPS>;
+    auto kern = vl::theta_sweep_bulk_kernel<T, NSTAGE, R_THETA, TB_NS, TB_WARPS, TB_MINB>;
+    CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES));
+    int occ = 1;
+    CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, TB_WARPS * 32, C::SMEM_BYTES));
+    if (occ < 1) occ = 1;
+    const int nchunks = cdiv(G.ntheta, C::CHUNK);
+    int bands = G.tune_bands > 0 ? G.tune_bands : (G.sm_count * occ * TB_WARPS) / nchunks;
+    const int max_bands = G.np >= 16 ? G.np / 8 : 1;  // at least 8 rows per pipeline
+    if (bands > max_bands && G.tune_bands <= 0) bands = max_bands;
+    if (bands < 1) bands = 1;
+    if (bands > G.np) bands = G.np;
+    vl::ThetaBulkGrid g;
+    g.nchunks = nchunks;
+    g.rows_per_band = cdiv(G.np, bands);
+    g.nbands = cdiv(G.np, g.rows_per_band);
+    G.bgrid[NSTAGE] = g;
+    G.bctas[NSTAGE] = cdiv(g.nchunks * g.nbands, TB_WARPS);
+    return VLASOV_OK;
+}
+
 template <typename T>
 int configure_all() {
     int rc;
     if ((rc = configure_theta<T, 1>(G.tune_nw1)) != 0) return rc;
     if ((rc = configure_theta<T, 2>(G.tune_nw2)) != 0) return rc;
+    G.theta_bulk = (G.ntheta % (16 / (int)sizeof(T)) == 0) && !G.force_generic;
+    if (G.theta_bulk) {
+        if ((rc = configure_theta_bulk<T, 1>()) != 0) return rc;
+        if ((rc = configure_theta_bulk<T, 2>()) != 0) return rc;
+    }
     // p shift: 128 adjacent columns per CTA; segments so that a bit more than one wave of CTAs exists
     G.p_tx = G.tune_ptx > 0 ? G.tune_ptx : 128;
     if (G.p_tx > 256) G.p_tx = 256;
@@ -196,7 +233,7 @@ int configure_all() {
     CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, vl::p_sweep_kernel<T>, G.p_tx, 0));
     if (occ < 1) occ = 1;
     const int colblocks = cdiv(G.ntheta, G.p_tx);
-    int nseg = cdiv(G.sm_count * occ, colblocks);
+    int nseg = (G.sm_count * occ) / colblocks;  // floor: every CTA resident at once, no second partial wave
     if (nseg < 1) nseg = 1;
     int seg = G.tune_pseg > 0 ? G.tune_pseg : cdiv(G.np, nseg);
     if (seg < 40 && G.tune_pseg <= 0) seg = 40;  // keep the 9-row halo re-read below ~20 %
@@ -232,7 +269,7 @@ int prepare() {
 
     // per-row shift of one half step: displacement p_j tau (eq (9)), u = -disp/dx cells
     std::vector<int> srow(np);
-    std::vector<double> wrow((size_t)np * 10);
+    std::vector<double> wrow((size_t)np * vl::WROW_STRIDE, 0.0);
     for (int j = 0; j < np; ++j) {
         const double p = G.pmin + (double)j * dp;
         const double disp = p * tau;
@@ -245,7 +282,8 @@ int prepare() {
             sf = fmin(fmax(sf, -lim), lim);
         }
         srow[j] = (int)sf;
-        vl::spline_fd8_weights(a, &wrow[(size_t)j * 10]);
+        vl::spline_fd8_weights(a, &wrow[(size_t)j * vl::WROW_STRIDE]);
+        wrow[(size_t)j * vl::WROW_STRIDE + 10] = sf;
     }
     std::vector<double> ct(nt), st(nt);
     for (int i = 0; i < nt; ++i) {
@@ -254,11 +292,11 @@ int prepare() {
         st[i] = sin(th);
     }
     CU(cudaMalloc(&G.srow, sizeof(int) * np));
-    CU(cudaMalloc(&G.wrow, sizeof(double) * np * 10));
+    CU(cudaMalloc(&G.wrow, sizeof(double) * np * vl::WROW_STRIDE));
     CU(cudaMalloc(&G.cos_t, sizeof(double) * nt));
     CU(cudaMalloc(&G.sin_t, sizeof(double) * nt));
     CU(cudaMemcpy(G.srow, srow.data(), sizeof(int) * np, cudaMemcpyHostToDevice));
-    CU(cudaMemcpy(G.wrow, wrow.data(), sizeof(double) * np * 10, cudaMemcpyHostToDevice));
+    CU(cudaMemcpy(G.wrow, wrow.data(), sizeof(double) * np * vl::WROW_STRIDE, cudaMemcpyHostToDevice));
     CU(cudaMemcpy(G.cos_t, ct.data(), sizeof(double) * nt, cudaMemcpyHostToDevice));
     CU(cudaMemcpy(G.sin_t, st.data(), sizeof(double) * nt, cudaMemcpyHostToDevice));
     if (G.model == VLASOV_MODEL_RING) {
@@ -323,16 +361,24 @@ int launch_theta(bool want_colsums) {
     a.np = G.np;
     a.bc_x = G.bc_x;
     a.rows_per_band = G.rpb[NSTAGE];
-    const int nw = G.nw[NSTAGE];
-    dim3 grid(G.nchunks[NSTAGE], G.nbands[NSTAGE]);
     prof_begin(NSTAGE - 1);
-    vl::theta_sweep_kernel<T, NSTAGE, R_THETA>
-        <<<grid, nw * 32, theta_smem_bytes<T, NSTAGE>(nw), G.stream>>>(a);
+    if (G.theta_bulk) {
+        using C = vl::ThetaBulk<T, NSTAGE, R_THETA, TB_NS, TB_WARPS>;
+        vl::theta_sweep_bulk_kernel<T, NSTAGE, R_THETA, TB_NS, TB_WARPS, TB_MINB>
+            <<<G.bctas[NSTAGE], TB_WARPS * 32, C::SMEM_BYTES, G.stream>>>(a, G.bgrid[NSTAGE]);
+    } else {
+        const int nw = G.nw[NSTAGE];
+        dim3 grid(G.nchunks[NSTAGE], G.nbands[NSTAGE]);
+        vl::theta_sweep_generic_kernel<T, NSTAGE, R_THETA>
+            <<<grid, nw * 32, theta_smem_bytes<T, NSTAGE>(nw), G.stream>>>(a);
+    }
     prof_end(NSTAGE - 1);
     LAUNCH_CHECK();
     G.cur ^= 1;
     return VLASOV_OK;
 }
+
+int theta_bands(int nstage) { return G.theta_bulk ? G.bgrid[nstage].nbands : G.nbands[nstage]; }
 
 int theta_pass(int nstage, bool want_colsums) {
     if (G.prec == 32)
@@ -512,6 +558,7 @@ int vlasov_set_param(int key, double value) {
         case KEY_TUNE_BANDS: G.tune_bands = (int)value; break;
         case KEY_TUNE_PSEG: G.tune_pseg = (int)value; break;
         case KEY_TUNE_PTX: G.tune_ptx = (int)value; break;
+        case KEY_TUNE_GENERIC: G.force_generic = (value != 0.0); break;
         default: return fail(VLASOV_EINVAL, "vlasov_set_param: unknown key");
     }
     return VLASOV_OK;
@@ -596,7 +643,7 @@ int vlasov_step(int n) {
         if ((rc = theta_pass(1, true)) != 0) return rc;                       // eq (9)
         for (int k = 0; k < n; ++k) {
             prof_begin(3);
-            if ((rc = rho_from_colpart(G.nbands[k == 0 ? 1 : 2], G.rho, hmf)) != 0) return rc;
+            if ((rc = rho_from_colpart(theta_bands(k == 0 ? 1 : 2), G.rho, hmf)) != 0) return rc;
             if ((rc = force_from_rho()) != 0) return rc;                      // eq (10)
             prof_end(3);
             if ((rc = p_pass()) != 0) return rc;                              // eq (11)
@@ -610,7 +657,7 @@ int vlasov_step(int n) {
     } else {
         for (int k = 0; k < n; ++k) {
             if ((rc = theta_pass(1, true)) != 0) return rc;
-            if ((rc = rho_from_colpart(G.nbands[1], G.rho, hmf)) != 0) return rc;
+            if ((rc = rho_from_colpart(theta_bands(1), G.rho, hmf)) != 0) return rc;
             if ((rc = force_from_rho()) != 0) return rc;
             if ((rc = p_pass()) != 0) return rc;
             if ((rc = theta_pass(1, false)) != 0) return rc;
@@ -715,15 +762,17 @@ int vlasov_info(double* out, int n) {
     if (rc != 0) return rc;
     if (!out || n < 0) return fail(VLASOV_EINVAL, "vlasov_info: bad argument");
     if ((rc = prepare()) != 0) return rc;
+    const bool tb = G.theta_bulk;
     const double v[] = {(double)G.sm_count,
-                        (double)G.nchunks[2] * G.nbands[2],
+                        tb ? (double)G.bctas[2] : (double)G.nchunks[2] * G.nbands[2],
                         (double)cdiv(G.ntheta, G.p_tx) * G.p_nseg,
-                        (double)G.nbands[2],
-                        (double)G.nw[2],
-                        (double)G.nw[1],
-                        (double)G.nchunks[1] * G.nbands[1],
+                        (double)theta_bands(2),
+                        tb ? (double)TB_WARPS : (double)G.nw[2],
+                        tb ? (double)TB_WARPS : (double)G.nw[1],
+                        tb ? (double)G.bctas[1] : (double)G.nchunks[1] * G.nbands[1],
                         (double)G.p_seg,
-                        (double)G.p_tx};
+                        (double)G.p_tx,
+                        tb ? 1.0 : 0.0};
     const int m = (int)(sizeof(v) / sizeof(v[0]));
     const int k = n < m ? n : m;
     for (int q = 0; q < k; ++q) out[q] = v[q];

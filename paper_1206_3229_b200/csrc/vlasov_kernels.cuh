@@ -15,9 +15,14 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include "vlasov_ptx.cuh"
+
 namespace vl {
 
 enum { BC_PERIODIC = 0, BC_ZERO = 1 };
+
+// per-row table of the theta half shift: {w_0..w_9, (double) s, 0}; 96 bytes = one 16-byte-aligned bulk copy
+constexpr int WROW_STRIDE = 12;
 
 // eq (16), divided by 6 (the 1/6 of gamma, delta in eq (14)); index m+4, m = -4..4
 __host__ __device__ inline double c16_over_6(int m) {
@@ -64,6 +69,7 @@ __device__ __forceinline__ int wrap_index(int k, int n) {
 }
 
 // ------------------------------------------------------------------------------------------------
+// GENERIC theta shift (any Ntheta, any alignment; used when a row is not a multiple of 16 bytes).
 // theta shift (rows, contiguous axis).  NSTAGE = 1: one half shift (eq (9) or (12)).  NSTAGE = 2: the
 // half shift that ends step k followed by the one that opens step k+1, same row, same (s, w), the
 // intermediate row kept in registers (halo exchanged with warp shuffles).
@@ -78,13 +84,13 @@ struct ThetaArgs {
     const T* fin;
     T* fout;
     const int* srow;      // [Np] integer cell shift of one half step
-    const double* wrow;   // [Np][10] weights of one half step
+    const double* wrow;   // [Np][WROW_STRIDE]: ten weights of one half step, then s as a double
     double* colpart;      // [nbands][Ntheta] column sums of the OUTPUT over the band's rows (may be null)
     int ntheta, np, bc_x, rows_per_band;
 };
 
 template <typename T, int NSTAGE, int R>
-__global__ void __launch_bounds__(384) theta_sweep_kernel(const ThetaArgs<T> arg) {
+__global__ void __launch_bounds__(384) theta_sweep_generic_kernel(const ThetaArgs<T> arg) {
     constexpr int LANES = (NSTAGE == 2) ? 31 : 32;  // lanes that own outputs
     constexpr int TILE = LANES * R;                 // outputs per warp
     constexpr int HALO = 9 * NSTAGE;
@@ -151,7 +157,7 @@ __global__ void __launch_bounds__(384) theta_sweep_kernel(const ThetaArgs<T> arg
 
         T w[10];
         {
-            const double* __restrict__ wr = arg.wrow + (size_t)j * 10;
+            const double* __restrict__ wr = arg.wrow + (size_t)j * WROW_STRIDE;
 #pragma unroll
             for (int m = 0; m < 10; ++m) w[m] = (T)__ldg(wr + m);
         }

@@ -47,10 +47,10 @@ def measured_peak():
         return HBM_FALLBACK_GBS, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
-def committed_traffic(n: int, precision: int):
+def committed_traffic(kernel: str, n: int, precision: int):
     """DRAM bytes per launch of the dominant kernel from the committed ncu capture (profiles/), or None."""
     path = os.path.join(ROOT, "profiles", "traffic.txt")
-    key = "theta2_n%d_fp%d_dram_bytes_per_launch" % (n, precision)
+    key = "%s_n%d_fp%d_dram_bytes_per_launch" % (kernel, n, precision)
     try:
         with open(path) as fh:
             for line in fh:
@@ -194,7 +194,8 @@ def run_cuda(args):
     eb = 8 if prec == 64 else 4
     c = inputs.config("cfg5", n=n)
     f0 = c["f0"].astype(np.float64 if prec == 64 else np.float32)
-    g = vb.Vlasov(c["model"], c["grid"], c["domain"], c["dt"], precision=prec, device="cuda:%d" % local_rank)
+    g = vb.Vlasov(c["model"], c["grid"], c["domain"], c["dt"], precision=prec, device="cuda:%d" % local_rank,
+                  fuse=args.fuse)
     g.upload(f0)
     pts = float(n) * float(n)
 
@@ -238,19 +239,23 @@ def run_cuda(args):
                           "achieved_gbs": 2 * eb * pts / (avg_ms * 1e-3) / 1e9}
         elif d["launches"] > 0:
             kern[name] = {"avg_ms": d["ms"] / d["launches"], "launches": d["launches"]}
-    dom = "theta2" if "theta2" in kern else ("theta1" if "theta1" in kern else None)
-    if dom is not None and "p" in kern and kern["p"]["avg_ms"] > kern[dom]["avg_ms"]:
-        dom = "p"
+    sweeps = [k for k in kern if k != "force"]
+    dom = max(sweeps, key=lambda k: kern[k]["avg_ms"] * kern[k]["launches"]) if sweeps else None
+    passes = sum(kern[k]["launches"] for k in sweeps)
+    step_bytes = 2 * eb * passes / K  # algorithmic bytes per grid point per step of THIS run (one read + one write per pass)
     roofline = None
     if dom is not None:
         ach = kern[dom]["achieved_gbs"]
-        roofline = {"bound": "hbm", "kernel": {"theta2": "theta_sweep_kernel<2 shifts>", "theta1": "theta_sweep_kernel<1 shift>",
-                                                "p": "p_sweep_kernel"}[dom],
+        names = {"theta2": "theta_sweep_bulk_kernel<2 shifts>", "theta1": "theta_sweep_bulk_kernel<1 shift>",
+                 "p": "p_sweep_kernel", "ptheta2": "strang_fused_kernel<p + 2 theta shifts + density>",
+                 "ptheta1": "strang_fused_kernel<p + 1 theta shift>"}
+        roofline = {"bound": "hbm", "kernel": names[dom],
                     "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
-                    "traffic": committed_traffic(n, prec) if dom == "theta2" else None,
+                    "traffic": committed_traffic(dom, n, prec),
                     "peak_source": peak_src, "algorithmic_bytes_per_launch": 2 * eb * pts,
-                    "step_frac": (4 * eb * pts * K / (ms_local * 1e-3) / 1e9) / peak,
-                    "step_bytes_per_point": 4 * eb}
+                    "step_frac": (step_bytes * pts * K / (ms_local * 1e-3) / 1e9) / peak,
+                    "step_bytes_per_point": step_bytes,
+                    "two_pass_step_frac": (4 * eb * pts * K / (ms_local * 1e-3) / 1e9) / peak}
 
     # ---- end to end through the C ABI with host buffers
     Ke = min(K, args.e2e_steps)
@@ -297,7 +302,7 @@ def run_cuda(args):
         "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64" if prec == 64 else "f32", "data": "synthetic",
         "config": {"workload": "cfg5 HMF water-bag %dx%d %s, dt=0.1, theta periodic, p zero-extended, seeded 1e-6 noise" % (n, n, "fp64" if prec == 64 else "fp32"),
-                   "grid": [n, n], "passes_per_step": (2 * K + 1) / K,
+                   "grid": [n, n], "passes_per_step": passes / K, "fuse": args.fuse,
                    "l2": "state (%.0f MiB x 2 buffers) exceeds the 126 MB L2; no flush needed" % (pts * eb / 2 ** 20)
                    if pts * eb > 126e6 else "state fits L2: DRAM roofline not claimed",
                    "parallelism": "replicas x%d" % world if world > 1 else "single GPU", "launch": info},
@@ -321,6 +326,8 @@ def main():
     ap.add_argument("--cpu-seconds", type=float, default=10.0)
     ap.add_argument("--ref-n", type=int, default=1024, help="grid of the --impl reference sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--fuse", type=int, default=2, choices=[0, 1, 2],
+                    help="passes per step: 2 = one (p + theta in one kernel, default), 1 = two, 0 = three")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)

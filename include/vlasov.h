@@ -52,7 +52,10 @@ extern "C" {
 #define VLASOV_KEY_BC_X 3      /* 0 periodic (paper, L113; default for FREE/HMF/RING), 1 zero extension     */
 #define VLASOV_KEY_BC_P 4      /* 0 periodic (paper, L113), 1 zero extension "f = 0 beyond" (default)       */
 #define VLASOV_KEY_HISTORY 5   /* 1: vlasov_step records the 8 moments after every step (no a6 fusion)      */
-#define VLASOV_KEY_FUSE 6      /* 1 (default): consecutive half theta-shifts of steps k, k+1 run as one pass */
+#define VLASOV_KEY_FUSE 6      /* passes over f per step in vlasov_step(n): 0: three (theta, p, theta); 1: two (the
+                                  adjacent half theta shifts of steps k, k+1 share a pass); 2 (default): ONE
+                                  (p shift, both half theta shifts and the density of the next step share a pass;
+                                  needs periodic x, otherwise behaves like 1)                                   */
 #define VLASOV_KEY_PROFILE 7   /* 1: bracket every sweep launch of vlasov_step with CUDA events (any time)   */
 
 /* sub-steps for vlasov_substep (parity tests of single stages; same kernels as vlasov_step) */
@@ -60,6 +63,9 @@ extern "C" {
 #define VLASOV_SUB_FORCE 1       /* eq (10): density + force of the CURRENT f (runs its own density pass)    */
 #define VLASOV_SUB_P_FULL 2      /* eq (11): f(x, p - F dt) with the force vector currently stored           */
 #define VLASOV_SUB_THETA_TWICE 3 /* two half shifts in one pass (the fused a5 o a1 kernel)                   */
+#define VLASOV_SUB_P_THETA_HALF 4  /* one-pass kernel: eq (11) with the stored force, then eq (12); then the density
+                                      and force of the result are left in the RHO / FORCE vectors (FUSE = 2 only) */
+#define VLASOV_SUB_P_THETA_TWICE 5 /* one-pass kernel: eq (11), eq (12), eq (9) of the next step, then density, force */
 
 /* vectors for vlasov_get_vector / vlasov_set_vector (Ntheta doubles each) */
 #define VLASOV_VEC_RHO 0   /* density rho_i = dp sum_j f_ij used by the last force evaluation */
@@ -140,10 +146,10 @@ int vlasov_sync(void);
 /* Number of kernels the library has launched since vlasov_init (for bench.py's gpu_launches). */
 int vlasov_launch_count(unsigned long long* out);
 
-/* With PROFILE = 1: out (host) = {ms, launches} summed over the launches recorded since the last call, for
- * the kernel classes {theta x1, theta x2 (fused), p, density+force}; CUDA-event times on the launch stream.
- * Blocks until the stream is idle; resets the records. */
-int vlasov_kernel_times(double out[8]);
+/* With PROFILE = 1: out (host, 12 doubles) = {ms, launches} summed over the launches recorded since the last
+ * call, for the kernel classes {theta x1, theta x2, p, density+force, p+theta x2 (one pass), p+theta x1};
+ * CUDA-event times on the launch stream.  Blocks until the stream is idle; resets the records. */
+int vlasov_kernel_times(double out[12]);
 
 /* Fill out[0..n) (host) with implementation facts for reports: {SM count, theta-kernel CTAs, p-kernel CTAs,
  * bands, warps per theta CTA (2-shift), warps per theta CTA (1-shift)}; returns how many were written. */

@@ -18,8 +18,8 @@ from . import build as _build
 
 MODEL_FREE, MODEL_HMF, MODEL_RING, MODEL_SHEET = 0, 1, 2, 3
 KEY_EPS, KEY_PRECISION, KEY_BC_X, KEY_BC_P, KEY_HISTORY, KEY_FUSE, KEY_PROFILE = 1, 2, 3, 4, 5, 6, 7
-KEY_TUNE_NW1, KEY_TUNE_NW2, KEY_TUNE_BANDS, KEY_TUNE_PSEG, KEY_TUNE_PTX, KEY_TUNE_GENERIC = 101, 102, 103, 104, 105, 106
-SUB_THETA_HALF, SUB_FORCE, SUB_P_FULL, SUB_THETA_TWICE = 0, 1, 2, 3
+KEY_TUNE_NW1, KEY_TUNE_NW2, KEY_TUNE_BANDS, KEY_TUNE_PSEG, KEY_TUNE_PTX, KEY_TUNE_GENERIC, KEY_TUNE_FBANDS = 101, 102, 103, 104, 105, 106, 107
+SUB_THETA_HALF, SUB_FORCE, SUB_P_FULL, SUB_THETA_TWICE, SUB_P_THETA_HALF, SUB_P_THETA_TWICE = 0, 1, 2, 3, 4, 5
 VEC_RHO, VEC_FORCE = 0, 1
 OK, EINVAL, ENOTINIT, ECUDA, ENOMEM = 0, -1, -2, -3, -4
 
@@ -188,9 +188,9 @@ def vlasov_launch_count() -> int:
 
 
 def vlasov_kernel_times() -> dict:
-    buf = np.zeros(8, dtype=np.float64)
+    buf = np.zeros(12, dtype=np.float64)
     _chk(load().vlasov_kernel_times(buf.ctypes.data_as(_dp)), "vlasov_kernel_times")
-    names = ["theta1", "theta2", "p", "force"]
+    names = ["theta1", "theta2", "p", "force", "ptheta2", "ptheta1"]
     return {k: {"ms": float(buf[2 * i]), "launches": int(buf[2 * i + 1])} for i, k in enumerate(names)}
 
 
@@ -231,7 +231,8 @@ class Vlasov:
             vlasov_set_param(KEY_PRECISION, precision)
         keys = {"eps": KEY_EPS, "bc_x": KEY_BC_X, "bc_p": KEY_BC_P, "history": KEY_HISTORY, "fuse": KEY_FUSE, "profile": KEY_PROFILE,
                 "tune_nw1": KEY_TUNE_NW1, "tune_nw2": KEY_TUNE_NW2, "tune_bands": KEY_TUNE_BANDS,
-                "tune_pseg": KEY_TUNE_PSEG, "tune_ptx": KEY_TUNE_PTX, "tune_generic": KEY_TUNE_GENERIC}
+                "tune_pseg": KEY_TUNE_PSEG, "tune_ptx": KEY_TUNE_PTX, "tune_generic": KEY_TUNE_GENERIC,
+                "tune_fbands": KEY_TUNE_FBANDS}
         for k, v in params.items():
             vlasov_set_param(keys[k], float(v))
         self.f_dev = self.work_dev = None

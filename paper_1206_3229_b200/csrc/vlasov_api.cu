@@ -16,6 +16,7 @@
 #include "../../include/vlasov.h"
 #include "vlasov_kernels.cuh"
 #include "vlasov_theta_bulk.cuh"
+#include "vlasov_fused.cuh"
 
 namespace {
 
@@ -23,6 +24,11 @@ constexpr int R_THETA = 9;       // consecutive outputs per lane in the theta ke
 constexpr int TB_NS = 3;         // rows in flight per warp in the bulk-copy theta kernel
 constexpr int TB_WARPS = 4;      // warps per CTA (independent pipelines)
 constexpr int TB_MINB = 3;       // CTAs per SM the register budget is set for
+constexpr int FU_NT = 384;       // threads per CTA of the one-pass kernel (one per source column)
+constexpr int FU_R = 11;         // consecutive outputs per lane in its theta stage (odd)
+constexpr int FU_NSTG = 3;       // cp.async ring depth (phases of 12 rows)
+constexpr int NCLS = 6;          // profiled kernel classes: theta x1, theta x2, p, rho+force, p+theta x2, p+theta x1
+constexpr int KEY_TUNE_FBANDS = 107;
 constexpr int KEY_TUNE_NW1 = 101, KEY_TUNE_NW2 = 102, KEY_TUNE_BANDS = 103, KEY_TUNE_PSEG = 104,
               KEY_TUNE_PTX = 105, KEY_TUNE_GENERIC = 106;
 
@@ -33,7 +39,8 @@ struct Ctx {
     int model = 0, ntheta = 0, np = 0;
     double xmin = 0, xmax = 0, pmin = 0, pmax = 0, dt = 0, eps = 0.01, t = 0;
     int bc_x = 0, bc_p = 1, prec = 64;
-    bool history = false, fuse = true;
+    bool history = false;
+    int fuse = 2;  // 0: p and theta passes apart, 1: adjacent half theta shifts in one pass, 2: p + theta in one pass
     cudaStream_t stream = nullptr;
     int sm_count = 148;
 
@@ -50,6 +57,13 @@ struct Ctx {
     double *rho = nullptr, *force = nullptr, *rho_m = nullptr, *phi = nullptr, *mpart = nullptr, *pkpart = nullptr,
            *mom_dev = nullptr, *hist = nullptr;
     int hist_cap = 0, hist_count = 0;
+    // one-pass kernel: composite theta weights, band shift ranges, its own density partials
+    double *wrow2 = nullptr, *colpart_f = nullptr;
+    int* band_s[3] = {nullptr, nullptr, nullptr};
+    int fbands[3] = {0, 0, 0}, frpb[3] = {0, 0, 0}, fcols[3] = {0, 0, 0};
+    bool onepass = false;
+    int tune_fbands = 0;
+    std::vector<int> h_srow;
 
     // launch configuration
     int nw[3] = {0, 6, 6};         // warps per theta CTA for NSTAGE = 1, 2
@@ -66,8 +80,8 @@ struct Ctx {
 
     // optional per-kernel timing with CUDA events on the launch stream (KEY_PROFILE)
     bool profile = false;
-    std::vector<cudaEvent_t> ev[4][2];  // class: 0 theta x1, 1 theta x2, 2 p, 3 rho+force
-    size_t ev_used[4] = {0, 0, 0, 0};
+    std::vector<cudaEvent_t> ev[NCLS][2];  // class: 0 theta x1, 1 theta x2, 2 p, 3 rho+force, 4 p+theta x2, 5 p+theta x1
+    size_t ev_used[NCLS] = {0, 0, 0, 0, 0, 0};
 };
 
 Ctx G;
@@ -89,7 +103,7 @@ void prof_end(int cls) {
     G.ev_used[cls]++;
 }
 void prof_free() {
-    for (int c = 0; c < 4; ++c)
+    for (int c = 0; c < NCLS; ++c)
         for (int k = 0; k < 2; ++k) {
             for (cudaEvent_t e : G.ev[c][k]) cudaEventDestroy(e);
             G.ev[c][k].clear();
@@ -125,12 +139,13 @@ int cdiv(int a, int b) { return (a + b - 1) / b; }
 
 void free_small() {
     void* ptrs[] = {G.srow, G.wrow, G.cos_t, G.sin_t, G.ringK, G.ringV, G.rho, G.force, G.rho_m,
-                    G.phi,  G.mpart, G.pkpart, G.mom_dev, G.hist};
+                    G.phi,  G.mpart, G.pkpart, G.mom_dev, G.hist, G.wrow2, G.colpart_f, G.band_s[1], G.band_s[2]};
     for (void* p : ptrs)
         if (p) cudaFree(p);
     G.srow = nullptr;
     G.wrow = G.cos_t = G.sin_t = G.ringK = G.ringV = G.rho = G.force = G.rho_m = G.phi = G.mpart = G.pkpart =
-        G.mom_dev = G.hist = nullptr;
+        G.mom_dev = G.hist = G.wrow2 = G.colpart_f = nullptr;
+    G.band_s[1] = G.band_s[2] = nullptr;
     G.hist_cap = G.hist_count = 0;
 }
 
@@ -216,6 +231,49 @@ int configure_theta_bulk() {
     return VLASOV_OK;
 }
 
+// one-pass kernel (p shift + NST theta half shifts): column blocks x bands, one CTA per SM; a band is short
+// enough that the integer theta shift drifts by at most MAX_DRIFT (and Ntheta) columns inside it
+template <typename T, int NST>
+int configure_fused() {
+    using C = vl::FusedCfg<T, NST, FU_NT, FU_R, FU_NSTG>;
+    auto kern = vl::strang_fused_kernel<T, NST, FU_NT, FU_R, FU_NSTG>;
+    CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM_BYTES));
+    const int np = G.np;
+    const int cols = cdiv(G.ntheta, C::TI);
+    int bands = G.tune_fbands > 0 ? G.tune_fbands : G.sm_count / cols;
+    if (bands < 1) bands = 1;
+    if (bands > np) bands = np;
+    int rpb = cdiv(np, bands);
+    const int limit = C::MAX_DRIFT < G.ntheta ? C::MAX_DRIFT : G.ntheta;
+    std::vector<int> bs;
+    for (;;) {
+        bands = cdiv(np, rpb);
+        bs.assign((size_t)2 * bands, 0);
+        int worst = 0;
+        for (int b = 0; b < bands; ++b) {
+            int lo = 1 << 30, hi = -(1 << 30);
+            for (int j = b * rpb; j < np && j < (b + 1) * rpb; ++j) {
+                const int S = NST * G.h_srow[j];
+                lo = S < lo ? S : lo;
+                hi = S > hi ? S : hi;
+            }
+            bs[2 * b + 0] = lo;
+            bs[2 * b + 1] = hi;
+            worst = (hi - lo) > worst ? (hi - lo) : worst;
+        }
+        if (worst <= limit || rpb == 1) break;
+        rpb = (rpb + 1) / 2;
+    }
+    G.fbands[NST] = bands;
+    G.frpb[NST] = rpb;
+    G.fcols[NST] = cols;
+    if (G.band_s[NST]) CU(cudaFree(G.band_s[NST]));
+    G.band_s[NST] = nullptr;
+    CU(cudaMalloc(&G.band_s[NST], sizeof(int) * 2 * bands));
+    CU(cudaMemcpy(G.band_s[NST], bs.data(), sizeof(int) * 2 * bands, cudaMemcpyHostToDevice));
+    return VLASOV_OK;
+}
+
 template <typename T>
 int configure_all() {
     int rc;
@@ -225,6 +283,11 @@ int configure_all() {
     if (G.theta_bulk) {
         if ((rc = configure_theta_bulk<T, 1>()) != 0) return rc;
         if ((rc = configure_theta_bulk<T, 2>()) != 0) return rc;
+    }
+    G.onepass = (G.fuse >= 2) && (G.bc_x == vl::BC_PERIODIC);
+    if (G.onepass) {
+        if ((rc = configure_fused<T, 1>()) != 0) return rc;
+        if ((rc = configure_fused<T, 2>()) != 0) return rc;
     }
     // p shift: 128 adjacent columns per CTA; segments so that a bit more than one wave of CTAs exists
     G.p_tx = G.tune_ptx > 0 ? G.tune_ptx : 128;
@@ -285,6 +348,20 @@ int prepare() {
         vl::spline_fd8_weights(a, &wrow[(size_t)j * vl::WROW_STRIDE]);
         wrow[(size_t)j * vl::WROW_STRIDE + 10] = sf;
     }
+    G.h_srow = srow;
+    // composite weights of two equal half shifts, W = w * w (19 taps): the one-pass kernel applies both at once
+    std::vector<double> wrow2((size_t)np * 20, 0.0);
+    for (int j = 0; j < np; ++j) {
+        const double* w = &wrow[(size_t)j * vl::WROW_STRIDE];
+        double* W = &wrow2[(size_t)j * 20];
+        for (int n = 0; n < 19; ++n) {
+            double acc = 0.0;
+            for (int m = (n > 9 ? n - 9 : 0); m <= (n < 9 ? n : 9); ++m) acc += w[m] * w[n - m];
+            W[n] = acc;
+        }
+    }
+    CU(cudaMalloc(&G.wrow2, sizeof(double) * np * 20));
+    CU(cudaMemcpy(G.wrow2, wrow2.data(), sizeof(double) * np * 20, cudaMemcpyHostToDevice));
     std::vector<double> ct(nt), st(nt);
     for (int i = 0; i < nt; ++i) {
         const double th = G.xmin + (double)i * dx;
@@ -326,6 +403,11 @@ int prepare() {
     int rc = (G.prec == 32) ? configure_all<float>() : configure_all<double>();
     if (rc != 0) return rc;
     CU(cudaMalloc(&G.pkpart, sizeof(double) * 2 * (size_t)G.mbands * cdiv(nt, 256)));
+    if (G.onepass) {
+        const size_t nb = (size_t)(G.fbands[2] > G.fbands[1] ? G.fbands[2] : G.fbands[1]);
+        CU(cudaMalloc(&G.colpart_f, sizeof(double) * nb * nt));
+        CU(cudaMemset(G.colpart_f, 0, sizeof(double) * nb * nt));
+    }
     G.cp_bands = max_bands_bound();
     G.prepared = true;
     return VLASOV_OK;
@@ -409,11 +491,47 @@ int launch_p() {
 
 int p_pass() { return G.prec == 32 ? launch_p<float>() : launch_p<double>(); }
 
+// one pass: momentum shift with the stored force, then NST theta half shifts, then (optionally) the density
+// partials of the result in colpart_f (eqs (11), (12), (9), (10))
+template <typename T, int NST>
+int launch_fused(bool want_colsums) {
+    using C = vl::FusedCfg<T, NST, FU_NT, FU_R, FU_NSTG>;
+    vl::FusedArgs<T> a;
+    a.fin = static_cast<const T*>(G.f[G.cur]);
+    a.fout = static_cast<T*>(G.f[G.cur ^ 1]);
+    a.force = G.force;
+    a.srow = G.srow;
+    a.wtab = NST == 2 ? G.wrow2 : G.wrow;
+    a.wstride = NST == 2 ? 20 : vl::WROW_STRIDE;
+    a.band_s = G.band_s[NST];
+    a.colpart = want_colsums ? G.colpart_f : nullptr;
+    a.ntheta = G.ntheta;
+    a.np = G.np;
+    a.bc_p = G.bc_p;
+    a.rows_per_band = G.frpb[NST];
+    a.dt = G.dt;
+    a.dp = (G.pmax - G.pmin) / (double)G.np;
+    dim3 grid(G.fcols[NST], G.fbands[NST]);
+    prof_begin(NST == 2 ? 4 : 5);
+    vl::strang_fused_kernel<T, NST, FU_NT, FU_R, FU_NSTG><<<grid, FU_NT, C::SMEM_BYTES, G.stream>>>(a);
+    prof_end(NST == 2 ? 4 : 5);
+    LAUNCH_CHECK();
+    G.cur ^= 1;
+    return VLASOV_OK;
+}
+
+int fused_pass(int nstage, bool want_colsums) {
+    if (G.prec == 32)
+        return nstage == 2 ? launch_fused<float, 2>(want_colsums) : launch_fused<float, 1>(want_colsums);
+    return nstage == 2 ? launch_fused<double, 2>(want_colsums) : launch_fused<double, 1>(want_colsums);
+}
+
 // rho (and for HMF the moment partials) from the column sums left in colpart by `bands` bands
-int rho_from_colpart(int bands, double* rho_out, bool hmf_partials) {
+int rho_from_colpart(int bands, double* rho_out, bool hmf_partials, double* colpart = nullptr, bool zero_after = false) {
     const double dp = (G.pmax - G.pmin) / (double)G.np;
     vl::rho_reduce_kernel<<<cdiv(G.ntheta, 256), 256, 0, G.stream>>>(
-        G.colpart, bands, G.ntheta, dp, rho_out, G.cos_t, G.sin_t, hmf_partials ? G.mpart : nullptr);
+        colpart ? colpart : G.colpart, bands, G.ntheta, dp, rho_out, G.cos_t, G.sin_t,
+        hmf_partials ? G.mpart : nullptr, zero_after ? 1 : 0);
     LAUNCH_CHECK();
     return VLASOV_OK;
 }
@@ -551,7 +669,11 @@ int vlasov_set_param(int key, double value) {
             G.bc_p = (int)value;
             break;
         case VLASOV_KEY_HISTORY: G.history = (value != 0.0); break;
-        case VLASOV_KEY_FUSE: G.fuse = (value != 0.0); break;
+        case VLASOV_KEY_FUSE:
+            if (value != 0.0 && value != 1.0 && value != 2.0) return fail(VLASOV_EINVAL, "FUSE must be 0, 1 or 2");
+            G.fuse = (int)value;
+            break;
+        case KEY_TUNE_FBANDS: G.tune_fbands = (int)value; break;
         case VLASOV_KEY_PROFILE: G.profile = (value != 0.0); break;
         case KEY_TUNE_NW1: G.tune_nw1 = (int)value; break;
         case KEY_TUNE_NW2: G.tune_nw2 = (int)value; break;
@@ -638,8 +760,20 @@ int vlasov_step(int n) {
         }
         G.hist_count = 0;
     }
-    const bool fused = G.fuse && !G.history;
-    if (fused) {
+    if (G.onepass && !G.history) {
+        // n + 1 passes: theta(dt/2), then per step ONE pass  p(dt) -> theta(dt/2) [-> theta(dt/2) of the next step]
+        if ((rc = theta_pass(1, true)) != 0) return rc;                           // eq (9)
+        for (int k = 0; k < n; ++k) {
+            prof_begin(3);
+            if (k == 0) rc = rho_from_colpart(theta_bands(1), G.rho, hmf);
+            else rc = rho_from_colpart(G.fbands[2], G.rho, hmf, G.colpart_f, true);
+            if (rc != 0) return rc;
+            if ((rc = force_from_rho()) != 0) return rc;                          // eq (10)
+            prof_end(3);
+            if ((rc = fused_pass(k + 1 < n ? 2 : 1, k + 1 < n)) != 0) return rc;  // eqs (11), (12) [, (9)]
+        }
+        G.t += (double)n * G.dt;
+    } else if (G.fuse >= 1 && !G.history) {
         if ((rc = theta_pass(1, true)) != 0) return rc;                       // eq (9)
         for (int k = 0; k < n; ++k) {
             prof_begin(3);
@@ -659,8 +793,12 @@ int vlasov_step(int n) {
             if ((rc = theta_pass(1, true)) != 0) return rc;
             if ((rc = rho_from_colpart(theta_bands(1), G.rho, hmf)) != 0) return rc;
             if ((rc = force_from_rho()) != 0) return rc;
-            if ((rc = p_pass()) != 0) return rc;
-            if ((rc = theta_pass(1, false)) != 0) return rc;
+            if (G.onepass) {
+                if ((rc = fused_pass(1, false)) != 0) return rc;              // eqs (11), (12) in one pass
+            } else {
+                if ((rc = p_pass()) != 0) return rc;
+                if ((rc = theta_pass(1, false)) != 0) return rc;
+            }
             G.t += G.dt;
             if (G.history) {
                 if ((rc = moments_async(G.hist + 8 * (size_t)k)) != 0) return rc;
@@ -683,6 +821,14 @@ int vlasov_substep(int which) {
             if ((rc = rho_from_colpart(G.mbands, G.rho, G.model == VLASOV_MODEL_HMF)) != 0) return rc;
             return force_from_rho();
         case VLASOV_SUB_P_FULL: return p_pass();
+        case VLASOV_SUB_P_THETA_HALF:
+        case VLASOV_SUB_P_THETA_TWICE: {
+            if (!G.onepass) return fail(VLASOV_EINVAL, "vlasov_substep: the one-pass kernel needs FUSE = 2 and periodic x");
+            const int nst = which == VLASOV_SUB_P_THETA_TWICE ? 2 : 1;
+            if ((rc = fused_pass(nst, true)) != 0) return rc;
+            if ((rc = rho_from_colpart(G.fbands[nst], G.rho, G.model == VLASOV_MODEL_HMF, G.colpart_f, true)) != 0) return rc;
+            return force_from_rho();
+        }
         default: return fail(VLASOV_EINVAL, "vlasov_substep: unknown stage");
     }
 }
@@ -738,12 +884,12 @@ int vlasov_launch_count(unsigned long long* out) {
     return VLASOV_OK;
 }
 
-int vlasov_kernel_times(double out[8]) {
+int vlasov_kernel_times(double out[12]) {
     int rc = check_ready();
     if (rc != 0) return rc;
     if (!out) return fail(VLASOV_EINVAL, "vlasov_kernel_times: null");
     CU(cudaStreamSynchronize(G.stream));
-    for (int c = 0; c < 4; ++c) {
+    for (int c = 0; c < NCLS; ++c) {
         double total = 0.0;
         for (size_t k = 0; k < G.ev_used[c]; ++k) {
             float ms = 0.f;

@@ -344,11 +344,13 @@ __device__ __forceinline__ double block_sum(double v, double* red /* NT/32 doubl
 }
 
 // rho_i = dp * sum_b colpart[b][i];  for HMF also per-block partial sums of cos(theta_i) rho_i, sin(theta_i) rho_i
-__global__ void __launch_bounds__(256) rho_reduce_kernel(const double* __restrict__ colpart, int nbands, int ntheta,
+// zero_after: the partials are accumulated by atomic adds (one-pass kernel) and must be zero for the next pass
+__global__ void __launch_bounds__(256) rho_reduce_kernel(double* __restrict__ colpart, int nbands, int ntheta,
                                                          double dp, double* __restrict__ rho,
                                                          const double* __restrict__ cos_t,
                                                          const double* __restrict__ sin_t,
-                                                         double* __restrict__ mpart /* [gridDim.x][2] */) {
+                                                         double* __restrict__ mpart /* [gridDim.x][2] */,
+                                                         int zero_after) {
     __shared__ double red[8];
     const int i = blockIdx.x * 256 + threadIdx.x;
     double acc = 0.0;
@@ -362,6 +364,8 @@ __global__ void __launch_bounds__(256) rho_reduce_kernel(const double* __restric
             a3 += colpart[(size_t)(b + 3) * ntheta + i];
         }
         for (; b < nbands; ++b) a0 += colpart[(size_t)b * ntheta + i];
+        if (zero_after)
+            for (b = 0; b < nbands; ++b) colpart[(size_t)b * ntheta + i] = 0.0;
         acc = ((a0 + a1) + (a2 + a3)) * dp;
         rho[i] = acc;
     }

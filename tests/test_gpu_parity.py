@@ -113,6 +113,54 @@ def test_density_after_theta_sweep_epilogue():
     g.close()
 
 
+# ----------------------------------------------------------------------------- one-pass kernel (p + theta)
+ONEPASS_GRIDS = [(64, 48), (352, 30), (353, 61), (1000, 137), (2233, 25), (31, 9), (1, 5), (7, 1), (720, 700)]
+
+
+@pytest.mark.parametrize("grid", ONEPASS_GRIDS)
+@pytest.mark.parametrize("bc_p", [BC_ZERO, BC_PERIODIC])
+@pytest.mark.parametrize("which,dt,amp", [(1, 0.1, 0.5), (2, 0.1, 0.5), (2, -0.37, 30.0), (1, 9.0, 2000.0),
+                                          (2, 9.0, 30.0), (2, 3.0, 0.0)])
+def test_one_pass_p_then_theta(grid, bc_p, which, dt, amp):
+    """p shift with a given force, then one or two half theta shifts, then density and force of the result:
+    the one-pass kernel against the oracle's separate sweeps (eqs (11), (12), (9), (10))."""
+    dom = (-PI, PI, -4.0, 4.0)
+    f0 = smooth_state(grid[0], grid[1], dom, seed=5)
+    th = inputs.nodes(dom[0], dom[1], grid[0])
+    F = amp * np.sin(2 * th + 0.1) + 0.3 * amp
+    o, g = pair(MODEL_HMF, grid, dom, dt, f0, bc_p=bc_p)
+    o.p_sweep(dt, force=F)
+    for _ in range(which):
+        o.theta_sweep(0.5 * dt)
+    g.set_force(F)
+    g.substep(vb.SUB_P_THETA_TWICE if which == 2 else vb.SUB_P_THETA_HALF)
+    fo = o.download()
+    assert rel_err(g.download(), fo) < 1e-13
+    rho_o = o.density()
+    assert np.max(np.abs(g.density() - rho_o)) <= 1e-13 * np.max(np.abs(rho_o))
+    F_o = o.force()
+    assert np.max(np.abs(g.force() - F_o)) <= 1e-12 * max(np.max(np.abs(F_o)), np.max(np.abs(rho_o)))
+    g.close()
+
+
+@pytest.mark.parametrize("fbands", [1, 3, 50])
+def test_one_pass_band_split_does_not_change_the_result(fbands):
+    dom = (-PI, PI, -4.0, 4.0)
+    grid = (800, 300)
+    f0 = smooth_state(grid[0], grid[1], dom, seed=6)
+    th = inputs.nodes(dom[0], dom[1], grid[0])
+    F = 3.0 * np.sin(th + 0.2)
+    o, g = pair(MODEL_HMF, grid, dom, 0.7, f0, gpu_params=dict(tune_fbands=fbands))
+    o.p_sweep(0.7, force=F)
+    o.theta_sweep(0.35)
+    o.theta_sweep(0.35)
+    g.set_force(F)
+    g.substep(vb.SUB_P_THETA_TWICE)
+    assert rel_err(g.download(), o.download()) < 1e-13
+    assert np.max(np.abs(g.density() - o.density())) <= 1e-13 * np.max(o.density())
+    g.close()
+
+
 # ----------------------------------------------------------------------------- full steps (T2, T3)
 CASES = [
     ("cfg1", dict()),                        # the real cfg 1: 256 x 256, 100 steps
@@ -124,7 +172,7 @@ CASES = [
 
 
 @pytest.mark.parametrize("name,kw", CASES)
-@pytest.mark.parametrize("fuse", [1, 0])
+@pytest.mark.parametrize("fuse", [2, 1, 0])
 def test_100_steps_match_oracle(name, kw, fuse):
     c = inputs.config(name, **kw)
     o, g = pair(c["model"], c["grid"], c["domain"], c["dt"], c["f0"], gpu_params=dict(fuse=fuse), **c["params"])
@@ -151,21 +199,39 @@ def test_history_records_every_step_and_matches_oracle():
     g.close()
 
 
-def test_fused_multi_step_equals_single_steps():
-    """P18: step(5) == 5 x step(1) (same kernels' arithmetic; the intermediate row is rounded to fp64 in both)."""
+@pytest.mark.parametrize("fuse", [2, 1])
+def test_fused_multi_step_equals_single_steps(fuse):
+    """P18: step(5) == 5 x step(1).  FUSE = 1 keeps the operation order (the intermediate row is rounded to fp64
+    in both): bitwise.  FUSE = 2 applies two half shifts with the composite weights W = w * w: round-off."""
     c = inputs.config("cfg5", ntheta=700, npts=260)
-    g = vb.Vlasov(c["model"], c["grid"], c["domain"], c["dt"])
+    g = vb.Vlasov(c["model"], c["grid"], c["domain"], c["dt"], fuse=fuse)
     g.upload(c["f0"])
     g.step(5)
     a = g.download()
     g.close()
-    g = vb.Vlasov(c["model"], c["grid"], c["domain"], c["dt"])
+    g = vb.Vlasov(c["model"], c["grid"], c["domain"], c["dt"], fuse=fuse)
     g.upload(c["f0"])
     for _ in range(5):
         g.step(1)
     b = g.download()
     g.close()
-    assert np.array_equal(a, b)
+    if fuse == 1:
+        assert np.array_equal(a, b)
+    else:
+        assert rel_err(a, b) < 1e-13
+
+
+def test_one_pass_is_reproducible_run_to_run():
+    """The density partials are accumulated with atomic adds of at most two terms per entry: same bits every run."""
+    c = inputs.config("cfg5", ntheta=1500, npts=900)
+    outs = []
+    for _ in range(3):
+        g = vb.Vlasov(c["model"], c["grid"], c["domain"], c["dt"])
+        g.upload(c["f0"])
+        g.step(7)
+        outs.append(g.download())
+        g.close()
+    assert np.array_equal(outs[0], outs[1]) and np.array_equal(outs[0], outs[2])
 
 
 def test_library_owned_buffers_and_checkpoint_roundtrip():

@@ -152,7 +152,9 @@ int vlasov_launch_count(unsigned long long* out);
 int vlasov_kernel_times(double out[12]);
 
 /* Fill out[0..n) (host) with implementation facts for reports: {SM count, theta-kernel CTAs, p-kernel CTAs,
- * bands, warps per theta CTA (2-shift), warps per theta CTA (1-shift)}; returns how many were written. */
+ * bands, warps per theta CTA (2-shift), warps per theta CTA (1-shift), theta1 CTAs, p segment length, p threads,
+ * bulk-copy theta kernel in use, one-pass kernel in use (0/1), its CTAs, bands, rows per band}; returns how many
+ * were written. */
 int vlasov_info(double* out, int n);
 
 void vlasov_free(void);

@@ -198,7 +198,7 @@ def vlasov_info() -> dict:
     buf = np.zeros(16, dtype=np.float64)
     n = _chk(load().vlasov_info(buf.ctypes.data_as(_dp), 16), "vlasov_info")
     names = ["sm_count", "theta2_ctas", "p_ctas", "theta2_bands", "theta2_warps", "theta1_warps", "theta1_ctas",
-             "p_seg_len", "p_threads", "theta_bulk"]
+             "p_seg_len", "p_threads", "theta_bulk", "onepass", "onepass_ctas", "onepass_bands", "onepass_rows_per_band"]
     return {k: int(buf[i]) for i, k in enumerate(names[:n])}
 
 

@@ -27,6 +27,8 @@ constexpr int TB_MINB = 3;       // CTAs per SM the register budget is set for
 constexpr int FU_NT = 384;       // threads per CTA of the one-pass kernel (one per source column)
 constexpr int FU_R = 11;         // consecutive outputs per lane in its theta stage (odd)
 constexpr int FU_NSTG = 3;       // cp.async ring depth (phases of 12 rows)
+constexpr int FU_NW = FU_NT / 32;  // warps of the one-pass kernel = density partial rows per band
+constexpr int FU_PAD = 12;       // rows of padding of the theta weight tables (the last phase of a band reads on)
 constexpr int NCLS = 6;          // profiled kernel classes: theta x1, theta x2, p, rho+force, p+theta x2, p+theta x1
 constexpr int KEY_TUNE_FBANDS = 107;
 constexpr int KEY_TUNE_NW1 = 101, KEY_TUNE_NW2 = 102, KEY_TUNE_BANDS = 103, KEY_TUNE_PSEG = 104,
@@ -59,7 +61,6 @@ struct Ctx {
     int hist_cap = 0, hist_count = 0;
     // one-pass kernel: composite theta weights, band shift ranges, its own density partials
     double *wrow2 = nullptr, *colpart_f = nullptr;
-    int* band_s[3] = {nullptr, nullptr, nullptr};
     int fbands[3] = {0, 0, 0}, frpb[3] = {0, 0, 0}, fcols[3] = {0, 0, 0};
     bool onepass = false;
     int tune_fbands = 0;
@@ -139,13 +140,12 @@ int cdiv(int a, int b) { return (a + b - 1) / b; }
 
 void free_small() {
     void* ptrs[] = {G.srow, G.wrow, G.cos_t, G.sin_t, G.ringK, G.ringV, G.rho, G.force, G.rho_m,
-                    G.phi,  G.mpart, G.pkpart, G.mom_dev, G.hist, G.wrow2, G.colpart_f, G.band_s[1], G.band_s[2]};
+                    G.phi,  G.mpart, G.pkpart, G.mom_dev, G.hist, G.wrow2, G.colpart_f};
     for (void* p : ptrs)
         if (p) cudaFree(p);
     G.srow = nullptr;
     G.wrow = G.cos_t = G.sin_t = G.ringK = G.ringV = G.rho = G.force = G.rho_m = G.phi = G.mpart = G.pkpart =
         G.mom_dev = G.hist = G.wrow2 = G.colpart_f = nullptr;
-    G.band_s[1] = G.band_s[2] = nullptr;
     G.hist_cap = G.hist_count = 0;
 }
 
@@ -231,46 +231,51 @@ int configure_theta_bulk() {
     return VLASOV_OK;
 }
 
-// one-pass kernel (p shift + NST theta half shifts): column blocks x bands, one CTA per SM; a band is short
-// enough that the integer theta shift drifts by at most MAX_DRIFT (and Ntheta) columns inside it
+// one-pass kernel (p shift + NST theta half shifts): column blocks x bands, one CTA per SM.  Conditions: the
+// integer theta shift must not increase with the row (the column sums follow it by moving left), and inside a
+// band it may drift by at most the width of the narrowest column block (then at most two CTAs add to an entry
+// of the density partials).  Sets G.fbands[NST] = 0 when the grid does not qualify.
 template <typename T, int NST>
 int configure_fused() {
     using C = vl::FusedCfg<T, NST, FU_NT, FU_R, FU_NSTG>;
     auto kern = vl::strang_fused_kernel<T, NST, FU_NT, FU_R, FU_NSTG>;
     CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM_BYTES));
-    const int np = G.np;
-    const int cols = cdiv(G.ntheta, C::TI);
+    const int np = G.np, nt = G.ntheta;
+    G.fbands[NST] = 0;
+    for (int j = 1; j < np; ++j)
+        if (G.h_srow[j] > G.h_srow[j - 1]) return VLASOV_OK;  // shift wrapped around the circle: not monotonic
+    if ((double)nt * sizeof(T) >= 2147483648.0) return VLASOV_OK;
+    const int units = cdiv(nt, FU_R);
+    const int cols = cdiv(units, 32);
+    int wmin = nt;
+    for (int c = 0; c < cols; ++c) {
+        int i0, wd;
+        vl::fused_block_range(c, cols, nt, FU_R, &i0, &wd);
+        wmin = wd < wmin ? wd : wmin;
+    }
+    if (wmin < 1) return VLASOV_OK;
     int bands = G.tune_fbands > 0 ? G.tune_fbands : G.sm_count / cols;
     if (bands < 1) bands = 1;
     if (bands > np) bands = np;
     int rpb = cdiv(np, bands);
-    const int limit = C::MAX_DRIFT < G.ntheta ? C::MAX_DRIFT : G.ntheta;
-    std::vector<int> bs;
     for (;;) {
         bands = cdiv(np, rpb);
-        bs.assign((size_t)2 * bands, 0);
         int worst = 0;
         for (int b = 0; b < bands; ++b) {
-            int lo = 1 << 30, hi = -(1 << 30);
-            for (int j = b * rpb; j < np && j < (b + 1) * rpb; ++j) {
-                const int S = NST * G.h_srow[j];
-                lo = S < lo ? S : lo;
-                hi = S > hi ? S : hi;
-            }
-            bs[2 * b + 0] = lo;
-            bs[2 * b + 1] = hi;
-            worst = (hi - lo) > worst ? (hi - lo) : worst;
+            const int ja = b * rpb, jb = (b + 1) * rpb < np ? (b + 1) * rpb : np;
+            const int drift = NST * (G.h_srow[ja] - G.h_srow[jb - 1]);
+            worst = drift > worst ? drift : worst;
         }
-        if (worst <= limit || rpb == 1) break;
+        if (worst <= wmin || rpb == 1) {
+            if (worst > wmin) return VLASOV_OK;
+            break;
+        }
         rpb = (rpb + 1) / 2;
     }
+    if ((size_t)bands * C::NW > (size_t)G.sm_count * 64) return VLASOV_OK;  // partials would outgrow the state
     G.fbands[NST] = bands;
     G.frpb[NST] = rpb;
     G.fcols[NST] = cols;
-    if (G.band_s[NST]) CU(cudaFree(G.band_s[NST]));
-    G.band_s[NST] = nullptr;
-    CU(cudaMalloc(&G.band_s[NST], sizeof(int) * 2 * bands));
-    CU(cudaMemcpy(G.band_s[NST], bs.data(), sizeof(int) * 2 * bands, cudaMemcpyHostToDevice));
     return VLASOV_OK;
 }
 
@@ -288,6 +293,7 @@ int configure_all() {
     if (G.onepass) {
         if ((rc = configure_fused<T, 1>()) != 0) return rc;
         if ((rc = configure_fused<T, 2>()) != 0) return rc;
+        G.onepass = G.fbands[1] > 0 && G.fbands[2] > 0;
     }
     // p shift: 128 adjacent columns per CTA; segments so that a bit more than one wave of CTAs exists
     G.p_tx = G.tune_ptx > 0 ? G.tune_ptx : 128;
@@ -332,7 +338,7 @@ int prepare() {
 
     // per-row shift of one half step: displacement p_j tau (eq (9)), u = -disp/dx cells
     std::vector<int> srow(np);
-    std::vector<double> wrow((size_t)np * vl::WROW_STRIDE, 0.0);
+    std::vector<double> wrow((size_t)(np + FU_PAD) * vl::WROW_STRIDE, 0.0);  // FU_PAD rows of padding
     for (int j = 0; j < np; ++j) {
         const double p = G.pmin + (double)j * dp;
         const double disp = p * tau;
@@ -350,7 +356,7 @@ int prepare() {
     }
     G.h_srow = srow;
     // composite weights of two equal half shifts, W = w * w (19 taps): the one-pass kernel applies both at once
-    std::vector<double> wrow2((size_t)np * 20, 0.0);
+    std::vector<double> wrow2((size_t)(np + FU_PAD) * 20, 0.0);
     for (int j = 0; j < np; ++j) {
         const double* w = &wrow[(size_t)j * vl::WROW_STRIDE];
         double* W = &wrow2[(size_t)j * 20];
@@ -359,9 +365,10 @@ int prepare() {
             for (int m = (n > 9 ? n - 9 : 0); m <= (n < 9 ? n : 9); ++m) acc += w[m] * w[n - m];
             W[n] = acc;
         }
+        W[19] = 2.0 * (double)srow[j];  // integer part of the two half shifts together
     }
-    CU(cudaMalloc(&G.wrow2, sizeof(double) * np * 20));
-    CU(cudaMemcpy(G.wrow2, wrow2.data(), sizeof(double) * np * 20, cudaMemcpyHostToDevice));
+    CU(cudaMalloc(&G.wrow2, sizeof(double) * wrow2.size()));
+    CU(cudaMemcpy(G.wrow2, wrow2.data(), sizeof(double) * wrow2.size(), cudaMemcpyHostToDevice));
     std::vector<double> ct(nt), st(nt);
     for (int i = 0; i < nt; ++i) {
         const double th = G.xmin + (double)i * dx;
@@ -369,11 +376,11 @@ int prepare() {
         st[i] = sin(th);
     }
     CU(cudaMalloc(&G.srow, sizeof(int) * np));
-    CU(cudaMalloc(&G.wrow, sizeof(double) * np * vl::WROW_STRIDE));
+    CU(cudaMalloc(&G.wrow, sizeof(double) * wrow.size()));
     CU(cudaMalloc(&G.cos_t, sizeof(double) * nt));
     CU(cudaMalloc(&G.sin_t, sizeof(double) * nt));
     CU(cudaMemcpy(G.srow, srow.data(), sizeof(int) * np, cudaMemcpyHostToDevice));
-    CU(cudaMemcpy(G.wrow, wrow.data(), sizeof(double) * np * vl::WROW_STRIDE, cudaMemcpyHostToDevice));
+    CU(cudaMemcpy(G.wrow, wrow.data(), sizeof(double) * wrow.size(), cudaMemcpyHostToDevice));
     CU(cudaMemcpy(G.cos_t, ct.data(), sizeof(double) * nt, cudaMemcpyHostToDevice));
     CU(cudaMemcpy(G.sin_t, st.data(), sizeof(double) * nt, cudaMemcpyHostToDevice));
     if (G.model == VLASOV_MODEL_RING) {
@@ -404,7 +411,7 @@ int prepare() {
     if (rc != 0) return rc;
     CU(cudaMalloc(&G.pkpart, sizeof(double) * 2 * (size_t)G.mbands * cdiv(nt, 256)));
     if (G.onepass) {
-        const size_t nb = (size_t)(G.fbands[2] > G.fbands[1] ? G.fbands[2] : G.fbands[1]);
+        const size_t nb = (size_t)(G.fbands[2] > G.fbands[1] ? G.fbands[2] : G.fbands[1]) * FU_NW;
         CU(cudaMalloc(&G.colpart_f, sizeof(double) * nb * nt));
         CU(cudaMemset(G.colpart_f, 0, sizeof(double) * nb * nt));
     }
@@ -500,10 +507,8 @@ int launch_fused(bool want_colsums) {
     a.fin = static_cast<const T*>(G.f[G.cur]);
     a.fout = static_cast<T*>(G.f[G.cur ^ 1]);
     a.force = G.force;
-    a.srow = G.srow;
     a.wtab = NST == 2 ? G.wrow2 : G.wrow;
-    a.wstride = NST == 2 ? 20 : vl::WROW_STRIDE;
-    a.band_s = G.band_s[NST];
+    a.bulk_ok = (G.ntheta % C::EPV == 0) ? 1 : 0;
     a.colpart = want_colsums ? G.colpart_f : nullptr;
     a.ntheta = G.ntheta;
     a.np = G.np;
@@ -766,7 +771,7 @@ int vlasov_step(int n) {
         for (int k = 0; k < n; ++k) {
             prof_begin(3);
             if (k == 0) rc = rho_from_colpart(theta_bands(1), G.rho, hmf);
-            else rc = rho_from_colpart(G.fbands[2], G.rho, hmf, G.colpart_f, true);
+            else rc = rho_from_colpart(G.fbands[2] * FU_NW, G.rho, hmf, G.colpart_f, true);
             if (rc != 0) return rc;
             if ((rc = force_from_rho()) != 0) return rc;                          // eq (10)
             prof_end(3);
@@ -823,10 +828,15 @@ int vlasov_substep(int which) {
         case VLASOV_SUB_P_FULL: return p_pass();
         case VLASOV_SUB_P_THETA_HALF:
         case VLASOV_SUB_P_THETA_TWICE: {
-            if (!G.onepass) return fail(VLASOV_EINVAL, "vlasov_substep: the one-pass kernel needs FUSE = 2 and periodic x");
             const int nst = which == VLASOV_SUB_P_THETA_TWICE ? 2 : 1;
+            if (!G.onepass) {  // grid or shift pattern outside the one-pass kernel's conditions: separate passes
+                if ((rc = p_pass()) != 0) return rc;
+                if ((rc = theta_pass(nst, true)) != 0) return rc;
+                if ((rc = rho_from_colpart(theta_bands(nst), G.rho, G.model == VLASOV_MODEL_HMF)) != 0) return rc;
+                return force_from_rho();
+            }
             if ((rc = fused_pass(nst, true)) != 0) return rc;
-            if ((rc = rho_from_colpart(G.fbands[nst], G.rho, G.model == VLASOV_MODEL_HMF, G.colpart_f, true)) != 0) return rc;
+            if ((rc = rho_from_colpart(G.fbands[nst] * FU_NW, G.rho, G.model == VLASOV_MODEL_HMF, G.colpart_f, true)) != 0) return rc;
             return force_from_rho();
         }
         default: return fail(VLASOV_EINVAL, "vlasov_substep: unknown stage");
@@ -918,7 +928,11 @@ int vlasov_info(double* out, int n) {
                         tb ? (double)G.bctas[1] : (double)G.nchunks[1] * G.nbands[1],
                         (double)G.p_seg,
                         (double)G.p_tx,
-                        tb ? 1.0 : 0.0};
+                        tb ? 1.0 : 0.0,
+                        G.onepass ? 1.0 : 0.0,
+                        (double)G.fcols[2] * G.fbands[2],
+                        (double)G.fbands[2],
+                        (double)G.frpb[2]};
     const int m = (int)(sizeof(v) / sizeof(v[0]));
     const int k = n < m ? n : m;
     for (int q = 0; q < k; ++q) out[q] = v[q];

@@ -133,6 +133,8 @@ def test_one_pass_p_then_theta(grid, bc_p, which, dt, amp):
     for _ in range(which):
         o.theta_sweep(0.5 * dt)
     g.set_force(F)
+    if 0.0 < dt < 1.0:  # moderate forward steps must really take the one-pass kernel (others may fall back)
+        assert g.info()["onepass"] == 1
     g.substep(vb.SUB_P_THETA_TWICE if which == 2 else vb.SUB_P_THETA_HALF)
     fo = o.download()
     assert rel_err(g.download(), fo) < 1e-13

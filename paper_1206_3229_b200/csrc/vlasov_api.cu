@@ -17,6 +17,7 @@
 #include "vlasov_kernels.cuh"
 #include "vlasov_theta_bulk.cuh"
 #include "vlasov_fused.cuh"
+#include "vlasov_fused_ws.cuh"
 
 namespace {
 
@@ -27,7 +28,9 @@ constexpr int TB_MINB = 3;       // CTAs per SM the register budget is set for
 constexpr int FU_NT = 384;       // threads per CTA of the one-pass kernel (one per source column)
 constexpr int FU_R = 11;         // consecutive outputs per lane in its theta stage (odd)
 constexpr int FU_NSTG = 3;       // cp.async ring depth (phases of 12 rows)
-constexpr int FU_NW = FU_NT / 32;  // warps of the one-pass kernel = density partial rows per band
+constexpr int FU_NW = FU_NT / 32;  // density partial rows per band of the one-pass kernel, variant 1 (all warps alike)
+constexpr int FW_NSTG = 3;       // ring depth (groups of 12 rows) of the warp-specialised one-pass kernel (variant 0)
+constexpr int KEY_TUNE_FVARIANT = 108;
 constexpr int FU_PAD = 12;       // rows of padding of the theta weight tables (the last phase of a band reads on)
 constexpr int NCLS = 6;          // profiled kernel classes: theta x1, theta x2, p, rho+force, p+theta x2, p+theta x1
 constexpr int KEY_TUNE_FBANDS = 107;
@@ -64,6 +67,8 @@ struct Ctx {
     int fbands[3] = {0, 0, 0}, frpb[3] = {0, 0, 0}, fcols[3] = {0, 0, 0};
     bool onepass = false;
     int tune_fbands = 0;
+    int fvariant = 0;              // 0: warp-specialised one-pass kernel, 1: every warp does both stages
+    int fnw() const { return fvariant == 1 ? FU_NW : vl::FusedWsCfg<double, 2, FU_R, FW_NSTG>::NTW; }
     std::vector<int> h_srow;
 
     // launch configuration
@@ -238,8 +243,11 @@ int configure_theta_bulk() {
 template <typename T, int NST>
 int configure_fused() {
     using C = vl::FusedCfg<T, NST, FU_NT, FU_R, FU_NSTG>;
-    auto kern = vl::strang_fused_kernel<T, NST, FU_NT, FU_R, FU_NSTG>;
-    CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM_BYTES));
+    using CW = vl::FusedWsCfg<T, NST, FU_R, FW_NSTG>;
+    CU(cudaFuncSetAttribute(vl::strang_fused_kernel<T, NST, FU_NT, FU_R, FU_NSTG>,
+                            cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM_BYTES));
+    CU(cudaFuncSetAttribute(vl::strang_fused_ws_kernel<T, NST, FU_R, FW_NSTG>,
+                            cudaFuncAttributeMaxDynamicSharedMemorySize, (int)CW::SMEM_BYTES));
     const int np = G.np, nt = G.ntheta;
     G.fbands[NST] = 0;
     for (int j = 1; j < np; ++j)
@@ -272,7 +280,7 @@ int configure_fused() {
         }
         rpb = (rpb + 1) / 2;
     }
-    if ((size_t)bands * C::NW > (size_t)G.sm_count * 64) return VLASOV_OK;  // partials would outgrow the state
+    if ((size_t)bands * G.fnw() > (size_t)G.sm_count * 64) return VLASOV_OK;  // partials would outgrow the state
     G.fbands[NST] = bands;
     G.frpb[NST] = rpb;
     G.fcols[NST] = cols;
@@ -411,7 +419,7 @@ int prepare() {
     if (rc != 0) return rc;
     CU(cudaMalloc(&G.pkpart, sizeof(double) * 2 * (size_t)G.mbands * cdiv(nt, 256)));
     if (G.onepass) {
-        const size_t nb = (size_t)(G.fbands[2] > G.fbands[1] ? G.fbands[2] : G.fbands[1]) * FU_NW;
+        const size_t nb = (size_t)(G.fbands[2] > G.fbands[1] ? G.fbands[2] : G.fbands[1]) * G.fnw();
         CU(cudaMalloc(&G.colpart_f, sizeof(double) * nb * nt));
         CU(cudaMemset(G.colpart_f, 0, sizeof(double) * nb * nt));
     }
@@ -518,7 +526,12 @@ int launch_fused(bool want_colsums) {
     a.dp = (G.pmax - G.pmin) / (double)G.np;
     dim3 grid(G.fcols[NST], G.fbands[NST]);
     prof_begin(NST == 2 ? 4 : 5);
-    vl::strang_fused_kernel<T, NST, FU_NT, FU_R, FU_NSTG><<<grid, FU_NT, C::SMEM_BYTES, G.stream>>>(a);
+    if (G.fvariant == 1) {
+        vl::strang_fused_kernel<T, NST, FU_NT, FU_R, FU_NSTG><<<grid, FU_NT, C::SMEM_BYTES, G.stream>>>(a);
+    } else {
+        using CW = vl::FusedWsCfg<T, NST, FU_R, FW_NSTG>;
+        vl::strang_fused_ws_kernel<T, NST, FU_R, FW_NSTG><<<grid, CW::NT, CW::SMEM_BYTES, G.stream>>>(a);
+    }
     prof_end(NST == 2 ? 4 : 5);
     LAUNCH_CHECK();
     G.cur ^= 1;
@@ -679,6 +692,7 @@ int vlasov_set_param(int key, double value) {
             G.fuse = (int)value;
             break;
         case KEY_TUNE_FBANDS: G.tune_fbands = (int)value; break;
+        case KEY_TUNE_FVARIANT: G.fvariant = (value != 0.0) ? 1 : 0; break;
         case VLASOV_KEY_PROFILE: G.profile = (value != 0.0); break;
         case KEY_TUNE_NW1: G.tune_nw1 = (int)value; break;
         case KEY_TUNE_NW2: G.tune_nw2 = (int)value; break;
@@ -771,7 +785,7 @@ int vlasov_step(int n) {
         for (int k = 0; k < n; ++k) {
             prof_begin(3);
             if (k == 0) rc = rho_from_colpart(theta_bands(1), G.rho, hmf);
-            else rc = rho_from_colpart(G.fbands[2] * FU_NW, G.rho, hmf, G.colpart_f, true);
+            else rc = rho_from_colpart(G.fbands[2] * G.fnw(), G.rho, hmf, G.colpart_f, true);
             if (rc != 0) return rc;
             if ((rc = force_from_rho()) != 0) return rc;                          // eq (10)
             prof_end(3);
@@ -836,7 +850,7 @@ int vlasov_substep(int which) {
                 return force_from_rho();
             }
             if ((rc = fused_pass(nst, true)) != 0) return rc;
-            if ((rc = rho_from_colpart(G.fbands[nst] * FU_NW, G.rho, G.model == VLASOV_MODEL_HMF, G.colpart_f, true)) != 0) return rc;
+            if ((rc = rho_from_colpart(G.fbands[nst] * G.fnw(), G.rho, G.model == VLASOV_MODEL_HMF, G.colpart_f, true)) != 0) return rc;
             return force_from_rho();
         }
         default: return fail(VLASOV_EINVAL, "vlasov_substep: unknown stage");

@@ -1,0 +1,365 @@
+// vlasov_fused_ws.cuh -- the one-pass Strang kernel (see vlasov_fused.cuh for the method and the geometry) with
+// WARP SPECIALISATION: the momentum shift and the theta shifts run concurrently on different warps of the CTA.
+//
+//   p warps (4)      thread t owns the three source columns t, t + 128, t + 256 of the CTA.  For each column a
+//                    register window slides down (one new value + ten FMAs per row, eq (11)); new values
+//                    arrive by per-thread cp.async into a ring of NSTG groups of 12 rows; the shifted value
+//                    overwrites the tap in place.  After every 4 rows ("sub-slot") the warp arrives on the
+//                    sub-slot's READY mbarrier.  Before refilling a group it waits for the EMPTY mbarriers of its
+//                    three sub-slots.
+//   theta warps (8)  warp w takes the rows r = w (mod 8) of the band: waits READY of the row's sub-slot, pulls its
+//                    window of the row into registers, arrives on EMPTY (the ring row is free again), applies the
+//                    NTAP composite theta weights (eqs (12), (9)), keeps the column sums (eq (10)) and hands the
+//                    row to the bulk-copy engine.  The weights of its next row are prefetched (cp.async) into a
+//                    private two-entry buffer.
+// No block-wide barrier after the set-up: the fp64 pipe sees a p warp and two theta warps per scheduler, each an
+// uninterrupted stream of FMAs, instead of twelve warps that all load, all multiply and all store in step.
+#pragma once
+#include <type_traits>
+
+#include "vlasov_fused.cuh"
+
+namespace vl {
+
+template <typename T, int NST, int R, int NSTG>
+struct FusedWsCfg {
+    static constexpr int NPW = 4, NTW = 8;              // p warps, theta warps
+    static constexpr int NT = (NPW + NTW) * 32;
+    static constexpr int NPT = NPW * 32;                // p threads
+    static constexpr int CPT = 3;                       // columns per p thread
+    static constexpr int PITCH = NPT * CPT;             // columns of a ring row
+    static constexpr int RG = 12;                       // rows per group = length of the register ring
+    static constexpr int SUB = 4;                       // rows per sub-slot (granularity of READY / EMPTY)
+    static constexpr int SPG = RG / SUB;                // sub-slots per group
+    static constexpr int NSUB = NSTG * SPG;
+    static constexpr int NTAP = NST == 2 ? 19 : 10;
+    static constexpr int WST = NST == 2 ? 20 : WROW_STRIDE;
+    static constexpr int TI = 32 * R;
+    static constexpr int NTA = TI + NTAP - 1;
+    static constexpr int EPV = 16 / (int)sizeof(T);
+    static constexpr int OB = (TI + EPV + EPV - 1) / EPV * EPV;
+    static constexpr size_t RING_BYTES = (size_t)NSTG * RG * PITCH * sizeof(T);
+    static constexpr size_t O_BYTES = (size_t)NTW * 2 * OB * sizeof(T);
+    static constexpr size_t W_BYTES = (size_t)NTW * 2 * WST * sizeof(double);
+    static constexpr size_t BAR_BYTES = (size_t)2 * NSUB * sizeof(uint64_t);
+    static constexpr size_t SMEM_BYTES = RING_BYTES + O_BYTES + W_BYTES + BAR_BYTES;
+    static constexpr int W_COPIES = WST * 8 / 16;
+    static_assert(NTA <= PITCH, "source columns must fit the ring row");
+    static_assert(R & 1, "lane stride R must be odd (shared-memory banks)");
+    static_assert(NTW == 2 * SUB, "a sub-slot is released by SUB different theta warps");
+    static_assert(RING_BYTES % 16 == 0 && O_BYTES % 16 == 0 && W_BYTES % 16 == 0, "");
+    static_assert(NSTG >= 2 && W_COPIES <= 32, "");
+};
+
+template <typename T, int NST, int R, int NSTG>
+__global__ void __launch_bounds__(384, 1) strang_fused_ws_kernel(const FusedArgs<T> arg) {
+    using C = FusedWsCfg<T, NST, R, NSTG>;
+    constexpr int NTAP = C::NTAP, NTA = C::NTA, WST = C::WST, EPV = C::EPV, OB = C::OB, PITCH = C::PITCH, RG = C::RG,
+                  SUB = C::SUB, SPG = C::SPG, NSUB = C::NSUB, CPT = C::CPT, NPT = C::NPT, NTW = C::NTW;
+    constexpr unsigned FULL = 0xffffffffu;
+
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    T* ring = reinterpret_cast<T*>(smem_raw);                                                  // [NSTG][RG][PITCH]
+    T* obuf = reinterpret_cast<T*>(smem_raw + C::RING_BYTES);                                  // [NTW][2][OB]
+    double* wbuf = reinterpret_cast<double*>(smem_raw + C::RING_BYTES + C::O_BYTES);           // [NTW][2][WST]
+    uint64_t* ready = reinterpret_cast<uint64_t*>(smem_raw + C::RING_BYTES + C::O_BYTES + C::W_BYTES);  // [NSUB]
+    uint64_t* empty = ready + NSUB;                                                            // [NSUB]
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int ntheta = arg.ntheta, np = arg.np;
+    int i0, qmax;
+    fused_block_range((int)blockIdx.x, (int)gridDim.x, ntheta, R, &i0, &qmax);
+    const int band = blockIdx.y;
+    const int jA = band * arg.rows_per_band;
+    const int nrows = min(np, jA + arg.rows_per_band) - jA;
+    if (nrows <= 0 || qmax <= 0) return;  // whole CTA
+    const int ngroups = (nrows + RG - 1) / RG;
+    const unsigned pitch = (unsigned)ntheta;
+
+    if (tid == 0) {
+#pragma unroll
+        for (int k = 0; k < NSUB; ++k) {
+            ptx::mbar_init(&ready[k], C::NPW);
+            ptx::mbar_init(&empty[k], SUB);
+        }
+        ptx::fence_mbar_init();
+    }
+    __syncthreads();
+
+    if (warp < C::NPW) {
+        // =========================== p warps: momentum shift (eq (11)) ===========================
+        const bool p_periodic = (arg.bc_p == BC_PERIODIC);
+        bool act[CPT];
+        const T* col[CPT];
+        int rn[CPT];
+        T w[CPT][10];
+        T v[CPT][12];  // register rings: taps of output row r of a group are v[k][(r + m) % 12]
+#pragma unroll
+        for (int k = 0; k < CPT; ++k) {
+            const int q = tid + k * NPT;
+            act[k] = q < NTA;
+            const int c = wrap_index(i0 - 4 * NST + q, ntheta);
+            double sf, a;
+            split_shift(-((act[k] ? arg.force[c] : 0.0) * arg.dt) / arg.dp, &sf, &a);
+            int s;
+            if (p_periodic) {
+                sf = fmod(sf, (double)np);
+                s = (int)sf;
+                if (s < 0) s += np;
+            } else {
+                const double lim = (double)np + 64.0;
+                s = (int)fmin(fmax(sf, -lim), lim);
+            }
+            double wd[10];
+            spline_fd8_weights(a, wd);
+#pragma unroll
+            for (int m = 0; m < 10; ++m) w[k][m] = (T)wd[m];
+            col[k] = arg.fin + c;
+            // row of tap m of output row j is j + s + m - 4; rn = row of the next value the window has not seen
+            rn[k] = jA + s - 4;
+            if (p_periodic) rn[k] = wrap_index(rn[k], np);
+        }
+#pragma unroll
+        for (int k = 0; k < CPT; ++k) {
+#pragma unroll
+            for (int m = 0; m < 9; ++m) {
+                const bool ok = act[k] && (p_periodic || (unsigned)rn[k] < (unsigned)np);
+                v[k][m] = ok ? __ldg(col[k] + (size_t)rn[k] * pitch) : T(0);
+                ++rn[k];
+                if (p_periodic && rn[k] >= np) rn[k] = 0;
+            }
+            v[k][9] = v[k][10] = v[k][11] = T(0);
+        }
+
+        const uint32_t ring_u32 = ptx::smem_u32(ring) + (uint32_t)tid * (uint32_t)sizeof(T);
+        // new taps of the RG rows of a group -> ring slot `slot`
+        auto issue_group = [&](int slot) {
+            const uint32_t dst0 = ring_u32 + (uint32_t)slot * (uint32_t)(RG * PITCH * sizeof(T));
+#pragma unroll
+            for (int k = 0; k < CPT; ++k) {
+                if (!act[k]) continue;
+                const uint32_t dst = dst0 + (uint32_t)(k * NPT * sizeof(T));
+                if (rn[k] >= 0 && rn[k] + RG <= np) {  // all RG rows exist: no per-row tests
+                    const T* src = col[k] + (long long)rn[k] * (long long)pitch;
+#pragma unroll
+                    for (int r = 0; r < RG; ++r)
+                        ptx::cp_async<(int)sizeof(T)>(dst + (uint32_t)(r * PITCH * sizeof(T)),
+                                                      src + (size_t)((unsigned)r * pitch));
+                    rn[k] += RG;
+                    if (p_periodic && rn[k] >= np) rn[k] = 0;
+                } else {
+#pragma unroll
+                    for (int r = 0; r < RG; ++r) {
+                        const bool ok = p_periodic || (unsigned)rn[k] < (unsigned)np;
+                        const T* src = ok ? col[k] + (size_t)rn[k] * pitch : arg.fin;
+                        ptx::cp_async_zfill<(int)sizeof(T)>(dst + (uint32_t)(r * PITCH * sizeof(T)), src,
+                                                            ok ? (unsigned)sizeof(T) : 0u);
+                        ++rn[k];
+                        if (p_periodic && rn[k] >= np) rn[k] = 0;
+                    }
+                }
+            }
+        };
+
+#pragma unroll
+        for (int st = 0; st < NSTG - 1; ++st) {
+            if (st < ngroups) issue_group(st);
+            ptx::cp_async_commit();
+        }
+
+        int slot = 0;
+        for (int g = 0; g < ngroups; ++g) {
+            ptx::cp_async_wait<NSTG - 2>();  // this thread's copies of group g have landed
+            T* sl = ring + (size_t)slot * (RG * PITCH) + tid;
+#pragma unroll
+            for (int sub = 0; sub < SPG; ++sub) {
+#pragma unroll
+                for (int rr = 0; rr < SUB; ++rr) {
+                    const int r = sub * SUB + rr;
+#pragma unroll
+                    for (int k = 0; k < CPT; ++k) {
+                        if (!act[k]) continue;
+                        v[k][(r + 9) % 12] = sl[r * PITCH + k * NPT];
+                        T acc = w[k][0] * v[k][r % 12];
+#pragma unroll
+                        for (int m = 1; m < 10; ++m) acc = fma(w[k][m], v[k][(r + m) % 12], acc);
+                        sl[r * PITCH + k * NPT] = acc;
+                    }
+                }
+                __syncwarp();
+                if (lane == 0) ptx::mbar_arrive(&ready[slot * SPG + sub]);
+            }
+            // refill the slot of group g - 1 with group g + NSTG - 1 once the theta warps have let go of it
+            const int gn = g + NSTG - 1;
+            int nslot = slot + NSTG - 1;
+            if (nslot >= NSTG) nslot -= NSTG;
+            if (gn < ngroups) {
+                if (gn >= NSTG) {
+                    const unsigned par = (unsigned)((gn / NSTG) - 1) & 1u;
+#pragma unroll
+                    for (int sub = 0; sub < SPG; ++sub) ptx::mbar_wait(&empty[nslot * SPG + sub], par);
+                }
+                issue_group(nslot);
+            }
+            ptx::cp_async_commit();
+            if (++slot == NSTG) slot = 0;
+        }
+        ptx::cp_async_wait<0>();
+        return;
+    }
+
+    // =========================== theta warps: eqs (12), (9), (10) ===========================
+    const int tw = warp - C::NPW;
+    double* wb = wbuf + (size_t)tw * 2 * WST;
+    const uint32_t wb_u32 = ptx::smem_u32(wb) + (uint32_t)lane * 16u;
+    auto prefetch_w = [&](int r, int buf) {  // weight row of band row r -> private buffer `buf`
+        if (lane < C::W_COPIES) {
+            const char* src = reinterpret_cast<const char*>(arg.wtab + (size_t)(jA + r) * WST) + lane * 16;
+            ptx::cp_async<16>(wb_u32 + (uint32_t)(buf * WST * sizeof(double)), src);
+        }
+    };
+
+    double csum[R];
+#pragma unroll
+    for (int k = 0; k < R; ++k) csum[k] = 0.0;
+    const int nv = max(0, min(R, qmax - lane * R));  // valid outputs of this lane
+    int curS = 0, cbase = 0;                         // shift of the rows summed so far, output column of q = 0
+    bool have = false;
+    double* __restrict__ cpw = arg.colpart ? arg.colpart + ((size_t)band * NTW + tw) * (size_t)ntheta : nullptr;
+
+    // one column leaves on the left (its sum is final for this warp), K columns enter on the right
+    auto shift_sums = [&](auto kc) {
+        constexpr int K = decltype(kc)::value;
+#pragma unroll
+        for (int u = 0; u < K; ++u) {
+            if (lane == 0 && cpw != nullptr) {
+                int cidx = cbase + u;
+                if (cidx >= ntheta) cidx -= ntheta;
+                ptx::red_add_f64(cpw + cidx, csum[u]);
+            }
+        }
+        double in[K];
+#pragma unroll
+        for (int u = 0; u < K; ++u) {
+            in[u] = __shfl_down_sync(FULL, csum[u], 1);
+            if (lane == 31) in[u] = 0.0;
+        }
+#pragma unroll
+        for (int k = 0; k + K < R; ++k) csum[k] = csum[k + K];
+#pragma unroll
+        for (int u = 0; u < K; ++u) csum[R - K + u] = in[u];
+        curS -= K;
+        cbase += K;
+        if (cbase >= ntheta) cbase -= ntheta;
+    };
+
+    if (tw < nrows) prefetch_w(tw, 0);
+    ptx::cp_async_commit();
+
+    int it = 0;
+    for (int r = tw; r < nrows; r += NTW, ++it) {
+        if (r + NTW < nrows) prefetch_w(r + NTW, (it + 1) & 1);
+        ptx::cp_async_commit();
+        ptx::cp_async_wait<1>();
+        __syncwarp();  // the weight row of r is visible to every lane
+        const double* Wr = wb + (it & 1) * WST;
+
+        const int grp = r / RG, rin = r - grp * RG;
+        const int slot = grp % NSTG;
+        const int sidx = slot * SPG + rin / SUB;
+        ptx::mbar_wait(&ready[sidx], (unsigned)(grp / NSTG) & 1u);
+
+        const T* grow = ring + ((size_t)slot * RG + rin) * PITCH + lane * R;
+        T x[R + NTAP - 1];
+#pragma unroll
+        for (int k = 0; k < R + NTAP - 1; ++k) x[k] = grow[k];
+        __syncwarp();
+        if (lane == 0) ptx::mbar_arrive(&empty[sidx]);  // the ring row may be refilled
+
+        const int S = (int)Wr[NTAP];
+        if (!have) {
+            curS = S;
+            cbase = wrap_index(i0 - S, ntheta);
+            have = true;
+        }
+        while (curS - S >= 2) shift_sums(std::integral_constant<int, 2>());
+        if (curS > S) shift_sums(std::integral_constant<int, 1>());
+
+        T out[R];
+        {
+            const T W0 = (T)Wr[0];
+#pragma unroll
+            for (int q = 0; q < R; ++q) out[q] = W0 * x[q];
+        }
+#pragma unroll
+        for (int n = 1; n < NTAP; ++n) {
+            const T Wn = (T)Wr[n];
+#pragma unroll
+            for (int q = 0; q < R; ++q) out[q] = fma(Wn, x[q + n], out[q]);
+        }
+
+        if (nv == R) {
+#pragma unroll
+            for (int q = 0; q < R; ++q) csum[q] += (double)out[q];
+        } else if (nv > 0) {
+#pragma unroll
+            for (int q = 0; q < R; ++q)
+                if (q < nv) csum[q] += (double)out[q];
+        }
+
+        // the tile used two rows ago must have been read by the copy engine
+        if (lane == 0) ptx::bulk_wait_read<1>();
+        __syncwarp();
+        T* O = obuf + (size_t)(tw * 2 + (it & 1)) * OB;
+        const int base = cbase;  // output column of q = 0: wrap(i0 - S)
+        T* __restrict__ orow = arg.fout + (size_t)(jA + r) * pitch;
+        if (arg.bulk_ok) {
+            const int al = base & (EPV - 1);
+#pragma unroll
+            for (int q = 0; q < R; ++q) O[al + lane * R + q] = out[q];
+            ptx::fence_proxy_async_smem();
+            __syncwarp();
+            // q in [qb, qb + len) -> columns [gcol, gcol + len): aligned body by the copy engine, edges by lanes
+            auto store_piece = [&](int qb, int len, int gcol) {
+                T* dst = orow + gcol;
+                const T* src = O + al + qb;
+                const int h = min(len, (EPV - (gcol & (EPV - 1))) & (EPV - 1));
+                const int nb = (len - h) & ~(EPV - 1);
+                const int t0 = h + nb;
+                if (lane < h) dst[lane] = src[lane];
+                if (lane < len - t0) dst[t0 + lane] = src[t0 + lane];
+                if (lane == 0 && nb > 0) ptx::bulk_s2g(dst + h, src + h, (unsigned)(nb * sizeof(T)));
+            };
+            const int qa = min(qmax, ntheta - base);
+            store_piece(0, qa, base);
+            if (qa < qmax) store_piece(qa, qmax - qa, 0);
+            if (lane == 0) ptx::bulk_commit();
+        } else {
+#pragma unroll
+            for (int q = 0; q < R; ++q) O[lane * R + q] = out[q];
+            __syncwarp();
+            for (int q = lane; q < qmax; q += 32) {
+                int i = base + q;
+                if (i >= ntheta) i -= ntheta;
+                orow[i] = O[q];
+            }
+        }
+        __syncwarp();  // every lane is done with this row's weights before the next prefetch overwrites them
+    }
+    ptx::cp_async_wait<0>();
+    if (lane == 0) ptx::bulk_wait_read<0>();
+
+    if (cpw != nullptr && have) {
+#pragma unroll
+        for (int q = 0; q < R; ++q) {
+            if (q < nv && csum[q] != 0.0) {
+                int cidx = cbase + lane * R + q;
+                if (cidx >= ntheta) cidx -= ntheta;
+                if (cidx >= ntheta) cidx -= ntheta;
+                ptx::red_add_f64(cpw + cidx, csum[q]);
+            }
+        }
+    }
+}
+
+}  // namespace vl

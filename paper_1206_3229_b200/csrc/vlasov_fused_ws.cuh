@@ -10,7 +10,7 @@
 //   theta warps (8)  warp w takes the rows r = w (mod 8) of the band: waits READY of the row's sub-slot, pulls its
 //                    window of the row into registers, arrives on EMPTY (the ring row is free again), applies the
 //                    NTAP composite theta weights (eqs (12), (9)), keeps the column sums (eq (10)) and hands the
-//                    row to the bulk-copy engine.  The weights of its next row are prefetched (cp.async) into a
+//                    row on through a private shared tile (coalesced stores).  The weights of its next row are prefetched (cp.async) into a
 //                    private two-entry buffer.
 // No block-wide barrier after the set-up: the fp64 pipe sees a p warp and two theta warps per scheduler, each an
 // uninterrupted stream of FMAs, instead of twelve warps that all load, all multiply and all store in step.
@@ -177,8 +177,7 @@ __global__ void __launch_bounds__(384, 1) strang_fused_ws_kernel(const FusedArgs
                 for (int rr = 0; rr < SUB; ++rr) {
                     const int r = sub * SUB + rr;
 #pragma unroll
-                    for (int k = 0; k < CPT; ++k) {
-                        if (!act[k]) continue;
+                    for (int k = 0; k < CPT; ++k) {  // columns beyond NTA compute on whatever the ring holds: never read
                         v[k][(r + 9) % 12] = sl[r * PITCH + k * NPT];
                         T acc = w[k][0] * v[k][r % 12];
 #pragma unroll
@@ -307,47 +306,33 @@ __global__ void __launch_bounds__(384, 1) strang_fused_ws_kernel(const FusedArgs
                 if (q < nv) csum[q] += (double)out[q];
         }
 
-        // the tile used two rows ago must have been read by the copy engine
-        if (lane == 0) ptx::bulk_wait_read<1>();
-        __syncwarp();
+        // transpose through the warp's private tile (two tiles alternate: no barrier after the reads), then
+        // coalesced stores: 32 consecutive columns per instruction
         T* O = obuf + (size_t)(tw * 2 + (it & 1)) * OB;
+#pragma unroll
+        for (int q = 0; q < R; ++q) O[lane * R + q] = out[q];
+        __syncwarp();
         const int base = cbase;  // output column of q = 0: wrap(i0 - S)
         T* __restrict__ orow = arg.fout + (size_t)(jA + r) * pitch;
-        if (arg.bulk_ok) {
-            const int al = base & (EPV - 1);
+        if (base + qmax <= ntheta) {  // the row does not cross the periodic boundary
+            T* __restrict__ dst = orow + base + lane;
 #pragma unroll
-            for (int q = 0; q < R; ++q) O[al + lane * R + q] = out[q];
-            ptx::fence_proxy_async_smem();
-            __syncwarp();
-            // q in [qb, qb + len) -> columns [gcol, gcol + len): aligned body by the copy engine, edges by lanes
-            auto store_piece = [&](int qb, int len, int gcol) {
-                T* dst = orow + gcol;
-                const T* src = O + al + qb;
-                const int h = min(len, (EPV - (gcol & (EPV - 1))) & (EPV - 1));
-                const int nb = (len - h) & ~(EPV - 1);
-                const int t0 = h + nb;
-                if (lane < h) dst[lane] = src[lane];
-                if (lane < len - t0) dst[t0 + lane] = src[t0 + lane];
-                if (lane == 0 && nb > 0) ptx::bulk_s2g(dst + h, src + h, (unsigned)(nb * sizeof(T)));
-            };
-            const int qa = min(qmax, ntheta - base);
-            store_piece(0, qa, base);
-            if (qa < qmax) store_piece(qa, qmax - qa, 0);
-            if (lane == 0) ptx::bulk_commit();
+            for (int k = 0; k < R; ++k)
+                if (lane + 32 * k < qmax) dst[32 * k] = O[lane + 32 * k];
         } else {
 #pragma unroll
-            for (int q = 0; q < R; ++q) O[lane * R + q] = out[q];
-            __syncwarp();
-            for (int q = lane; q < qmax; q += 32) {
-                int i = base + q;
-                if (i >= ntheta) i -= ntheta;
-                orow[i] = O[q];
+            for (int k = 0; k < R; ++k) {
+                const int q = lane + 32 * k;
+                if (q < qmax) {
+                    int i = base + q;
+                    if (i >= ntheta) i -= ntheta;
+                    orow[i] = O[q];
+                }
             }
         }
         __syncwarp();  // every lane is done with this row's weights before the next prefetch overwrites them
     }
     ptx::cp_async_wait<0>();
-    if (lane == 0) ptx::bulk_wait_read<0>();
 
     if (cpw != nullptr && have) {
 #pragma unroll

@@ -30,6 +30,7 @@ constexpr int FU_R = 11;         // consecutive outputs per lane in its theta st
 constexpr int FU_NSTG = 3;       // cp.async ring depth (phases of 12 rows)
 constexpr int FU_NW = FU_NT / 32;  // density partial rows per band of the one-pass kernel, variant 1 (all warps alike)
 constexpr int FW_NSTG = 3;       // ring depth (groups of 12 rows) of the warp-specialised one-pass kernel (variant 0)
+constexpr int FW_NTW = 8;        // its theta warps (8 or 12)
 constexpr int KEY_TUNE_FVARIANT = 108;
 constexpr int FU_PAD = 12;       // rows of padding of the theta weight tables (the last phase of a band reads on)
 constexpr int NCLS = 6;          // profiled kernel classes: theta x1, theta x2, p, rho+force, p+theta x2, p+theta x1
@@ -68,7 +69,7 @@ struct Ctx {
     bool onepass = false;
     int tune_fbands = 0;
     int fvariant = 0;              // 0: warp-specialised one-pass kernel, 1: every warp does both stages
-    int fnw() const { return fvariant == 1 ? FU_NW : vl::FusedWsCfg<double, 2, FU_R, FW_NSTG>::NTW; }
+    int fnw() const { return fvariant == 1 ? FU_NW : vl::FusedWsCfg<double, 2, FU_R, FW_NSTG, FW_NTW>::NTW; }
     std::vector<int> h_srow;
 
     // launch configuration
@@ -243,10 +244,10 @@ int configure_theta_bulk() {
 template <typename T, int NST>
 int configure_fused() {
     using C = vl::FusedCfg<T, NST, FU_NT, FU_R, FU_NSTG>;
-    using CW = vl::FusedWsCfg<T, NST, FU_R, FW_NSTG>;
+    using CW = vl::FusedWsCfg<T, NST, FU_R, FW_NSTG, FW_NTW>;
     CU(cudaFuncSetAttribute(vl::strang_fused_kernel<T, NST, FU_NT, FU_R, FU_NSTG>,
                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM_BYTES));
-    CU(cudaFuncSetAttribute(vl::strang_fused_ws_kernel<T, NST, FU_R, FW_NSTG>,
+    CU(cudaFuncSetAttribute(vl::strang_fused_ws_kernel<T, NST, FU_R, FW_NSTG, FW_NTW>,
                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)CW::SMEM_BYTES));
     const int np = G.np, nt = G.ntheta;
     G.fbands[NST] = 0;
@@ -529,8 +530,8 @@ int launch_fused(bool want_colsums) {
     if (G.fvariant == 1) {
         vl::strang_fused_kernel<T, NST, FU_NT, FU_R, FU_NSTG><<<grid, FU_NT, C::SMEM_BYTES, G.stream>>>(a);
     } else {
-        using CW = vl::FusedWsCfg<T, NST, FU_R, FW_NSTG>;
-        vl::strang_fused_ws_kernel<T, NST, FU_R, FW_NSTG><<<grid, CW::NT, CW::SMEM_BYTES, G.stream>>>(a);
+        using CW = vl::FusedWsCfg<T, NST, FU_R, FW_NSTG, FW_NTW>;
+        vl::strang_fused_ws_kernel<T, NST, FU_R, FW_NSTG, FW_NTW><<<grid, CW::NT, CW::SMEM_BYTES, G.stream>>>(a);
     }
     prof_end(NST == 2 ? 4 : 5);
     LAUNCH_CHECK();

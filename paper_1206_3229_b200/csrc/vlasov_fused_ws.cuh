@@ -21,9 +21,9 @@
 
 namespace vl {
 
-template <typename T, int NST, int R, int NSTG>
+template <typename T, int NST, int R, int NSTG, int NTW_ = 8>
 struct FusedWsCfg {
-    static constexpr int NPW = 4, NTW = 8;              // p warps, theta warps
+    static constexpr int NPW = 4, NTW = NTW_;            // p warps (one warpgroup), theta warps (two or three warpgroups)
     static constexpr int NT = (NPW + NTW) * 32;
     static constexpr int NPT = NPW * 32;                // p threads
     static constexpr int CPT = 3;                       // columns per p thread
@@ -46,14 +46,18 @@ struct FusedWsCfg {
     static constexpr int W_COPIES = WST * 8 / 16;
     static_assert(NTA <= PITCH, "source columns must fit the ring row");
     static_assert(R & 1, "lane stride R must be odd (shared-memory banks)");
-    static_assert(NTW == 2 * SUB, "a sub-slot is released by SUB different theta warps");
+    static_assert(NTW % SUB == 0 && NTW <= RG, "a sub-slot is released by SUB different theta warps");
+    // registers per thread after setmaxnreg: 128*152 + 384*120 = 65536; 128*152 + 256*176 = 64512
+    static constexpr int P_REGS = 152, T_REGS = NTW == 12 ? 120 : 176;
+    static constexpr int LAUNCH_REGS = 65536 / NT / 8 * 8;
+    static_assert(NPW * 32 * P_REGS + NTW * 32 * T_REGS <= 65536 && P_REGS % 8 == 0 && T_REGS % 8 == 0, "");
     static_assert(RING_BYTES % 16 == 0 && O_BYTES % 16 == 0 && W_BYTES % 16 == 0, "");
     static_assert(NSTG >= 2 && W_COPIES <= 32, "");
 };
 
-template <typename T, int NST, int R, int NSTG>
-__global__ void __launch_bounds__(384, 1) strang_fused_ws_kernel(const FusedArgs<T> arg) {
-    using C = FusedWsCfg<T, NST, R, NSTG>;
+template <typename T, int NST, int R, int NSTG, int NTW_>
+__global__ void __launch_bounds__((4 + NTW_) * 32, 1) strang_fused_ws_kernel(const FusedArgs<T> arg) {
+    using C = FusedWsCfg<T, NST, R, NSTG, NTW_>;
     constexpr int NTAP = C::NTAP, NTA = C::NTA, WST = C::WST, EPV = C::EPV, OB = C::OB, PITCH = C::PITCH, RG = C::RG,
                   SUB = C::SUB, SPG = C::SPG, NSUB = C::NSUB, CPT = C::CPT, NPT = C::NPT, NTW = C::NTW;
     constexpr unsigned FULL = 0xffffffffu;
@@ -85,8 +89,11 @@ __global__ void __launch_bounds__(384, 1) strang_fused_ws_kernel(const FusedArgs
         ptx::fence_mbar_init();
     }
     __syncthreads();
+    const uint32_t ready_u32 = ptx::smem_u32(ready), empty_u32 = ptx::smem_u32(empty);
 
     if (warp < C::NPW) {
+        if (C::P_REGS > C::LAUNCH_REGS) asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(C::P_REGS));
+        else asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(C::P_REGS));
         // =========================== p warps: momentum shift (eq (11)) ===========================
         const bool p_periodic = (arg.bc_p == BC_PERIODIC);
         bool act[CPT];
@@ -186,7 +193,7 @@ __global__ void __launch_bounds__(384, 1) strang_fused_ws_kernel(const FusedArgs
                     }
                 }
                 __syncwarp();
-                if (lane == 0) ptx::mbar_arrive(&ready[slot * SPG + sub]);
+                if (lane == 0) ptx::mbar_arrive_u32(ready_u32 + (uint32_t)((slot * SPG + sub) * 8));
             }
             // refill the slot of group g - 1 with group g + NSTG - 1 once the theta warps have let go of it
             const int gn = g + NSTG - 1;
@@ -196,7 +203,8 @@ __global__ void __launch_bounds__(384, 1) strang_fused_ws_kernel(const FusedArgs
                 if (gn >= NSTG) {
                     const unsigned par = (unsigned)((gn / NSTG) - 1) & 1u;
 #pragma unroll
-                    for (int sub = 0; sub < SPG; ++sub) ptx::mbar_wait(&empty[nslot * SPG + sub], par);
+                    for (int sub = 0; sub < SPG; ++sub)
+                        ptx::mbar_wait_u32(empty_u32 + (uint32_t)((nslot * SPG + sub) * 8), par);
                 }
                 issue_group(nslot);
             }
@@ -208,15 +216,21 @@ __global__ void __launch_bounds__(384, 1) strang_fused_ws_kernel(const FusedArgs
     }
 
     // =========================== theta warps: eqs (12), (9), (10) ===========================
-    const int tw = warp - C::NPW;
-    double* wb = wbuf + (size_t)tw * 2 * WST;
-    const uint32_t wb_u32 = ptx::smem_u32(wb) + (uint32_t)lane * 16u;
-    auto prefetch_w = [&](int r, int buf) {  // weight row of band row r -> private buffer `buf`
-        if (lane < C::W_COPIES) {
-            const char* src = reinterpret_cast<const char*>(arg.wtab + (size_t)(jA + r) * WST) + lane * 16;
-            ptx::cp_async<16>(wb_u32 + (uint32_t)(buf * WST * sizeof(double)), src);
-        }
-    };
+    if (C::T_REGS > C::LAUNCH_REGS) asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(C::T_REGS));
+    else asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(C::T_REGS));
+    const int tw = warp - C::NPW;  // this warp takes the band rows r = tw + NTW * it
+
+    // everything that changes from row to row is advanced, not recomputed
+    const uint32_t wb_u32 = ptx::smem_u32(wbuf) + (uint32_t)(tw * 2 * WST * 8 + lane * 16);
+    const double* wb = wbuf + (size_t)tw * 2 * WST;
+    const char* wsrc = reinterpret_cast<const char*>(arg.wtab + (size_t)(jA + tw) * WST) + lane * 16;  // weight row of r
+    constexpr size_t WSRC_STEP = (size_t)NTW * WST * sizeof(double);
+    const T* xrow0 = ring + lane * R;
+    T* const O0 = obuf + (size_t)tw * 2 * OB;
+    const uint32_t O0_u32 = ptx::smem_u32(obuf) + (uint32_t)(tw * 2 * OB * sizeof(T));
+    T* orow = arg.fout + (size_t)(jA + tw) * pitch;
+    const size_t orow_step = (size_t)NTW * pitch;
+    const bool wlane = lane < C::W_COPIES;
 
     double csum[R];
 #pragma unroll
@@ -226,7 +240,7 @@ __global__ void __launch_bounds__(384, 1) strang_fused_ws_kernel(const FusedArgs
     bool have = false;
     double* __restrict__ cpw = arg.colpart ? arg.colpart + ((size_t)band * NTW + tw) * (size_t)ntheta : nullptr;
 
-    // one column leaves on the left (its sum is final for this warp), K columns enter on the right
+    // K columns leave on the left (their sums are final for this warp), K columns enter on the right
     auto shift_sums = [&](auto kc) {
         constexpr int K = decltype(kc)::value;
 #pragma unroll
@@ -252,28 +266,27 @@ __global__ void __launch_bounds__(384, 1) strang_fused_ws_kernel(const FusedArgs
         if (cbase >= ntheta) cbase -= ntheta;
     };
 
-    if (tw < nrows) prefetch_w(tw, 0);
+    if (tw < nrows && wlane) ptx::cp_async<16>(wb_u32, wsrc);
     ptx::cp_async_commit();
 
-    int it = 0;
-    for (int r = tw; r < nrows; r += NTW, ++it) {
-        if (r + NTW < nrows) prefetch_w(r + NTW, (it + 1) & 1);
+    int slot = 0, wsel = 0, rin = tw;  // row r is row `rin` of the group in ring slot `slot`
+    unsigned par = 0;
+    for (int r = tw; r < nrows; r += NTW) {
+        wsrc += WSRC_STEP;
+        if (r + NTW < nrows && wlane) ptx::cp_async<16>(wb_u32 + (uint32_t)((wsel ^ 1) * WST * 8), wsrc);
         ptx::cp_async_commit();
         ptx::cp_async_wait<1>();
         __syncwarp();  // the weight row of r is visible to every lane
-        const double* Wr = wb + (it & 1) * WST;
+        const double* Wr = wb + wsel * WST;
 
-        const int grp = r / RG, rin = r - grp * RG;
-        const int slot = grp % NSTG;
-        const int sidx = slot * SPG + rin / SUB;
-        ptx::mbar_wait(&ready[sidx], (unsigned)(grp / NSTG) & 1u);
-
-        const T* grow = ring + ((size_t)slot * RG + rin) * PITCH + lane * R;
+        const uint32_t boff = (uint32_t)((slot * SPG + rin / SUB) * 8);
+        ptx::mbar_wait_u32(ready_u32 + boff, par);
+        const T* grow = xrow0 + (size_t)(slot * RG + rin) * PITCH;
         T x[R + NTAP - 1];
 #pragma unroll
         for (int k = 0; k < R + NTAP - 1; ++k) x[k] = grow[k];
         __syncwarp();
-        if (lane == 0) ptx::mbar_arrive(&empty[sidx]);  // the ring row may be refilled
+        if (lane == 0) ptx::mbar_arrive_u32(empty_u32 + boff);  // the ring row may be refilled
 
         const int S = (int)Wr[NTAP];
         if (!have) {
@@ -306,20 +319,39 @@ __global__ void __launch_bounds__(384, 1) strang_fused_ws_kernel(const FusedArgs
                 if (q < nv) csum[q] += (double)out[q];
         }
 
-        // transpose through the warp's private tile (two tiles alternate: no barrier after the reads), then
-        // coalesced stores: 32 consecutive columns per instruction
-        T* O = obuf + (size_t)(tw * 2 + (it & 1)) * OB;
-#pragma unroll
-        for (int q = 0; q < R; ++q) O[lane * R + q] = out[q];
+        // hand the row to the bulk-copy engine through one of the warp's two private tiles (shared -> global,
+        // 16-byte aligned body; the 0..EPV-1 elements before and after an aligned body are stored by lanes)
+        if (lane == 0) ptx::bulk_wait_read<1>();  // the tile used two rows ago has been read
         __syncwarp();
+        T* O = O0 + wsel * OB;
         const int base = cbase;  // output column of q = 0: wrap(i0 - S)
-        T* __restrict__ orow = arg.fout + (size_t)(jA + r) * pitch;
-        if (base + qmax <= ntheta) {  // the row does not cross the periodic boundary
-            T* __restrict__ dst = orow + base + lane;
+        if (arg.bulk_ok) {
+            const int al = base & (EPV - 1);
 #pragma unroll
-            for (int k = 0; k < R; ++k)
-                if (lane + 32 * k < qmax) dst[32 * k] = O[lane + 32 * k];
+            for (int q = 0; q < R; ++q) O[al + lane * R + q] = out[q];
+            ptx::fence_proxy_async_smem();
+            __syncwarp();
+            const uint32_t O_u32 = O0_u32 + (uint32_t)((wsel * OB + al) * sizeof(T));
+            // q in [qb, qb + len) -> columns [gcol, gcol + len)
+            auto store_piece = [&](int qb, int len, int gcol) {
+                const int h = min(len, (EPV - (gcol & (EPV - 1))) & (EPV - 1));
+                const int nb = (len - h) & ~(EPV - 1);
+                const int t0 = h + nb;
+                if (h | (len - t0)) {  // warp-uniform: some elements outside the aligned body
+                    if (lane < h) orow[gcol + lane] = O[al + qb + lane];
+                    if (lane < len - t0) orow[gcol + t0 + lane] = O[al + qb + t0 + lane];
+                }
+                if (lane == 0 && nb > 0)
+                    ptx::bulk_s2g_u32(orow + gcol + h, O_u32 + (uint32_t)((qb + h) * sizeof(T)), (unsigned)(nb * sizeof(T)));
+            };
+            const int qa = min(qmax, ntheta - base);
+            store_piece(0, qa, base);
+            if (qa < qmax) store_piece(qa, qmax - qa, 0);
+            if (lane == 0) ptx::bulk_commit();
         } else {
+#pragma unroll
+            for (int q = 0; q < R; ++q) O[lane * R + q] = out[q];
+            __syncwarp();
 #pragma unroll
             for (int k = 0; k < R; ++k) {
                 const int q = lane + 32 * k;
@@ -330,16 +362,26 @@ __global__ void __launch_bounds__(384, 1) strang_fused_ws_kernel(const FusedArgs
                 }
             }
         }
-        __syncwarp();  // every lane is done with this row's weights before the next prefetch overwrites them
+        __syncwarp();  // every lane is done with the tile and with this row's weights
+        orow += orow_step;
+        wsel ^= 1;
+        rin += NTW;
+        if (rin >= RG) {
+            rin -= RG;
+            if (++slot == NSTG) {
+                slot = 0;
+                par ^= 1u;
+            }
+        }
     }
     ptx::cp_async_wait<0>();
+    if (lane == 0) ptx::bulk_wait_read<0>();
 
     if (cpw != nullptr && have) {
 #pragma unroll
         for (int q = 0; q < R; ++q) {
             if (q < nv && csum[q] != 0.0) {
                 int cidx = cbase + lane * R + q;
-                if (cidx >= ntheta) cidx -= ntheta;
                 if (cidx >= ntheta) cidx -= ntheta;
                 ptx::red_add_f64(cpw + cidx, csum[q]);
             }

@@ -40,6 +40,25 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, unsigned parity) {
         : "memory");
 }
 
+// the same on 32-bit shared-window addresses (no generic -> shared conversion inside loops); the wait lets the
+// hardware suspend the thread until the phase completes (or the hint, in ns, runs out) instead of spinning
+__device__ __forceinline__ void mbar_arrive_u32(uint32_t bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait_u32(uint32_t bar, unsigned parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred P1;\n"
+        "LAB_WAIT:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1, %2;\n"
+        "@P1 bra DONE;\n"
+        "bra LAB_WAIT;\n"
+        "DONE:\n"
+        "}\n" ::"r"(bar),
+        "r"(parity), "r"(100000u)
+        : "memory");
+}
+
 // global -> shared, 16-byte aligned addresses and size; completion counted in bytes on `bar`
 __device__ __forceinline__ void bulk_g2s(void* dst_smem, const void* src_gmem, unsigned bytes, uint64_t* bar) {
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
@@ -60,6 +79,10 @@ __device__ __forceinline__ void bulk_g2s_hint(void* dst_smem, const void* src_gm
 __device__ __forceinline__ void bulk_s2g(void* dst_gmem, const void* src_smem, unsigned bytes) {
     asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst_gmem), "r"(smem_u32(src_smem)),
                  "r"(bytes)
+                 : "memory");
+}
+__device__ __forceinline__ void bulk_s2g_u32(void* dst_gmem, uint32_t src_smem, unsigned bytes) {
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst_gmem), "r"(src_smem), "r"(bytes)
                  : "memory");
 }
 __device__ __forceinline__ void bulk_s2g_hint(void* dst_gmem, const void* src_smem, unsigned bytes, uint64_t policy) {

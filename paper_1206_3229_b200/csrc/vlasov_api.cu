@@ -30,7 +30,6 @@ constexpr int FU_R = 11;         // consecutive outputs per lane in its theta st
 constexpr int FU_NSTG = 3;       // cp.async ring depth (phases of 12 rows)
 constexpr int FU_NW = FU_NT / 32;  // density partial rows per band of the one-pass kernel, variant 1 (all warps alike)
 constexpr int FW_NSTG = 3;       // ring depth (groups of 12 rows) of the warp-specialised one-pass kernel (variant 0)
-constexpr int FW_NTW = 8;        // its theta warps (8 or 12)
 constexpr int KEY_TUNE_FVARIANT = 108;
 constexpr int FU_PAD = 12;       // rows of padding of the theta weight tables (the last phase of a band reads on)
 constexpr int NCLS = 6;          // profiled kernel classes: theta x1, theta x2, p, rho+force, p+theta x2, p+theta x1
@@ -68,8 +67,9 @@ struct Ctx {
     int fbands[3] = {0, 0, 0}, frpb[3] = {0, 0, 0}, fcols[3] = {0, 0, 0};
     bool onepass = false;
     int tune_fbands = 0;
-    int fvariant = 0;              // 0: warp-specialised one-pass kernel, 1: every warp does both stages
-    int fnw() const { return fvariant == 1 ? FU_NW : vl::FusedWsCfg<double, 2, FU_R, FW_NSTG, FW_NTW>::NTW; }
+    int fvariant = 2;              // 0 / 2: warp-specialised one-pass kernel with 8 / 12 theta warps, 1: every warp does both stages
+    int fnw() const { return fvariant == 1 ? FU_NW : (fvariant == 2 ? 12 : 8); }
+    int fgran(size_t elem) const { return fvariant == 1 ? 1 : (int)(16 / elem); }  // lanes per column-block granule
     std::vector<int> h_srow;
 
     // launch configuration
@@ -244,22 +244,23 @@ int configure_theta_bulk() {
 template <typename T, int NST>
 int configure_fused() {
     using C = vl::FusedCfg<T, NST, FU_NT, FU_R, FU_NSTG>;
-    using CW = vl::FusedWsCfg<T, NST, FU_R, FW_NSTG, FW_NTW>;
     CU(cudaFuncSetAttribute(vl::strang_fused_kernel<T, NST, FU_NT, FU_R, FU_NSTG>,
                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM_BYTES));
-    CU(cudaFuncSetAttribute(vl::strang_fused_ws_kernel<T, NST, FU_R, FW_NSTG, FW_NTW>,
-                            cudaFuncAttributeMaxDynamicSharedMemorySize, (int)CW::SMEM_BYTES));
+    CU(cudaFuncSetAttribute(vl::strang_fused_ws_kernel<T, NST, FU_R, FW_NSTG, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                            (int)vl::FusedWsCfg<T, NST, FU_R, FW_NSTG, 8>::SMEM_BYTES));
+    CU(cudaFuncSetAttribute(vl::strang_fused_ws_kernel<T, NST, FU_R, FW_NSTG, 12>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                            (int)vl::FusedWsCfg<T, NST, FU_R, FW_NSTG, 12>::SMEM_BYTES));
     const int np = G.np, nt = G.ntheta;
     G.fbands[NST] = 0;
     for (int j = 1; j < np; ++j)
         if (G.h_srow[j] > G.h_srow[j - 1]) return VLASOV_OK;  // shift wrapped around the circle: not monotonic
     if ((double)nt * sizeof(T) >= 2147483648.0) return VLASOV_OK;
-    const int units = cdiv(nt, FU_R);
-    const int cols = cdiv(units, 32);
+    const int gran = G.fgran(sizeof(T));
+    const int cols = vl::fused_block_cols(nt, FU_R, gran);
     int wmin = nt;
     for (int c = 0; c < cols; ++c) {
         int i0, wd;
-        vl::fused_block_range(c, cols, nt, FU_R, &i0, &wd);
+        vl::fused_block_range(c, cols, nt, FU_R, gran, &i0, &wd);
         wmin = wd < wmin ? wd : wmin;
     }
     if (wmin < 1) return VLASOV_OK;
@@ -518,6 +519,7 @@ int launch_fused(bool want_colsums) {
     a.force = G.force;
     a.wtab = NST == 2 ? G.wrow2 : G.wrow;
     a.bulk_ok = (G.ntheta % C::EPV == 0) ? 1 : 0;
+    a.gran = G.fgran(sizeof(T));
     a.colpart = want_colsums ? G.colpart_f : nullptr;
     a.ntheta = G.ntheta;
     a.np = G.np;
@@ -529,9 +531,12 @@ int launch_fused(bool want_colsums) {
     prof_begin(NST == 2 ? 4 : 5);
     if (G.fvariant == 1) {
         vl::strang_fused_kernel<T, NST, FU_NT, FU_R, FU_NSTG><<<grid, FU_NT, C::SMEM_BYTES, G.stream>>>(a);
+    } else if (G.fvariant == 2) {
+        using CW = vl::FusedWsCfg<T, NST, FU_R, FW_NSTG, 12>;
+        vl::strang_fused_ws_kernel<T, NST, FU_R, FW_NSTG, 12><<<grid, CW::NT, CW::SMEM_BYTES, G.stream>>>(a);
     } else {
-        using CW = vl::FusedWsCfg<T, NST, FU_R, FW_NSTG, FW_NTW>;
-        vl::strang_fused_ws_kernel<T, NST, FU_R, FW_NSTG, FW_NTW><<<grid, CW::NT, CW::SMEM_BYTES, G.stream>>>(a);
+        using CW = vl::FusedWsCfg<T, NST, FU_R, FW_NSTG, 8>;
+        vl::strang_fused_ws_kernel<T, NST, FU_R, FW_NSTG, 8><<<grid, CW::NT, CW::SMEM_BYTES, G.stream>>>(a);
     }
     prof_end(NST == 2 ? 4 : 5);
     LAUNCH_CHECK();
@@ -693,7 +698,7 @@ int vlasov_set_param(int key, double value) {
             G.fuse = (int)value;
             break;
         case KEY_TUNE_FBANDS: G.tune_fbands = (int)value; break;
-        case KEY_TUNE_FVARIANT: G.fvariant = (value != 0.0) ? 1 : 0; break;
+        case KEY_TUNE_FVARIANT: G.fvariant = (value == 1.0 || value == 2.0) ? (int)value : 0; break;
         case VLASOV_KEY_PROFILE: G.profile = (value != 0.0); break;
         case KEY_TUNE_NW1: G.tune_nw1 = (int)value; break;
         case KEY_TUNE_NW2: G.tune_nw2 = (int)value; break;

@@ -48,7 +48,7 @@ struct FusedArgs {
     const double* wtab;      // [Np + RB][WST] theta weights of the row, then its integer shift as a double:
                              //   NST = 1: w_0..w_9, s;  NST = 2: W_0..W_18, 2 s   (s non-increasing with the row)
     double* colpart;         // [nbands * NW][Ntheta], zero on entry; column sums are ADDED (may be null)
-    int ntheta, np, bc_p, rows_per_band, bulk_ok;
+    int ntheta, np, bc_p, rows_per_band, bulk_ok, gran;
     double dt, dp;
 };
 
@@ -97,14 +97,21 @@ __device__ __forceinline__ void red_add_f64(double* addr, double v) {
 }
 }  // namespace ptx
 
-// first source-side column and width of column block c of `cols`: the ceil(Ntheta / R) lane units of R columns are
-// dealt out evenly, so only the last block can end inside a lane
-__host__ __device__ inline void fused_block_range(int c, int cols, int ntheta, int R, int* i0, int* width) {
-    const long long U = (ntheta + R - 1) / R;
+// Column blocks.  The Ntheta columns are cut into granules of gran * R columns (gran lanes of the theta stage; gran =
+// elements per 16 bytes makes every block start on a 16-byte boundary, gran = 1 is the finest split) and the
+// granules are dealt out evenly: block c of `cols` gets granules [c U / cols, (c + 1) U / cols), at most 32 lanes.
+// Only the last block can end inside a lane.
+__host__ __device__ inline int fused_block_cols(int ntheta, int R, int gran) {
+    const int U = (ntheta + R * gran - 1) / (R * gran);
+    const int per = 32 / gran;
+    return (U + per - 1) / per;
+}
+__host__ __device__ inline void fused_block_range(int c, int cols, int ntheta, int R, int gran, int* i0, int* width) {
+    const long long U = (ntheta + R * gran - 1) / (R * gran);
     const int u0 = (int)((long long)c * U / cols), u1 = (int)((long long)(c + 1) * U / cols);
-    const int e = u1 * R < ntheta ? u1 * R : ntheta;
-    *i0 = u0 * R;
-    *width = e - u0 * R;
+    const int e = u1 * R * gran < ntheta ? u1 * R * gran : ntheta;
+    *i0 = u0 * R * gran;
+    *width = e - u0 * R * gran;
 }
 
 template <typename T, int NST, int NT, int R, int NSTG>
@@ -121,7 +128,7 @@ __global__ void __launch_bounds__(NT, 1) strang_fused_kernel(const FusedArgs<T> 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int ntheta = arg.ntheta, np = arg.np;
     int i0, qmax;
-    fused_block_range((int)blockIdx.x, (int)gridDim.x, ntheta, R, &i0, &qmax);
+    fused_block_range((int)blockIdx.x, (int)gridDim.x, ntheta, R, arg.gran, &i0, &qmax);
     const int band = blockIdx.y;
     const int jA = band * arg.rows_per_band;
     const int jB = min(np, jA + arg.rows_per_band);

@@ -72,7 +72,7 @@ __global__ void __launch_bounds__((4 + NTW_) * 32, 1) strang_fused_ws_kernel(con
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int ntheta = arg.ntheta, np = arg.np;
     int i0, qmax;
-    fused_block_range((int)blockIdx.x, (int)gridDim.x, ntheta, R, &i0, &qmax);
+    fused_block_range((int)blockIdx.x, (int)gridDim.x, ntheta, R, arg.gran, &i0, &qmax);
     const int band = blockIdx.y;
     const int jA = band * arg.rows_per_band;
     const int nrows = min(np, jA + arg.rows_per_band) - jA;
@@ -282,11 +282,11 @@ __global__ void __launch_bounds__((4 + NTW_) * 32, 1) strang_fused_ws_kernel(con
         const uint32_t boff = (uint32_t)((slot * SPG + rin / SUB) * 8);
         ptx::mbar_wait_u32(ready_u32 + boff, par);
         const T* grow = xrow0 + (size_t)(slot * RG + rin) * PITCH;
+        // the window of the row in two halves (fewer values alive at a time): taps 0..NH-1 need x[0 .. R+NH-2]
+        constexpr int NH = (NTAP + 1) / 2;
         T x[R + NTAP - 1];
 #pragma unroll
-        for (int k = 0; k < R + NTAP - 1; ++k) x[k] = grow[k];
-        __syncwarp();
-        if (lane == 0) ptx::mbar_arrive_u32(empty_u32 + boff);  // the ring row may be refilled
+        for (int k = 0; k < R + NH - 1; ++k) x[k] = grow[k];
 
         const int S = (int)Wr[NTAP];
         if (!have) {
@@ -304,7 +304,17 @@ __global__ void __launch_bounds__((4 + NTW_) * 32, 1) strang_fused_ws_kernel(con
             for (int q = 0; q < R; ++q) out[q] = W0 * x[q];
         }
 #pragma unroll
-        for (int n = 1; n < NTAP; ++n) {
+        for (int n = 1; n < NH; ++n) {
+            const T Wn = (T)Wr[n];
+#pragma unroll
+            for (int q = 0; q < R; ++q) out[q] = fma(Wn, x[q + n], out[q]);
+        }
+#pragma unroll
+        for (int k = R + NH - 1; k < R + NTAP - 1; ++k) x[k] = grow[k];
+        __syncwarp();
+        if (lane == 0) ptx::mbar_arrive_u32(empty_u32 + boff);  // the ring row may be refilled
+#pragma unroll
+        for (int n = NH; n < NTAP; ++n) {
             const T Wn = (T)Wr[n];
 #pragma unroll
             for (int q = 0; q < R; ++q) out[q] = fma(Wn, x[q + n], out[q]);

@@ -206,11 +206,9 @@ def run_cuda(args):
             dist.barrier()
         torch.cuda.synchronize()
 
-    # ---- device-resident timing: W warm-up steps, then exactly K steps
+    # ---- device-resident timing: W warm-up steps, then exactly K steps (no per-kernel events in this region)
     if W:
         g.step(W)
-    vb.vlasov_set_param(vb.KEY_PROFILE, 1)
-    vb.vlasov_kernel_times()  # reset
     sampler = ClockSampler(local_rank)
     barrier()
     launches0 = vb.vlasov_launch_count()
@@ -223,6 +221,11 @@ def run_cuda(args):
     clocks = sampler.stop()
     ms_local = e0.elapsed_time(e1)
     launches = vb.vlasov_launch_count() - launches0
+
+    # ---- the same K steps again with a CUDA-event pair around every launch: per-kernel durations for the roofline
+    vb.vlasov_set_param(vb.KEY_PROFILE, 1)
+    vb.vlasov_kernel_times()  # reset
+    g.step(K)
     ktimes = vb.vlasov_kernel_times()
     vb.vlasov_set_param(vb.KEY_PROFILE, 0)
     ms = max_over_ranks(ms_local, world, dev)

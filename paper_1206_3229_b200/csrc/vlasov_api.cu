@@ -64,6 +64,7 @@ struct Ctx {
     int hist_cap = 0, hist_count = 0;
     // one-pass kernel: composite theta weights, band shift ranges, its own density partials
     double *wrow2 = nullptr, *colpart_f = nullptr;
+    unsigned* ticket = nullptr;    // last-CTA counter of rho_force_kernel
     int fbands[3] = {0, 0, 0}, frpb[3] = {0, 0, 0}, fcols[3] = {0, 0, 0};
     bool onepass = false;
     int tune_fbands = 0;
@@ -146,12 +147,13 @@ int cdiv(int a, int b) { return (a + b - 1) / b; }
 
 void free_small() {
     void* ptrs[] = {G.srow, G.wrow, G.cos_t, G.sin_t, G.ringK, G.ringV, G.rho, G.force, G.rho_m,
-                    G.phi,  G.mpart, G.pkpart, G.mom_dev, G.hist, G.wrow2, G.colpart_f};
+                    G.phi,  G.mpart, G.pkpart, G.mom_dev, G.hist, G.wrow2, G.colpart_f, G.ticket};
     for (void* p : ptrs)
         if (p) cudaFree(p);
     G.srow = nullptr;
     G.wrow = G.cos_t = G.sin_t = G.ringK = G.ringV = G.rho = G.force = G.rho_m = G.phi = G.mpart = G.pkpart =
         G.mom_dev = G.hist = G.wrow2 = G.colpart_f = nullptr;
+    G.ticket = nullptr;
     G.hist_cap = G.hist_count = 0;
 }
 
@@ -414,7 +416,9 @@ int prepare() {
     CU(cudaMalloc(&G.phi, sizeof(double) * nt));
     CU(cudaMemset(G.rho, 0, sizeof(double) * nt));
     CU(cudaMemset(G.force, 0, sizeof(double) * nt));
-    CU(cudaMalloc(&G.mpart, sizeof(double) * 2 * cdiv(nt, 256)));
+    CU(cudaMalloc(&G.mpart, sizeof(double) * 2 * cdiv(nt, vl::RR_COLS)));
+    CU(cudaMalloc(&G.ticket, sizeof(unsigned)));
+    CU(cudaMemset(G.ticket, 0, sizeof(unsigned)));
     CU(cudaMalloc(&G.mom_dev, sizeof(double) * 8));
 
     int rc = (G.prec == 32) ? configure_all<float>() : configure_all<double>();
@@ -550,12 +554,15 @@ int fused_pass(int nstage, bool want_colsums) {
     return nstage == 2 ? launch_fused<double, 2>(want_colsums) : launch_fused<double, 1>(want_colsums);
 }
 
-// rho (and for HMF the moment partials) from the column sums left in colpart by `bands` bands
-int rho_from_colpart(int bands, double* rho_out, bool hmf_partials, double* colpart = nullptr, bool zero_after = false) {
+// rho (and for HMF the moment partials) from the column sums left in colpart by `bands` bands; with
+// fuse_force (HMF only) the same kernel also writes the force
+int rho_from_colpart(int bands, double* rho_out, bool hmf_partials, double* colpart = nullptr, bool zero_after = false,
+                     bool fuse_force = false) {
     const double dp = (G.pmax - G.pmin) / (double)G.np;
-    vl::rho_reduce_kernel<<<cdiv(G.ntheta, 256), 256, 0, G.stream>>>(
-        colpart ? colpart : G.colpart, bands, G.ntheta, dp, rho_out, G.cos_t, G.sin_t,
-        hmf_partials ? G.mpart : nullptr, zero_after ? 1 : 0);
+    const double dx = (G.xmax - G.xmin) / (double)G.ntheta;
+    vl::rho_force_kernel<<<cdiv(G.ntheta, vl::RR_COLS), vl::RR_COLS * vl::RR_GROUPS, 0, G.stream>>>(
+        colpart ? colpart : G.colpart, bands, G.ntheta, dp, rho_out, G.cos_t, G.sin_t, hmf_partials ? G.mpart : nullptr,
+        zero_after ? 1 : 0, G.ticket, dx, (fuse_force && hmf_partials) ? G.force : nullptr);
     LAUNCH_CHECK();
     return VLASOV_OK;
 }
@@ -565,7 +572,7 @@ int force_from_rho() {
     const double dx = (G.xmax - G.xmin) / (double)nt;
     switch (G.model) {
         case VLASOV_MODEL_HMF:
-            vl::force_hmf_kernel<<<cdiv(nt, 256), 256, 0, G.stream>>>(G.mpart, cdiv(nt, 256), dx, G.cos_t, G.sin_t,
+            vl::force_hmf_kernel<<<cdiv(nt, 256), 256, 0, G.stream>>>(G.mpart, cdiv(nt, vl::RR_COLS), dx, G.cos_t, G.sin_t,
                                                                       nt, G.force, nullptr);
             break;
         case VLASOV_MODEL_RING:
@@ -580,6 +587,14 @@ int force_from_rho() {
     }
     LAUNCH_CHECK();
     return VLASOV_OK;
+}
+
+// density of the pass that just ran, then the force of the next momentum shift (eqs (10), (2)/(4)/(7)-(8))
+int rho_and_force(int bands, double* colpart, bool zero_after) {
+    const bool hmf = (G.model == VLASOV_MODEL_HMF);
+    int rc = rho_from_colpart(bands, G.rho, hmf, colpart, zero_after, true);
+    if (rc != 0 || hmf) return rc;
+    return force_from_rho();
 }
 
 template <typename T>
@@ -790,10 +805,9 @@ int vlasov_step(int n) {
         if ((rc = theta_pass(1, true)) != 0) return rc;                           // eq (9)
         for (int k = 0; k < n; ++k) {
             prof_begin(3);
-            if (k == 0) rc = rho_from_colpart(theta_bands(1), G.rho, hmf);
-            else rc = rho_from_colpart(G.fbands[2] * G.fnw(), G.rho, hmf, G.colpart_f, true);
+            if (k == 0) rc = rho_and_force(theta_bands(1), nullptr, false);              // eq (10)
+            else rc = rho_and_force(G.fbands[2] * G.fnw(), G.colpart_f, true);
             if (rc != 0) return rc;
-            if ((rc = force_from_rho()) != 0) return rc;                          // eq (10)
             prof_end(3);
             if ((rc = fused_pass(k + 1 < n ? 2 : 1, k + 1 < n)) != 0) return rc;  // eqs (11), (12) [, (9)]
         }
@@ -802,8 +816,7 @@ int vlasov_step(int n) {
         if ((rc = theta_pass(1, true)) != 0) return rc;                       // eq (9)
         for (int k = 0; k < n; ++k) {
             prof_begin(3);
-            if ((rc = rho_from_colpart(theta_bands(k == 0 ? 1 : 2), G.rho, hmf)) != 0) return rc;
-            if ((rc = force_from_rho()) != 0) return rc;                      // eq (10)
+            if ((rc = rho_and_force(theta_bands(k == 0 ? 1 : 2), nullptr, false)) != 0) return rc;  // eq (10)
             prof_end(3);
             if ((rc = p_pass()) != 0) return rc;                              // eq (11)
             if (k + 1 < n) {
@@ -816,8 +829,7 @@ int vlasov_step(int n) {
     } else {
         for (int k = 0; k < n; ++k) {
             if ((rc = theta_pass(1, true)) != 0) return rc;
-            if ((rc = rho_from_colpart(theta_bands(1), G.rho, hmf)) != 0) return rc;
-            if ((rc = force_from_rho()) != 0) return rc;
+            if ((rc = rho_and_force(theta_bands(1), nullptr, false)) != 0) return rc;
             if (G.onepass) {
                 if ((rc = fused_pass(1, false)) != 0) return rc;              // eqs (11), (12) in one pass
             } else {
@@ -843,8 +855,7 @@ int vlasov_substep(int which) {
         case VLASOV_SUB_THETA_TWICE: return theta_pass(2, true);
         case VLASOV_SUB_FORCE:
             if ((rc = moments_pass()) != 0) return rc;
-            if ((rc = rho_from_colpart(G.mbands, G.rho, G.model == VLASOV_MODEL_HMF)) != 0) return rc;
-            return force_from_rho();
+            return rho_and_force(G.mbands, nullptr, false);
         case VLASOV_SUB_P_FULL: return p_pass();
         case VLASOV_SUB_P_THETA_HALF:
         case VLASOV_SUB_P_THETA_TWICE: {
@@ -852,12 +863,10 @@ int vlasov_substep(int which) {
             if (!G.onepass) {  // grid or shift pattern outside the one-pass kernel's conditions: separate passes
                 if ((rc = p_pass()) != 0) return rc;
                 if ((rc = theta_pass(nst, true)) != 0) return rc;
-                if ((rc = rho_from_colpart(theta_bands(nst), G.rho, G.model == VLASOV_MODEL_HMF)) != 0) return rc;
-                return force_from_rho();
+                return rho_and_force(theta_bands(nst), nullptr, false);
             }
             if ((rc = fused_pass(nst, true)) != 0) return rc;
-            if ((rc = rho_from_colpart(G.fbands[nst] * G.fnw(), G.rho, G.model == VLASOV_MODEL_HMF, G.colpart_f, true)) != 0) return rc;
-            return force_from_rho();
+            return rho_and_force(G.fbands[nst] * G.fnw(), G.colpart_f, true);
         }
         default: return fail(VLASOV_EINVAL, "vlasov_substep: unknown stage");
     }

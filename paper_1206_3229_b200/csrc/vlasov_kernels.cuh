@@ -381,6 +381,86 @@ __global__ void __launch_bounds__(256) rho_reduce_kernel(double* __restrict__ co
     }
 }
 
+// The same reduction spread over more CTAs (64 columns x 4 groups of bands per CTA), and for the HMF model fused
+// with the force: the last CTA to finish (ticket counter) adds the per-CTA moment partials in index order --
+// the result does not depend on which CTA is last -- and writes F_i = -M_x sin(theta_i) + M_y cos(theta_i)
+// (eqs (7)-(8), L56-L63) for every column.
+constexpr int RR_COLS = 32, RR_GROUPS = 8, RR_MAXPARTS = 4096;
+__global__ void __launch_bounds__(RR_COLS* RR_GROUPS)
+    rho_force_kernel(double* __restrict__ colpart, int nbands, int ntheta, double dp, double* __restrict__ rho,
+                     const double* __restrict__ cos_t, const double* __restrict__ sin_t,
+                     double* __restrict__ mpart /* [gridDim.x][2] or null */, int zero_after,
+                     unsigned* __restrict__ ticket, double dtheta, double* __restrict__ force /* null: no force */) {
+    __shared__ double part[RR_GROUPS][RR_COLS];
+    __shared__ double2 mp[RR_COLS * RR_GROUPS];
+    __shared__ bool last;
+    const int tid = threadIdx.x, c = tid & (RR_COLS - 1), g = tid / RR_COLS;
+    const int i = blockIdx.x * RR_COLS + c;
+    double a0 = 0.0, a1 = 0.0;
+    if (i < ntheta) {
+        int b = g;
+        for (; b + RR_GROUPS < nbands; b += 2 * RR_GROUPS) {
+            a0 += colpart[(size_t)b * ntheta + i];
+            a1 += colpart[(size_t)(b + RR_GROUPS) * ntheta + i];
+        }
+        if (b < nbands) a0 += colpart[(size_t)b * ntheta + i];
+        if (zero_after)
+            for (b = g; b < nbands; b += RR_GROUPS) colpart[(size_t)b * ntheta + i] = 0.0;
+    }
+    part[g][c] = a0 + a1;
+    __syncthreads();
+    if (g == 0) {  // one warp
+        double acc = 0.0;
+        if (i < ntheta) {
+#pragma unroll
+            for (int q = 0; q < RR_GROUPS; ++q) acc += part[q][c];
+            acc *= dp;
+            rho[i] = acc;
+        }
+        if (mpart != nullptr) {
+            double cs = (i < ntheta) ? cos_t[i] * acc : 0.0;
+            double ss = (i < ntheta) ? sin_t[i] * acc : 0.0;
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) {
+                cs += __shfl_down_sync(0xffffffffu, cs, o);
+                ss += __shfl_down_sync(0xffffffffu, ss, o);
+            }
+            if (tid == 0) {
+                mpart[2 * blockIdx.x + 0] = cs;
+                mpart[2 * blockIdx.x + 1] = ss;
+                bool l = false;
+                if (force != nullptr) {
+                    __threadfence();
+                    l = (atomicAdd(ticket, 1u) == gridDim.x - 1);
+                    if (l) *ticket = 0u;
+                }
+                last = l;
+            }
+        }
+    }
+    if (mpart == nullptr) return;
+    __syncthreads();
+    if (!last) return;
+    // last CTA: M = dtheta * (sum of the partials in index order, the same in every thread), then the force
+    __threadfence();
+    double mx = 0.0, my = 0.0;
+    for (unsigned b0 = 0; b0 < gridDim.x; b0 += RR_COLS * RR_GROUPS) {
+        const unsigned b = b0 + tid;
+        if (b < gridDim.x) mp[tid] = make_double2(__ldcg(mpart + 2 * b), __ldcg(mpart + 2 * b + 1));
+        __syncthreads();
+        const unsigned n = min((unsigned)(RR_COLS * RR_GROUPS), gridDim.x - b0);
+        for (unsigned q = 0; q < n; ++q) {
+            mx += mp[q].x;
+            my += mp[q].y;
+        }
+        __syncthreads();
+    }
+    mx *= dtheta;
+    my *= dtheta;
+#pragma unroll 4
+    for (int k = tid; k < ntheta; k += RR_COLS * RR_GROUPS) force[k] = -sin_t[k] * mx + cos_t[k] * my;
+}
+
 // HMF, eqs (7)-(8) (L56-L63): F_i = -M_x sin(theta_i) + M_y cos(theta_i)
 __global__ void __launch_bounds__(256) force_hmf_kernel(const double* __restrict__ mpart, int nparts, double dtheta,
                                                         const double* __restrict__ cos_t,

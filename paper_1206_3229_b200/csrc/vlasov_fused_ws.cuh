@@ -21,8 +21,12 @@
 
 namespace vl {
 
+#ifndef VL_FW_NOB
+#define VL_FW_NOB 1
+#endif
 template <typename T, int NST, int R, int NSTG, int NTW_ = 8>
 struct FusedWsCfg {
+    static constexpr int NOB = VL_FW_NOB;               // output tiles per theta warp
     static constexpr int NPW = 4, NTW = NTW_;            // p warps (one warpgroup), theta warps (two or three warpgroups)
     static constexpr int NT = (NPW + NTW) * 32;
     static constexpr int NPT = NPW * 32;                // p threads
@@ -39,7 +43,7 @@ struct FusedWsCfg {
     static constexpr int EPV = 16 / (int)sizeof(T);
     static constexpr int OB = (TI + EPV + EPV - 1) / EPV * EPV;
     static constexpr size_t RING_BYTES = (size_t)NSTG * RG * PITCH * sizeof(T);
-    static constexpr size_t O_BYTES = (size_t)NTW * 2 * OB * sizeof(T);
+    static constexpr size_t O_BYTES = (size_t)NTW * NOB * OB * sizeof(T);
     static constexpr size_t W_BYTES = (size_t)NTW * 2 * WST * sizeof(double);
     static constexpr size_t BAR_BYTES = (size_t)2 * NSUB * sizeof(uint64_t);
     static constexpr size_t SMEM_BYTES = RING_BYTES + O_BYTES + W_BYTES + BAR_BYTES;
@@ -226,8 +230,8 @@ __global__ void __launch_bounds__((4 + NTW_) * 32, 1) strang_fused_ws_kernel(con
     const char* wsrc = reinterpret_cast<const char*>(arg.wtab + (size_t)(jA + tw) * WST) + lane * 16;  // weight row of r
     constexpr size_t WSRC_STEP = (size_t)NTW * WST * sizeof(double);
     const T* xrow0 = ring + lane * R;
-    T* const O0 = obuf + (size_t)tw * 2 * OB;
-    const uint32_t O0_u32 = ptx::smem_u32(obuf) + (uint32_t)(tw * 2 * OB * sizeof(T));
+    T* const O0 = obuf + (size_t)tw * C::NOB * OB;
+    const uint32_t O0_u32 = ptx::smem_u32(obuf) + (uint32_t)(tw * C::NOB * OB * sizeof(T));
     T* orow = arg.fout + (size_t)(jA + tw) * pitch;
     const size_t orow_step = (size_t)NTW * pitch;
     const bool wlane = lane < C::W_COPIES;
@@ -331,9 +335,10 @@ __global__ void __launch_bounds__((4 + NTW_) * 32, 1) strang_fused_ws_kernel(con
 
         // hand the row to the bulk-copy engine through one of the warp's two private tiles (shared -> global,
         // 16-byte aligned body; the 0..EPV-1 elements before and after an aligned body are stored by lanes)
-        if (lane == 0) ptx::bulk_wait_read<1>();  // the tile used two rows ago has been read
+        if (lane == 0) ptx::bulk_wait_read<C::NOB - 1>();  // the tile about to be overwritten has been read
         __syncwarp();
-        T* O = O0 + wsel * OB;
+        const int osel = C::NOB == 2 ? wsel : 0;
+        T* O = O0 + osel * OB;
         const int base = cbase;  // output column of q = 0: wrap(i0 - S)
         if (arg.bulk_ok) {
             const int al = base & (EPV - 1);
@@ -341,7 +346,7 @@ __global__ void __launch_bounds__((4 + NTW_) * 32, 1) strang_fused_ws_kernel(con
             for (int q = 0; q < R; ++q) O[al + lane * R + q] = out[q];
             ptx::fence_proxy_async_smem();
             __syncwarp();
-            const uint32_t O_u32 = O0_u32 + (uint32_t)((wsel * OB + al) * sizeof(T));
+            const uint32_t O_u32 = O0_u32 + (uint32_t)((osel * OB + al) * sizeof(T));
             // q in [qb, qb + len) -> columns [gcol, gcol + len)
             auto store_piece = [&](int qb, int len, int gcol) {
                 const int h = min(len, (EPV - (gcol & (EPV - 1))) & (EPV - 1));

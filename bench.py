@@ -11,8 +11,12 @@ theta half shift).  Prints ONE JSON line (rank 0).
              K steps timed as one vlasov_step(K) call with CUDA events
   e2e        same metric through the C ABI with HOST buffers: every step uploads f from pinned host memory,
              runs vlasov_step(1) and downloads f back to pinned host memory
-  roofline   dominant kernel (the fused double theta shift) against the measured HBM peak; algorithmic
-             bytes = 16 B per grid point per launch in fp64 (one read + one write of f)
+  roofline   dominant kernel (the one-pass kernel: p shift + two theta half shifts + density) against the
+             measured HBM peak; algorithmic bytes = 16 B per grid point per launch in fp64 (one read + one
+             write of f); its duration comes from CUDA events around every launch in a second run of the
+             same K steps (the timed region itself carries no per-kernel events); step_frac is the whole
+             step against the bytes this run's passes must move, two_pass_step_frac against the 32 B per
+             point of the two-pass minimum north_star names
   cpu_baseline  the CPU oracle (oracle/, as it stands) timed on this box's host cores on a bounded sample
 
 --impl reference times the oracle (there is no other reference implementation: the paper ships no code).
@@ -250,8 +254,8 @@ def run_cuda(args):
     if dom is not None:
         ach = kern[dom]["achieved_gbs"]
         names = {"theta2": "theta_sweep_bulk_kernel<2 shifts>", "theta1": "theta_sweep_bulk_kernel<1 shift>",
-                 "p": "p_sweep_kernel", "ptheta2": "strang_fused_kernel<p + 2 theta shifts + density>",
-                 "ptheta1": "strang_fused_kernel<p + 1 theta shift>"}
+                 "p": "p_sweep_kernel", "ptheta2": "strang_fused_ws_kernel<p shift + 2 theta half shifts + density>",
+                 "ptheta1": "strang_fused_ws_kernel<p shift + 1 theta half shift>"}
         roofline = {"bound": "hbm", "kernel": names[dom],
                     "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
                     "traffic": committed_traffic(dom, n, prec),

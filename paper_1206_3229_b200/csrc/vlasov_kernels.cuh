@@ -381,11 +381,11 @@ __global__ void __launch_bounds__(256) rho_reduce_kernel(double* __restrict__ co
     }
 }
 
-// The same reduction spread over more CTAs (64 columns x 4 groups of bands per CTA), and for the HMF model fused
-// with the force: the last CTA to finish (ticket counter) adds the per-CTA moment partials in index order --
-// the result does not depend on which CTA is last -- and writes F_i = -M_x sin(theta_i) + M_y cos(theta_i)
+// The same reduction spread over more CTAs (32 columns x 32 groups of bands per CTA), and for the HMF model fused
+// with the force: the last CTA to finish (ticket counter) adds the per-CTA moment partials over a fixed tree --
+// the tree is fixed, so the result does not depend on which CTA is last -- and writes F_i = -M_x sin(theta_i) + M_y cos(theta_i)
 // (eqs (7)-(8), L56-L63) for every column.
-constexpr int RR_COLS = 32, RR_GROUPS = 8, RR_MAXPARTS = 4096;
+constexpr int RR_COLS = 32, RR_GROUPS = 32;
 __global__ void __launch_bounds__(RR_COLS* RR_GROUPS)
     rho_force_kernel(double* __restrict__ colpart, int nbands, int ntheta, double dp, double* __restrict__ rho,
                      const double* __restrict__ cos_t, const double* __restrict__ sin_t,
@@ -398,14 +398,28 @@ __global__ void __launch_bounds__(RR_COLS* RR_GROUPS)
     const int i = blockIdx.x * RR_COLS + c;
     double a0 = 0.0, a1 = 0.0;
     if (i < ntheta) {
-        int b = g;
-        for (; b + RR_GROUPS < nbands; b += 2 * RR_GROUPS) {
-            a0 += colpart[(size_t)b * ntheta + i];
-            a1 += colpart[(size_t)(b + RR_GROUPS) * ntheta + i];
+        // batches of eight independent loads (the kernel is latency-bound); the order of the additions is fixed
+        constexpr int NB = 4;
+        for (int b0 = g; b0 < nbands; b0 += NB * RR_GROUPS) {
+            double v[NB];
+#pragma unroll
+            for (int k = 0; k < NB; ++k) {
+                const int b = b0 + k * RR_GROUPS;
+                v[k] = (b < nbands) ? __ldcg(colpart + (size_t)b * ntheta + i) : 0.0;
+            }
+            if (zero_after) {
+#pragma unroll
+                for (int k = 0; k < NB; ++k) {
+                    const int b = b0 + k * RR_GROUPS;
+                    if (b < nbands) __stcg(colpart + (size_t)b * ntheta + i, 0.0);
+                }
+            }
+#pragma unroll
+            for (int k = 0; k < NB; k += 2) {
+                a0 += v[k];
+                a1 += v[k + 1];
+            }
         }
-        if (b < nbands) a0 += colpart[(size_t)b * ntheta + i];
-        if (zero_after)
-            for (b = g; b < nbands; b += RR_GROUPS) colpart[(size_t)b * ntheta + i] = 0.0;
     }
     part[g][c] = a0 + a1;
     __syncthreads();
@@ -441,23 +455,36 @@ __global__ void __launch_bounds__(RR_COLS* RR_GROUPS)
     if (mpart == nullptr) return;
     __syncthreads();
     if (!last) return;
-    // last CTA: M = dtheta * (sum of the partials in index order, the same in every thread), then the force
+    // last CTA: M = dtheta * (sum of the partials over a fixed tree: thread t adds partials t, t + 1024, ...; then
+    // shuffles inside each warp, then across the warps), the same whichever CTA happens to be last; then the force
     __threadfence();
     double mx = 0.0, my = 0.0;
-    for (unsigned b0 = 0; b0 < gridDim.x; b0 += RR_COLS * RR_GROUPS) {
-        const unsigned b = b0 + tid;
-        if (b < gridDim.x) mp[tid] = make_double2(__ldcg(mpart + 2 * b), __ldcg(mpart + 2 * b + 1));
-        __syncthreads();
-        const unsigned n = min((unsigned)(RR_COLS * RR_GROUPS), gridDim.x - b0);
-        for (unsigned q = 0; q < n; ++q) {
-            mx += mp[q].x;
-            my += mp[q].y;
-        }
-        __syncthreads();
+    for (unsigned b = tid; b < gridDim.x; b += RR_COLS * RR_GROUPS) {
+        mx += __ldcg(mpart + 2 * b);
+        my += __ldcg(mpart + 2 * b + 1);
     }
-    mx *= dtheta;
-    my *= dtheta;
-#pragma unroll 4
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        mx += __shfl_down_sync(0xffffffffu, mx, o);
+        my += __shfl_down_sync(0xffffffffu, my, o);
+    }
+    if ((tid & 31) == 0) mp[tid >> 5] = make_double2(mx, my);
+    __syncthreads();
+    if (tid < 32) {
+        double2 t = mp[tid];  // RR_COLS * RR_GROUPS / 32 == 32 warps
+        mx = t.x;
+        my = t.y;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            mx += __shfl_down_sync(0xffffffffu, mx, o);
+            my += __shfl_down_sync(0xffffffffu, my, o);
+        }
+        if (tid == 0) mp[32] = make_double2(mx * dtheta, my * dtheta);
+    }
+    __syncthreads();
+    mx = mp[32].x;
+    my = mp[32].y;
+#pragma unroll 8
     for (int k = tid; k < ntheta; k += RR_COLS * RR_GROUPS) force[k] = -sin_t[k] * mx + cos_t[k] * my;
 }
 

@@ -335,7 +335,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--fuse", type=int, default=2, choices=[0, 1, 2],
                     help="passes per step: 2 = one (p + theta in one kernel, default), 1 = two, 0 = three")
-    ap.add_argument("--fvariant", type=int, default=2, choices=[0, 1, 2],
+    ap.add_argument("--fvariant", type=int, default=0, choices=[0, 1],
                     help="one-pass kernel: 0 = warp-specialised (default), 1 = every warp does both stages")
     args = ap.parse_args()
     if args.impl == "reference":

@@ -68,8 +68,8 @@ struct Ctx {
     int fbands[3] = {0, 0, 0}, frpb[3] = {0, 0, 0}, fcols[3] = {0, 0, 0};
     bool onepass = false;
     int tune_fbands = 0;
-    int fvariant = 2;              // 0 / 2: warp-specialised one-pass kernel with 8 / 12 theta warps, 1: every warp does both stages
-    int fnw() const { return fvariant == 1 ? FU_NW : (fvariant == 2 ? 12 : 8); }
+    int fvariant = 0;              // 0: warp-specialised one-pass kernel, 1: every warp does both stages
+    int fnw() const { return fvariant == 1 ? FU_NW : 12; }
     int fgran(size_t elem) const { return fvariant == 1 ? 1 : (int)(16 / elem); }  // lanes per column-block granule
     std::vector<int> h_srow;
 
@@ -248,8 +248,6 @@ int configure_fused() {
     using C = vl::FusedCfg<T, NST, FU_NT, FU_R, FU_NSTG>;
     CU(cudaFuncSetAttribute(vl::strang_fused_kernel<T, NST, FU_NT, FU_R, FU_NSTG>,
                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM_BYTES));
-    CU(cudaFuncSetAttribute(vl::strang_fused_ws_kernel<T, NST, FU_R, FW_NSTG, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                            (int)vl::FusedWsCfg<T, NST, FU_R, FW_NSTG, 8>::SMEM_BYTES));
     CU(cudaFuncSetAttribute(vl::strang_fused_ws_kernel<T, NST, FU_R, FW_NSTG, 12>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                             (int)vl::FusedWsCfg<T, NST, FU_R, FW_NSTG, 12>::SMEM_BYTES));
     const int np = G.np, nt = G.ntheta;
@@ -535,12 +533,9 @@ int launch_fused(bool want_colsums) {
     prof_begin(NST == 2 ? 4 : 5);
     if (G.fvariant == 1) {
         vl::strang_fused_kernel<T, NST, FU_NT, FU_R, FU_NSTG><<<grid, FU_NT, C::SMEM_BYTES, G.stream>>>(a);
-    } else if (G.fvariant == 2) {
+    } else {
         using CW = vl::FusedWsCfg<T, NST, FU_R, FW_NSTG, 12>;
         vl::strang_fused_ws_kernel<T, NST, FU_R, FW_NSTG, 12><<<grid, CW::NT, CW::SMEM_BYTES, G.stream>>>(a);
-    } else {
-        using CW = vl::FusedWsCfg<T, NST, FU_R, FW_NSTG, 8>;
-        vl::strang_fused_ws_kernel<T, NST, FU_R, FW_NSTG, 8><<<grid, CW::NT, CW::SMEM_BYTES, G.stream>>>(a);
     }
     prof_end(NST == 2 ? 4 : 5);
     LAUNCH_CHECK();
@@ -713,7 +708,7 @@ int vlasov_set_param(int key, double value) {
             G.fuse = (int)value;
             break;
         case KEY_TUNE_FBANDS: G.tune_fbands = (int)value; break;
-        case KEY_TUNE_FVARIANT: G.fvariant = (value == 1.0 || value == 2.0) ? (int)value : 0; break;
+        case KEY_TUNE_FVARIANT: G.fvariant = (value == 1.0) ? 1 : 0; break;
         case VLASOV_KEY_PROFILE: G.profile = (value != 0.0); break;
         case KEY_TUNE_NW1: G.tune_nw1 = (int)value; break;
         case KEY_TUNE_NW2: G.tune_nw2 = (int)value; break;

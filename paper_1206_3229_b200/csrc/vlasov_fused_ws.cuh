@@ -1,19 +1,28 @@
 // vlasov_fused_ws.cuh -- the one-pass Strang kernel (see vlasov_fused.cuh for the method and the geometry) with
 // WARP SPECIALISATION: the momentum shift and the theta shifts run concurrently on different warps of the CTA.
 //
-//   p warps (4)      thread t owns the three source columns t, t + 128, t + 256 of the CTA.  For each column a
-//                    register window slides down (one new value + ten FMAs per row, eq (11)); new values
-//                    arrive by per-thread cp.async into a ring of NSTG groups of 12 rows; the shifted value
-//                    overwrites the tap in place.  After every 4 rows ("sub-slot") the warp arrives on the
-//                    sub-slot's READY mbarrier.  Before refilling a group it waits for the EMPTY mbarriers of its
-//                    three sub-slots.
-//   theta warps (8)  warp w takes the rows r = w (mod 8) of the band: waits READY of the row's sub-slot, pulls its
-//                    window of the row into registers, arrives on EMPTY (the ring row is free again), applies the
-//                    NTAP composite theta weights (eqs (12), (9)), keeps the column sums (eq (10)) and hands the
-//                    row on through a private shared tile (coalesced stores).  The weights of its next row are prefetched (cp.async) into a
-//                    private two-entry buffer.
-// No block-wide barrier after the set-up: the fp64 pipe sees a p warp and two theta warps per scheduler, each an
-// uninterrupted stream of FMAs, instead of twelve warps that all load, all multiply and all store in step.
+//   p warps (4, one warpgroup, setmaxnreg 152)
+//       thread t owns the three source columns t, t + 128, t + 256 of the CTA.  For each column a register window
+//       slides down (one new value + ten FMAs per row, eq (11)); new values arrive by per-thread cp.async
+//       into a ring of NSTG groups of 12 rows; the shifted value overwrites the tap in place.  After every 4 rows
+//       ("sub-slot") the warp arrives on the sub-slot's READY mbarrier.  Before refilling a group it waits for
+//       the EMPTY mbarriers of its three sub-slots.
+//   theta warps (NTW = 12, three warpgroups, setmaxnreg 120; 8 at 176 registers also builds)
+//       warp w takes the rows r = w (mod NTW) of the band: waits READY of the row's sub-slot, pulls its window of
+//       the row into registers (in two halves: fewer values alive), arrives on EMPTY (the ring row is free again),
+//       applies the NTAP composite theta weights (eqs (12), (9)), keeps the column sums (eq (10)) and hands the row
+//       to the bulk-copy engine through a private tile.  The weights of its next row are prefetched (cp.async)
+//       into a private two-entry buffer.
+// No block-wide barrier after the set-up: the fp64 pipe sees a p warp and three theta warps per scheduler instead
+// of warps that all load, all multiply and all store in step.
+//
+// Tried and measured slower on B200 (8192^2 fp64, us per pass; this version: 258): plain coalesced stores instead
+// of the bulk copy (289); ring depth 2 (285) / 4 and 5 with > 186 KB of shared memory (316, 369: less L1 for the
+// copies in flight); the theta threads issuing the tap copies with a FULL mbarrier (265: the theta warps are the
+// critical path, the p warps have slack); that plus pairs of columns per 16-byte copy (313: the fallback path of a
+// pair with different shifts diverges the warp); column sums in a rotating register ring instead of moving them
+// (280: the dispatch on the rotation costs more than the moves).  Without the theta FMAs the pass takes 203 us,
+// without the p FMAs 255 us: the theta warps' serial work per row is what bounds the kernel.
 #pragma once
 #include <type_traits>
 
@@ -21,12 +30,6 @@
 
 namespace vl {
 
-#ifndef VL_EXP_PTAPS  // timing experiments only (wrong results): fewer FMAs per value
-#define VL_EXP_PTAPS 10
-#endif
-#ifndef VL_EXP_TTAPS
-#define VL_EXP_TTAPS 99
-#endif
 #ifndef VL_FW_NOB
 #define VL_FW_NOB 1
 #endif
@@ -50,20 +53,19 @@ struct FusedWsCfg {
     static constexpr int OB = (TI + EPV + EPV - 1) / EPV * EPV;
     static constexpr size_t RING_BYTES = (size_t)NSTG * RG * PITCH * sizeof(T);
     static constexpr size_t O_BYTES = (size_t)NTW * NOB * OB * sizeof(T);
-    static constexpr int NWB = NSTG + 1;                // weight-row buffers (one more than ring slots, see kernel)
-    static constexpr size_t W_BYTES = (size_t)NWB * RG * WST * sizeof(double);
-    static constexpr size_t BAR_BYTES = (size_t)(2 * NSUB + NSTG) * sizeof(uint64_t);
+    static constexpr size_t W_BYTES = (size_t)NTW * 2 * WST * sizeof(double);
+    static constexpr size_t BAR_BYTES = (size_t)2 * NSUB * sizeof(uint64_t);
     static constexpr size_t SMEM_BYTES = RING_BYTES + O_BYTES + W_BYTES + BAR_BYTES;
-    static constexpr int W_COPIES = RG * WST * 8 / 16;  // 16-byte copies of the weight rows of one group
+    static constexpr int W_COPIES = WST * 8 / 16;
     static_assert(NTA <= PITCH, "source columns must fit the ring row");
     static_assert(R & 1, "lane stride R must be odd (shared-memory banks)");
-    static_assert(NTW == RG && NTW * 32 == PITCH, "theta warp w takes row w of every group; theta thread t loads column t");
+    static_assert(NTW % SUB == 0 && NTW <= RG, "a sub-slot is released by SUB different theta warps");
     // registers per thread after setmaxnreg: 128*152 + 384*120 = 65536; 128*152 + 256*176 = 64512
     static constexpr int P_REGS = 152, T_REGS = NTW == 12 ? 120 : 176;
     static constexpr int LAUNCH_REGS = 65536 / NT / 8 * 8;
     static_assert(NPW * 32 * P_REGS + NTW * 32 * T_REGS <= 65536 && P_REGS % 8 == 0 && T_REGS % 8 == 0, "");
     static_assert(RING_BYTES % 16 == 0 && O_BYTES % 16 == 0 && W_BYTES % 16 == 0, "");
-    static_assert(NSTG >= 2 && W_COPIES <= NPT, "");
+    static_assert(NSTG >= 2 && W_COPIES <= 32, "");
 };
 
 template <typename T, int NST, int R, int NSTG, int NTW_>
@@ -76,10 +78,9 @@ __global__ void __launch_bounds__((4 + NTW_) * 32, 1) strang_fused_ws_kernel(con
     extern __shared__ __align__(128) unsigned char smem_raw[];
     T* ring = reinterpret_cast<T*>(smem_raw);                                                  // [NSTG][RG][PITCH]
     T* obuf = reinterpret_cast<T*>(smem_raw + C::RING_BYTES);                                  // [NTW][2][OB]
-    double* wsm = reinterpret_cast<double*>(smem_raw + C::RING_BYTES + C::O_BYTES);            // [NWB][RG][WST]
+    double* wbuf = reinterpret_cast<double*>(smem_raw + C::RING_BYTES + C::O_BYTES);           // [NTW][2][WST]
     uint64_t* ready = reinterpret_cast<uint64_t*>(smem_raw + C::RING_BYTES + C::O_BYTES + C::W_BYTES);  // [NSUB]
     uint64_t* empty = ready + NSUB;                                                            // [NSUB]
-    uint64_t* full = empty + NSUB;                                                             // [NSTG]
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int ntheta = arg.ntheta, np = arg.np;
@@ -98,27 +99,28 @@ __global__ void __launch_bounds__((4 + NTW_) * 32, 1) strang_fused_ws_kernel(con
             ptx::mbar_init(&ready[k], C::NPW);
             ptx::mbar_init(&empty[k], SUB);
         }
-#pragma unroll
-        for (int k = 0; k < NSTG; ++k) ptx::mbar_init(&full[k], NTW * 32);
         ptx::fence_mbar_init();
     }
     __syncthreads();
-    const uint32_t ready_u32 = ptx::smem_u32(ready), empty_u32 = ptx::smem_u32(empty), full_u32 = ptx::smem_u32(full);
-    const bool p_periodic = (arg.bc_p == BC_PERIODIC);
+    const uint32_t ready_u32 = ptx::smem_u32(ready), empty_u32 = ptx::smem_u32(empty);
 
     if (warp < C::NPW) {
         if (C::P_REGS > C::LAUNCH_REGS) asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(C::P_REGS));
         else asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(C::P_REGS));
         // =========================== p warps: momentum shift (eq (11)) ===========================
+        const bool p_periodic = (arg.bc_p == BC_PERIODIC);
+        bool act[CPT];
+        const T* col[CPT];
+        int rn[CPT];
         T w[CPT][10];
         T v[CPT][12];  // register rings: taps of output row r of a group are v[k][(r + m) % 12]
 #pragma unroll
         for (int k = 0; k < CPT; ++k) {
             const int q = tid + k * NPT;
-            const bool act = q < NTA;
+            act[k] = q < NTA;
             const int c = wrap_index(i0 - 4 * NST + q, ntheta);
             double sf, a;
-            split_shift(-((act ? arg.force[c] : 0.0) * arg.dt) / arg.dp, &sf, &a);
+            split_shift(-((act[k] ? arg.force[c] : 0.0) * arg.dt) / arg.dp, &sf, &a);
             int s;
             if (p_periodic) {
                 sf = fmod(sf, (double)np);
@@ -132,43 +134,62 @@ __global__ void __launch_bounds__((4 + NTW_) * 32, 1) strang_fused_ws_kernel(con
             spline_fd8_weights(a, wd);
 #pragma unroll
             for (int m = 0; m < 10; ++m) w[k][m] = (T)wd[m];
-            // row of tap m of output row j is j + s + m - 4: the first nine taps of the band come straight from
-            // global memory, every later one through the ring (the theta warps issue those copies)
-            const T* col = arg.fin + c;
-            int rn = jA + s - 4;
-            if (p_periodic) rn = wrap_index(rn, np);
+            col[k] = arg.fin + c;
+            // row of tap m of output row j is j + s + m - 4; rn = row of the next value the window has not seen
+            rn[k] = jA + s - 4;
+            if (p_periodic) rn[k] = wrap_index(rn[k], np);
+        }
+#pragma unroll
+        for (int k = 0; k < CPT; ++k) {
 #pragma unroll
             for (int m = 0; m < 9; ++m) {
-                const bool ok = act && (p_periodic || (unsigned)rn < (unsigned)np);
-                v[k][m] = ok ? __ldg(col + (size_t)rn * pitch) : T(0);
-                ++rn;
-                if (p_periodic && rn >= np) rn = 0;
+                const bool ok = act[k] && (p_periodic || (unsigned)rn[k] < (unsigned)np);
+                v[k][m] = ok ? __ldg(col[k] + (size_t)rn[k] * pitch) : T(0);
+                ++rn[k];
+                if (p_periodic && rn[k] >= np) rn[k] = 0;
             }
             v[k][9] = v[k][10] = v[k][11] = T(0);
         }
 
-        // the weight rows of the theta stage travel with the p warps: rows of group g -> buffer g % NWB, copied
-        // after FULL of group g - 1 has been seen.  A theta warp that still reads buffer g % NWB holds up FULL of
-        // group g + NSTG (it has not issued its share of those copies), so the p warps have seen FULL of group
-        // g + NSTG - 1 at most and have written buffer (g + NSTG) % NWB at most: NWB = NSTG + 1 buffers.
-        const uint32_t wsm_u32 = ptx::smem_u32(wsm) + (uint32_t)tid * 16u;
-        const char* wsrc = reinterpret_cast<const char*>(arg.wtab + (size_t)jA * WST) + tid * 16;
-        const bool wthread = tid < C::W_COPIES;
-        if (wthread) ptx::cp_async<16>(wsm_u32, wsrc);
-        ptx::cp_async_commit();
-
-        int slot = 0, wslot = 0;
-        unsigned fpar = 0;
-        for (int g = 0; g < ngroups; ++g) {
-            ptx::mbar_wait_u32(full_u32 + (uint32_t)(slot * 8), fpar);  // the taps of group g have landed
-            {   // only now (see above): the weight rows of group g + 1
-                int nw = wslot + 1;
-                if (nw == C::NWB) nw = 0;
-                wsrc += (size_t)RG * WST * sizeof(double);
-                if (g + 1 < ngroups && wthread) ptx::cp_async<16>(wsm_u32 + (uint32_t)(nw * RG * WST * 8), wsrc);
-                ptx::cp_async_commit();
-                wslot = nw;
+        const uint32_t ring_u32 = ptx::smem_u32(ring) + (uint32_t)tid * (uint32_t)sizeof(T);
+        // new taps of the RG rows of a group -> ring slot `slot`
+        auto issue_group = [&](int slot) {
+            const uint32_t dst0 = ring_u32 + (uint32_t)slot * (uint32_t)(RG * PITCH * sizeof(T));
+#pragma unroll
+            for (int k = 0; k < CPT; ++k) {
+                if (!act[k]) continue;
+                const uint32_t dst = dst0 + (uint32_t)(k * NPT * sizeof(T));
+                if (rn[k] >= 0 && rn[k] + RG <= np) {  // all RG rows exist: no per-row tests
+                    const T* src = col[k] + (long long)rn[k] * (long long)pitch;
+#pragma unroll
+                    for (int r = 0; r < RG; ++r)
+                        ptx::cp_async<(int)sizeof(T)>(dst + (uint32_t)(r * PITCH * sizeof(T)),
+                                                      src + (size_t)((unsigned)r * pitch));
+                    rn[k] += RG;
+                    if (p_periodic && rn[k] >= np) rn[k] = 0;
+                } else {
+#pragma unroll
+                    for (int r = 0; r < RG; ++r) {
+                        const bool ok = p_periodic || (unsigned)rn[k] < (unsigned)np;
+                        const T* src = ok ? col[k] + (size_t)rn[k] * pitch : arg.fin;
+                        ptx::cp_async_zfill<(int)sizeof(T)>(dst + (uint32_t)(r * PITCH * sizeof(T)), src,
+                                                            ok ? (unsigned)sizeof(T) : 0u);
+                        ++rn[k];
+                        if (p_periodic && rn[k] >= np) rn[k] = 0;
+                    }
+                }
             }
+        };
+
+#pragma unroll
+        for (int st = 0; st < NSTG - 1; ++st) {
+            if (st < ngroups) issue_group(st);
+            ptx::cp_async_commit();
+        }
+
+        int slot = 0;
+        for (int g = 0; g < ngroups; ++g) {
+            ptx::cp_async_wait<NSTG - 2>();  // this thread's copies of group g have landed
             T* sl = ring + (size_t)slot * (RG * PITCH) + tid;
 #pragma unroll
             for (int sub = 0; sub < SPG; ++sub) {
@@ -180,18 +201,28 @@ __global__ void __launch_bounds__((4 + NTW_) * 32, 1) strang_fused_ws_kernel(con
                         v[k][(r + 9) % 12] = sl[r * PITCH + k * NPT];
                         T acc = w[k][0] * v[k][r % 12];
 #pragma unroll
-                        for (int m = 1; m < VL_EXP_PTAPS; ++m) acc = fma(w[k][m], v[k][(r + m) % 12], acc);
+                        for (int m = 1; m < 10; ++m) acc = fma(w[k][m], v[k][(r + m) % 12], acc);
                         sl[r * PITCH + k * NPT] = acc;
                     }
                 }
-                if (sub == 0) ptx::cp_async_wait<1>();  // the weight rows of group g have landed too
                 __syncwarp();
                 if (lane == 0) ptx::mbar_arrive_u32(ready_u32 + (uint32_t)((slot * SPG + sub) * 8));
             }
-            if (++slot == NSTG) {
-                slot = 0;
-                fpar ^= 1u;
+            // refill the slot of group g - 1 with group g + NSTG - 1 once the theta warps have let go of it
+            const int gn = g + NSTG - 1;
+            int nslot = slot + NSTG - 1;
+            if (nslot >= NSTG) nslot -= NSTG;
+            if (gn < ngroups) {
+                if (gn >= NSTG) {
+                    const unsigned par = (unsigned)((gn / NSTG) - 1) & 1u;
+#pragma unroll
+                    for (int sub = 0; sub < SPG; ++sub)
+                        ptx::mbar_wait_u32(empty_u32 + (uint32_t)((nslot * SPG + sub) * 8), par);
+                }
+                issue_group(nslot);
             }
+            ptx::cp_async_commit();
+            if (++slot == NSTG) slot = 0;
         }
         ptx::cp_async_wait<0>();
         return;
@@ -202,65 +233,17 @@ __global__ void __launch_bounds__((4 + NTW_) * 32, 1) strang_fused_ws_kernel(con
     else asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(C::T_REGS));
     const int tw = warp - C::NPW;  // this warp takes the band rows r = tw + NTW * it
 
-    // ---- loader duty: thread t of the theta warps brings the taps of source column t into the ring (per-thread
-    // cp.async, completion on the FULL mbarrier of the group).  The p warps spend their instructions on FMAs.
-    const int lt = tw * 32 + lane;
-    const bool lact = lt < NTA;
-    const T* lcol;
-    int lrn;  // row of the next tap of the column that is not in flight yet
-    {
-        const int c = wrap_index(i0 - 4 * NST + lt, ntheta);
-        double sf, a;
-        split_shift(-((lact ? arg.force[c] : 0.0) * arg.dt) / arg.dp, &sf, &a);  // as the p warp owning the column
-        int s;
-        if (p_periodic) {
-            sf = fmod(sf, (double)np);
-            s = (int)sf;
-            if (s < 0) s += np;
-            lrn = wrap_index(jA + s - 4 + 9, np);
-        } else {
-            const double lim = (double)np + 64.0;
-            s = (int)fmin(fmax(sf, -lim), lim);
-            lrn = jA + s - 4 + 9;
-        }
-        lcol = arg.fin + c;
-    }
-    const uint32_t ldst0 = ptx::smem_u32(ring) + (uint32_t)lt * (uint32_t)sizeof(T);
-    auto issue_group = [&](int slot_) {  // the RG rows of the next group -> ring slot, then arrive on its FULL barrier
-        const uint32_t dst = ldst0 + (uint32_t)slot_ * (uint32_t)(RG * PITCH * sizeof(T));
-        if (lact) {
-            if (lrn >= 0 && lrn + RG <= np) {  // all RG rows exist: no per-row tests
-                const T* src = lcol + (long long)lrn * (long long)pitch;
-#pragma unroll
-                for (int r = 0; r < RG; ++r)
-                    ptx::cp_async<(int)sizeof(T)>(dst + (uint32_t)(r * PITCH * sizeof(T)), src + (size_t)((unsigned)r * pitch));
-                lrn += RG;
-                if (p_periodic && lrn >= np) lrn = 0;
-            } else {
-#pragma unroll
-                for (int r = 0; r < RG; ++r) {
-                    const bool ok = p_periodic || (unsigned)lrn < (unsigned)np;
-                    const T* src = ok ? lcol + (size_t)lrn * pitch : arg.fin;
-                    ptx::cp_async_zfill<(int)sizeof(T)>(dst + (uint32_t)(r * PITCH * sizeof(T)), src,
-                                                        ok ? (unsigned)sizeof(T) : 0u);
-                    ++lrn;
-                    if (p_periodic && lrn >= np) lrn = 0;
-                }
-            }
-        }
-        ptx::cp_async_mbar_arrive_noinc(full_u32 + (uint32_t)(slot_ * 8));
-    };
-#pragma unroll
-    for (int st = 0; st < NSTG - 1; ++st)
-        if (st < ngroups) issue_group(st);
-
     // everything that changes from row to row is advanced, not recomputed
-    const T* xrow0 = ring + (size_t)tw * PITCH + lane * R;
+    const uint32_t wb_u32 = ptx::smem_u32(wbuf) + (uint32_t)(tw * 2 * WST * 8 + lane * 16);
+    const double* wb = wbuf + (size_t)tw * 2 * WST;
+    const char* wsrc = reinterpret_cast<const char*>(arg.wtab + (size_t)(jA + tw) * WST) + lane * 16;  // weight row of r
+    constexpr size_t WSRC_STEP = (size_t)NTW * WST * sizeof(double);
+    const T* xrow0 = ring + lane * R;
     T* const O0 = obuf + (size_t)tw * C::NOB * OB;
     const uint32_t O0_u32 = ptx::smem_u32(obuf) + (uint32_t)(tw * C::NOB * OB * sizeof(T));
     T* orow = arg.fout + (size_t)(jA + tw) * pitch;
     const size_t orow_step = (size_t)NTW * pitch;
-    const uint32_t boff0 = (uint32_t)((tw / SUB) * 8);
+    const bool wlane = lane < C::W_COPIES;
 
     double csum[R];
 #pragma unroll
@@ -296,28 +279,22 @@ __global__ void __launch_bounds__((4 + NTW_) * 32, 1) strang_fused_ws_kernel(con
         if (cbase >= ntheta) cbase -= ntheta;
     };
 
-    int slot = 0, wslot = 0, nslot = NSTG - 1;  // ring slot / weight buffer of group g, ring slot of group g + NSTG - 1
-    unsigned par = 0, epar = 1;                 // phase parities: READY of group g; EMPTY of the group refilled next
-    for (int g = 0; g < ngroups; ++g) {
-        // ---- loader: the slot of group g - 1 takes group g + NSTG - 1 once every theta warp has let go of it
-        if (g + NSTG - 1 < ngroups) {
-            if (g >= 1) {
-#pragma unroll
-                for (int sub = 0; sub < SPG; ++sub) ptx::mbar_wait_u32(empty_u32 + (uint32_t)((nslot * SPG + sub) * 8), epar);
-            }
-            issue_group(nslot);
-        }
-        if (++nslot == NSTG) {  // the refills of the next round wait for the next EMPTY phase
-            nslot = 0;
-            epar ^= 1u;
-        }
+    if (tw < nrows && wlane) ptx::cp_async<16>(wb_u32, wsrc);
+    ptx::cp_async_commit();
 
-        const int r = tw + NTW * g;  // this warp's row of the group
-        if (r < nrows) {
-        const double* Wr = wsm + ((size_t)wslot * RG + tw) * WST;
-        const uint32_t boff = boff0 + (uint32_t)(slot * SPG * 8);
+    int slot = 0, wsel = 0, rin = tw;  // row r is row `rin` of the group in ring slot `slot`
+    unsigned par = 0;
+    for (int r = tw; r < nrows; r += NTW) {
+        wsrc += WSRC_STEP;
+        if (r + NTW < nrows && wlane) ptx::cp_async<16>(wb_u32 + (uint32_t)((wsel ^ 1) * WST * 8), wsrc);
+        ptx::cp_async_commit();
+        ptx::cp_async_wait<1>();
+        __syncwarp();  // the weight row of r is visible to every lane
+        const double* Wr = wb + wsel * WST;
+
+        const uint32_t boff = (uint32_t)((slot * SPG + rin / SUB) * 8);
         ptx::mbar_wait_u32(ready_u32 + boff, par);
-        const T* grow = xrow0 + (size_t)slot * (RG * PITCH);
+        const T* grow = xrow0 + (size_t)(slot * RG + rin) * PITCH;
         // the window of the row in two halves (fewer values alive at a time): taps 0..NH-1 need x[0 .. R+NH-2]
         constexpr int NH = (NTAP + 1) / 2;
         T x[R + NTAP - 1];
@@ -340,7 +317,7 @@ __global__ void __launch_bounds__((4 + NTW_) * 32, 1) strang_fused_ws_kernel(con
             for (int q = 0; q < R; ++q) out[q] = W0 * x[q];
         }
 #pragma unroll
-        for (int n = 1; n < (NH < VL_EXP_TTAPS ? NH : VL_EXP_TTAPS); ++n) {
+        for (int n = 1; n < NH; ++n) {
             const T Wn = (T)Wr[n];
 #pragma unroll
             for (int q = 0; q < R; ++q) out[q] = fma(Wn, x[q + n], out[q]);
@@ -350,7 +327,7 @@ __global__ void __launch_bounds__((4 + NTW_) * 32, 1) strang_fused_ws_kernel(con
         __syncwarp();
         if (lane == 0) ptx::mbar_arrive_u32(empty_u32 + boff);  // the ring row may be refilled
 #pragma unroll
-        for (int n = NH; n < (NTAP < VL_EXP_TTAPS ? NTAP : VL_EXP_TTAPS); ++n) {
+        for (int n = NH; n < NTAP; ++n) {
             const T Wn = (T)Wr[n];
 #pragma unroll
             for (int q = 0; q < R; ++q) out[q] = fma(Wn, x[q + n], out[q]);
@@ -369,7 +346,7 @@ __global__ void __launch_bounds__((4 + NTW_) * 32, 1) strang_fused_ws_kernel(con
         // 16-byte aligned body; the 0..EPV-1 elements before and after an aligned body are stored by lanes)
         if (lane == 0) ptx::bulk_wait_read<C::NOB - 1>();  // the tile about to be overwritten has been read
         __syncwarp();
-        const int osel = C::NOB == 2 ? (g & 1) : 0;
+        const int osel = C::NOB == 2 ? wsel : 0;
         T* O = O0 + osel * OB;
         const int base = cbase;  // output column of q = 0: wrap(i0 - S)
         if (arg.bulk_ok) {
@@ -410,12 +387,15 @@ __global__ void __launch_bounds__((4 + NTW_) * 32, 1) strang_fused_ws_kernel(con
             }
         }
         __syncwarp();  // every lane is done with the tile and with this row's weights
-        }  // r < nrows
         orow += orow_step;
-        if (++wslot == C::NWB) wslot = 0;
-        if (++slot == NSTG) {
-            slot = 0;
-            par ^= 1u;
+        wsel ^= 1;
+        rin += NTW;
+        if (rin >= RG) {
+            rin -= RG;
+            if (++slot == NSTG) {
+                slot = 0;
+                par ^= 1u;
+            }
         }
     }
     ptx::cp_async_wait<0>();

@@ -59,12 +59,6 @@ __device__ __forceinline__ void mbar_wait_u32(uint32_t bar, unsigned parity) {
         : "memory");
 }
 
-// one arrival on `bar` once all cp.async copies this thread has issued so far have landed (the barrier's expected
-// count must already include it: .noinc)
-__device__ __forceinline__ void cp_async_mbar_arrive_noinc(uint32_t bar) {
-    asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(bar) : "memory");
-}
-
 // global -> shared, 16-byte aligned addresses and size; completion counted in bytes on `bar`
 __device__ __forceinline__ void bulk_g2s(void* dst_smem, const void* src_gmem, unsigned bytes, uint64_t* bar) {
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(

@@ -57,6 +57,8 @@ extern "C" {
                                   (p shift, both half theta shifts and the density of the next step share a pass;
                                   needs periodic x, otherwise behaves like 1)                                   */
 #define VLASOV_KEY_PROFILE 7   /* 1: bracket every sweep launch of vlasov_step with CUDA events (any time)   */
+/* keys 101..108 (launch-shape overrides: warps, bands, segment lengths, kernel variant) exist for the tests and
+ * the tuning sweeps only; see binding.py KEY_TUNE_*.  Results never depend on them beyond rounding order.   */
 
 /* sub-steps for vlasov_substep (parity tests of single stages; same kernels as vlasov_step) */
 #define VLASOV_SUB_THETA_HALF 0  /* eq (9)/(12): f(x - p dt/2, p), also leaves the column sums for the force */
@@ -64,7 +66,8 @@ extern "C" {
 #define VLASOV_SUB_P_FULL 2      /* eq (11): f(x, p - F dt) with the force vector currently stored           */
 #define VLASOV_SUB_THETA_TWICE 3 /* two half shifts in one pass (the fused a5 o a1 kernel)                   */
 #define VLASOV_SUB_P_THETA_HALF 4  /* one-pass kernel: eq (11) with the stored force, then eq (12); then the density
-                                      and force of the result are left in the RHO / FORCE vectors (FUSE = 2 only) */
+                                      and force of the result are left in the RHO / FORCE vectors (where the
+                                      one-pass kernel does not apply -- vlasov_info says -- the separate kernels) */
 #define VLASOV_SUB_P_THETA_TWICE 5 /* one-pass kernel: eq (11), eq (12), eq (9) of the next step, then density, force */
 
 /* vectors for vlasov_get_vector / vlasov_set_vector (Ntheta doubles each) */
@@ -113,9 +116,12 @@ int vlasov_download(void* f_host);
 
 /*
  * Enqueue n >= 1 Strang steps (asynchronous).  The state afterwards is f(t0 + n dt) as n single steps give
- * it: theta(dt/2), [force, p(dt), theta(dt/2) theta(dt/2)] x (n-1), force, p(dt), theta(dt/2), where the
- * two adjacent half shifts are evaluated one after the other inside one kernel (unless FUSE = 0 or
- * HISTORY = 1).  Errors: EINVAL (n <= 0), ENOTINIT, ECUDA.
+ * it: theta(dt/2), [force, p(dt), theta(dt/2) theta(dt/2)] x (n-1), force, p(dt), theta(dt/2).  With FUSE = 2
+ * (default; periodic x, shift of a half step below one domain length) everything inside the brackets plus the
+ * density of the next force is ONE kernel and the two adjacent half shifts of a row are applied as one 19-tap
+ * filter (the convolution of the ten weights with themselves: the same map up to rounding order); with FUSE = 1
+ * they are evaluated one after the other inside one kernel; FUSE = 0 or HISTORY = 1: separate passes.
+ * Errors: EINVAL (n <= 0), ENOTINIT, ECUDA.
  */
 int vlasov_step(int n);
 

@@ -30,7 +30,7 @@ constexpr int FU_R = 11;         // consecutive outputs per lane in its theta st
 constexpr int FU_NSTG = 3;       // cp.async ring depth (phases of 12 rows)
 constexpr int FU_NW = FU_NT / 32;  // density partial rows per band of the one-pass kernel, variant 1 (all warps alike)
 constexpr int FW_NSTG = 3;       // ring depth (groups of 12 rows) of the warp-specialised one-pass kernel (variant 0)
-constexpr int KEY_TUNE_FVARIANT = 108;
+constexpr int KEY_TUNE_FVARIANT = 108, KEY_TUNE_GRAPH = 109;
 constexpr int FU_PAD = 12;       // rows of padding of the theta weight tables (the last phase of a band reads on)
 constexpr int NCLS = 6;          // profiled kernel classes: theta x1, theta x2, p, rho+force, p+theta x2, p+theta x1
 constexpr int KEY_TUNE_FBANDS = 107;
@@ -65,6 +65,11 @@ struct Ctx {
     // one-pass kernel: composite theta weights, band shift ranges, its own density partials
     double *wrow2 = nullptr, *colpart_f = nullptr;
     unsigned* ticket = nullptr;    // last-CTA counter of rho_force_kernel
+    // CUDA graph of two consecutive steady-state steps of the one-pass path (density/force + pass, twice), one
+    // per parity of the ping-pong; captured on a private stream, launched on the attached one
+    bool graphs = true;
+    cudaGraphExec_t gexec[2] = {nullptr, nullptr};
+    cudaStream_t cap_stream = nullptr;
     int fbands[3] = {0, 0, 0}, frpb[3] = {0, 0, 0}, fcols[3] = {0, 0, 0};
     bool onepass = false;
     int tune_fbands = 0;
@@ -157,7 +162,15 @@ void free_small() {
     G.hist_cap = G.hist_count = 0;
 }
 
+void free_graphs() {
+    for (int k = 0; k < 2; ++k) {
+        if (G.gexec[k]) cudaGraphExecDestroy(G.gexec[k]);
+        G.gexec[k] = nullptr;
+    }
+}
+
 void free_big() {
+    free_graphs();  // they hold the buffer addresses
     if (G.own_f && G.f[0]) cudaFree(G.f[0]);
     if (G.own_work && G.work) cudaFree(G.work);
     G.f[0] = G.f[1] = G.work = nullptr;
@@ -626,6 +639,41 @@ int moments_async(double* dev_out8) {
     return VLASOV_OK;
 }
 
+// two steady-state steps of the one-pass path (each: density/force of the previous pass, then the pass) as one
+// graph launch.  After two passes the ping-pong is back where it started, so one graph per starting parity serves
+// the whole run.  Captured on a private stream (the attached one may be the legacy default stream, which cannot
+// capture) and launched on the attached stream.
+int launch_step_pair_graph() {
+    const int par = G.cur;
+    if (G.gexec[par] == nullptr) {
+        if (G.cap_stream == nullptr) CU(cudaStreamCreateWithFlags(&G.cap_stream, cudaStreamNonBlocking));
+        cudaStream_t user = G.stream;
+        const unsigned long long l0 = G.launches;
+        G.stream = G.cap_stream;
+        int rc = VLASOV_OK;
+        cudaGraph_t graph = nullptr;
+        cudaError_t e = cudaStreamBeginCapture(G.cap_stream, cudaStreamCaptureModeThreadLocal);
+        if (e == cudaSuccess) {
+            for (int q = 0; q < 2 && rc == VLASOV_OK; ++q) {
+                rc = rho_and_force(G.fbands[2] * G.fnw(), G.colpart_f, true);
+                if (rc == VLASOV_OK) rc = fused_pass(2, true);
+            }
+            e = cudaStreamEndCapture(G.cap_stream, &graph);
+        }
+        G.stream = user;
+        G.launches = l0;
+        G.cur = par;
+        if (rc != VLASOV_OK) return rc;
+        CU(e);
+        e = cudaGraphInstantiate(&G.gexec[par], graph, 0);
+        cudaGraphDestroy(graph);
+        CU(e);
+    }
+    CU(cudaGraphLaunch(G.gexec[par], G.stream));
+    G.launches += 4;
+    return VLASOV_OK;
+}
+
 int check_ready() {
     if (!G.ready) return fail(VLASOV_ENOTINIT, "vlasov_init has not been called");
     if (G.cuda_failed) return VLASOV_ECUDA;
@@ -645,6 +693,7 @@ void vlasov_free(void) {
     prof_free();
     free_small();
     free_big();
+    if (G.cap_stream) cudaStreamDestroy(G.cap_stream);
     G = Ctx();
 }
 
@@ -709,6 +758,7 @@ int vlasov_set_param(int key, double value) {
             break;
         case KEY_TUNE_FBANDS: G.tune_fbands = (int)value; break;
         case KEY_TUNE_FVARIANT: G.fvariant = (value == 1.0) ? 1 : 0; break;
+        case KEY_TUNE_GRAPH: G.graphs = (value != 0.0); break;
         case VLASOV_KEY_PROFILE: G.profile = (value != 0.0); break;
         case KEY_TUNE_NW1: G.tune_nw1 = (int)value; break;
         case KEY_TUNE_NW2: G.tune_nw2 = (int)value; break;
@@ -798,13 +848,21 @@ int vlasov_step(int n) {
     if (G.onepass && !G.history) {
         // n + 1 passes: theta(dt/2), then per step ONE pass  p(dt) -> theta(dt/2) [-> theta(dt/2) of the next step]
         if ((rc = theta_pass(1, true)) != 0) return rc;                           // eq (9)
-        for (int k = 0; k < n; ++k) {
+        int k = 0;
+        while (k < n) {
+            // steps 1 .. n-2 are identical pairs of launches: two of them at a time as one CUDA graph
+            if (k >= 1 && k + 2 < n && G.graphs && !G.profile) {
+                if ((rc = launch_step_pair_graph()) != 0) return rc;
+                k += 2;
+                continue;
+            }
             prof_begin(3);
             if (k == 0) rc = rho_and_force(theta_bands(1), nullptr, false);              // eq (10)
             else rc = rho_and_force(G.fbands[2] * G.fnw(), G.colpart_f, true);
             if (rc != 0) return rc;
             prof_end(3);
             if ((rc = fused_pass(k + 1 < n ? 2 : 1, k + 1 < n)) != 0) return rc;  // eqs (11), (12) [, (9)]
+            ++k;
         }
         G.t += (double)n * G.dt;
     } else if (G.fuse >= 1 && !G.history) {

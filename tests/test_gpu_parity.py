@@ -237,6 +237,23 @@ def test_one_pass_is_reproducible_run_to_run():
     assert np.array_equal(outs[0], outs[1]) and np.array_equal(outs[0], outs[2])
 
 
+def test_graph_launches_change_nothing():
+    """Steady-state step pairs launched as CUDA graphs (default) and as plain launches: same kernels, same bits."""
+    c = inputs.config("cfg5", ntheta=900, npts=500)
+    outs, launches = [], []
+    for graph in (1, 0):
+        g = vb.Vlasov(c["model"], c["grid"], c["domain"], c["dt"], tune_graph=graph)
+        g.upload(c["f0"])
+        l0 = vb.vlasov_launch_count()
+        g.step(9)
+        g.step(4)
+        outs.append(g.download())
+        launches.append(vb.vlasov_launch_count() - l0)
+        g.close()
+    assert np.array_equal(outs[0], outs[1])
+    assert launches[0] == launches[1] == (1 + 2 * 9) + (1 + 2 * 4)
+
+
 def test_library_owned_buffers_and_checkpoint_roundtrip():
     c = inputs.config("cfg1", n=96)
     g = vb.Vlasov(c["model"], c["grid"], c["domain"], c["dt"], attach=False)

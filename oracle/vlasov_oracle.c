@@ -375,6 +375,38 @@ int oracle_step(int n) {
 }
 
 /*
+ * Casimir invariants (eq (18)): C[s] = int s(f) dp dx by the rectangle rule on the nodes.
+ *   out[0]  S  = dx dp sum s(f_ij),  s(f) = -f log f  (the entropy of Fig. 2); s(0) = 0 (its limit); the scheme is
+ *           not positivity preserving, and where it has produced f < 0 the entropy density is undefined: those
+ *           nodes contribute 0 here and their weight is reported in out[2] (reading D20)
+ *   out[1]  C2 = dx dp sum f_ij^2     (s(f) = f^2, the "enstrophy")
+ *   out[2]  N- = dx dp sum min(f_ij, 0)  (negative mass; 0 for a non-negative state)
+ *   out[3]  max f_ij
+ * Exact Vlasov dynamics conserves S and C2; on a grid both drift once filaments reach the mesh size (L188).
+ */
+int oracle_casimirs(double out[4]) {
+    if (!G.ready) return ORACLE_ENOTINIT;
+    long nx = G.nx, np = G.np;
+    long double S = 0.0L, C2 = 0.0L, neg = 0.0L;
+    double fmax = G.f[0];
+    for (long j = 0; j < np; ++j) {
+        for (long i = 0; i < nx; ++i) {
+            double v = G.f[(size_t)j * (size_t)nx + (size_t)i];
+            if (v > 0.0) S -= (long double)(v * log(v));
+            if (v < 0.0) neg += (long double)v;
+            C2 += (long double)(v * v);
+            if (v > fmax) fmax = v;
+        }
+    }
+    long double w = (long double)dx_() * (long double)dp_();
+    out[0] = (double)(S * w);
+    out[1] = (double)(C2 * w);
+    out[2] = (double)(neg * w);
+    out[3] = fmax;
+    return ORACLE_OK;
+}
+
+/*
  * out = {t, mass, P, K, U, Mx, My, E}.  Rectangle rule (D6):
  *   mass = dx dp sum f;  P = dx dp sum p_j f;  K = dx dp sum p_j^2/2 f;
  *   Mx, My: eq (8) (L62);  U = (1/2) int rho phi (D10):

@@ -49,6 +49,7 @@ def _load():
             lib.oracle_download.argtypes = [_dp]
             lib.oracle_step.argtypes = [ctypes.c_int]
             lib.oracle_moments.argtypes = [_dp]
+            lib.oracle_casimirs.argtypes = [_dp]
             lib.oracle_density.argtypes = [_dp]
             lib.oracle_force.argtypes = [_dp]
             lib.oracle_theta_sweep.argtypes = [ctypes.c_double]
@@ -165,6 +166,12 @@ class Oracle:
         """{t, mass, P, K, U, Mx, My, E}"""
         out = np.empty(8, dtype=np.float64)
         _check(self.lib.oracle_moments(_ptr(out)), "moments")
+        return out
+
+    def casimirs(self) -> np.ndarray:
+        """{S = -int f log f, C2 = int f^2, negative mass, max f}  (eq (18))"""
+        out = np.empty(4, dtype=np.float64)
+        _check(self.lib.oracle_casimirs(_ptr(out)), "casimirs")
         return out
 
     def close(self):

@@ -563,3 +563,66 @@ def test_density_and_moments_of_a_known_state():
     assert m[5] == pytest.approx(0.5 * PI * sp, rel=1e-13) and abs(m[6]) < 1e-14
     assert m[4] == pytest.approx(0.5 * (m[1] ** 2 - m[5] ** 2), rel=1e-13)
     assert m[7] == m[3] + m[4]
+
+
+# ----------------------------------------------------------------------------- Casimirs (eq (18))
+def test_p19_casimirs_of_a_gaussian_closed_form():
+    """f = exp(-p^2/2T) / (2 pi sqrt(2 pi T)) (mass 1):  S = -int f log f = log(2 pi sqrt(2 pi T)) + 1/2,
+    int f^2 = 1 / (4 pi sqrt(pi T)); the rectangle rule is spectrally accurate for it."""
+    T = 0.4
+    c = inputs.config("cfg2", n=256)
+    th = inputs.nodes(c["domain"][0], c["domain"][1], 256)
+    p = inputs.nodes(c["domain"][2], c["domain"][3], 256)
+    f0 = np.exp(-p[:, None] ** 2 / (2 * T)) / (2 * PI * math.sqrt(2 * PI * T)) * np.ones_like(th)[None, :]
+    o = run(MODEL_HMF, (256, 256), c["domain"], 0.05, f0)
+    S, C2, neg, fmax = o.casimirs()
+    assert S == pytest.approx(math.log(2 * PI * math.sqrt(2 * PI * T)) + 0.5, abs=1e-12)
+    assert C2 == pytest.approx(1.0 / (4 * PI * math.sqrt(PI * T)), rel=1e-12)
+    assert neg == 0.0
+    assert fmax == pytest.approx(1.0 / (2 * PI * math.sqrt(2 * PI * T)), rel=1e-15)
+
+
+def test_p19_casimirs_of_a_waterbag_and_of_signed_values():
+    """Noise-free water-bag of height f0 on n nodes: S = -n f0 log f0 dx dp, int f^2 = n f0^2 dx dp (exact counts);
+    a state with negative values: those nodes add nothing to S and their sum is the negative mass (D20)."""
+    c = inputs.config("cfg4", n=64)  # sheet water-bag, no noise
+    f0 = c["f0"]
+    h = float(f0.max())
+    n = int(np.count_nonzero(f0))
+    assert n > 0 and np.all((f0 == 0) | (f0 == h))
+    dxdp = (c["domain"][1] - c["domain"][0]) / 64 * (c["domain"][3] - c["domain"][2]) / 64
+    o = run(c["model"], c["grid"], c["domain"], c["dt"], f0)
+    S, C2, neg, fmax = o.casimirs()
+    assert S == pytest.approx(-n * h * math.log(h) * dxdp, rel=1e-14)
+    assert C2 == pytest.approx(n * h * h * dxdp, rel=1e-14)
+    assert neg == 0.0 and fmax == h
+    g = f0.copy()
+    g[3, 5] = -0.25
+    g[7, 9] = -0.5
+    o = run(c["model"], c["grid"], c["domain"], c["dt"], g)
+    S2, C22, neg2, _ = o.casimirs()
+    assert S2 == pytest.approx(S, rel=1e-14)                      # f[3,5], f[7,9] were 0 before: no change
+    assert neg2 == pytest.approx(-0.75 * dxdp, rel=1e-14)
+    assert C22 == pytest.approx(C2 + (0.0625 + 0.25) * dxdp, rel=1e-14)
+
+
+def test_p19_casimirs_invariant_under_integer_cell_shifts_and_bounded_drift():
+    """An integer-cell shift permutes the values along each line: every Casimir is unchanged (to the round-off of
+    the sums).  A fractional shift of smooth data changes S and C2 only at the order of the interpolation error;
+    int f^2 cannot grow beyond round-off for a periodic constant shift (|symbol| <= 1, pin P5)."""
+    n_t, n_p = 96, 64
+    dom = (-PI, PI, -3.0, 3.0)
+    th = inputs.nodes(dom[0], dom[1], n_t)
+    p = inputs.nodes(dom[2], dom[3], n_p)
+    f0 = np.exp(-p[:, None] ** 2) * (1.2 + np.cos(th)[None, :])
+    dx = 2 * PI / n_t
+    o = run(MODEL_FREE, (n_t, n_p), dom, 0.0, f0, bc_p=BC_PERIODIC)
+    base = o.casimirs()
+    o.p_sweep(1.0, force=np.full(n_t, -5 * 6.0 / n_p))          # five cells along p, periodic
+    after = o.casimirs()
+    assert np.allclose(after, base, rtol=1e-14, atol=0)
+    o2 = run(MODEL_FREE, (n_t, n_p), dom, 0.0, f0)
+    o2.theta_sweep(0.37 * dx)                                   # displacement p * 0.37 dx: fractional for most rows
+    a2 = o2.casimirs()
+    assert a2[1] <= base[1] * (1 + 1e-14)
+    assert abs(a2[0] - base[0]) < 1e-6 * abs(base[0]) and abs(a2[1] - base[1]) < 1e-6 * base[1]

@@ -141,6 +141,17 @@ int vlasov_set_vector(int which, const double* host_in);
  */
 int vlasov_moments(double out[8]);
 
+/*
+ * Casimir invariants of the current state (eq (18)), rectangle
+ * rule on the nodes; synchronises the stream; out (host, caller-owned):
+ *   out[0]  S  = -int f log f   (the entropy of Fig. 2; nodes with f <= 0 contribute 0)
+ *   out[1]  C2 = int f^2
+ *   out[2]  negative mass  int min(f, 0)  (the scheme is not positivity preserving)
+ *   out[3]  max f
+ * One read pass over f (8 bytes per grid point in fp64), on demand only.  Errors: EINVAL (null), ENOTINIT, ECUDA.
+ */
+int vlasov_casimirs(double out[4]);
+
 /* With HISTORY = 1: copy the records {t, mass, P, K, U, M_x, M_y, E} written after each of the steps of
  * the LAST vlasov_step call into out (host, 8*max_steps doubles); returns the number of records copied
  * (>= 0) or a negative code. */

@@ -26,7 +26,7 @@ OK, EINVAL, ENOTINIT, ECUDA, ENOMEM = 0, -1, -2, -3, -4
 EXPORTS = (
     "vlasov_init", "vlasov_set_param", "vlasov_state_bytes", "vlasov_workspace_bytes", "vlasov_attach",
     "vlasov_state_ptr", "vlasov_upload", "vlasov_download", "vlasov_step", "vlasov_substep",
-    "vlasov_get_vector", "vlasov_set_vector", "vlasov_moments", "vlasov_history", "vlasov_sync",
+    "vlasov_get_vector", "vlasov_set_vector", "vlasov_moments", "vlasov_casimirs", "vlasov_history", "vlasov_sync",
     "vlasov_launch_count", "vlasov_kernel_times", "vlasov_info", "vlasov_free", "vlasov_last_error",
 )
 
@@ -75,6 +75,7 @@ def load(build_if_missing: bool = True):
         "vlasov_get_vector": (ci, [ci, _dp]),
         "vlasov_set_vector": (ci, [ci, _dp]),
         "vlasov_moments": (ci, [_dp]),
+        "vlasov_casimirs": (ci, [_dp]),
         "vlasov_history": (ci, [_dp, ci]),
         "vlasov_sync": (ci, []),
         "vlasov_launch_count": (ci, [ctypes.POINTER(ctypes.c_ulonglong)]),
@@ -168,6 +169,12 @@ def vlasov_set_vector(which: int, v) -> None:
 def vlasov_moments() -> np.ndarray:
     out = np.empty(8, dtype=np.float64)
     _chk(load().vlasov_moments(out.ctypes.data_as(_dp)), "vlasov_moments")
+    return out
+
+
+def vlasov_casimirs() -> np.ndarray:
+    out = np.empty(4, dtype=np.float64)
+    _chk(load().vlasov_casimirs(out.ctypes.data_as(_dp)), "vlasov_casimirs")
     return out
 
 
@@ -278,6 +285,10 @@ class Vlasov:
 
     def sync(self) -> None:
         vlasov_sync()
+
+    def casimirs(self) -> np.ndarray:
+        """{S = -int f log f, C2 = int f^2, negative mass, max f}  (eq (18))"""
+        return vlasov_casimirs()
 
     def info(self) -> dict:
         return vlasov_info()

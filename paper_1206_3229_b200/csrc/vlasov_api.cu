@@ -65,6 +65,7 @@ struct Ctx {
     // one-pass kernel: composite theta weights, band shift ranges, its own density partials
     double *wrow2 = nullptr, *colpart_f = nullptr;
     unsigned* ticket = nullptr;    // last-CTA counter of rho_force_kernel
+    double* caspart = nullptr;     // [mbands * column blocks][4] partials of the Casimir pass, then 4 results
     // CUDA graph of two consecutive steady-state steps of the one-pass path (density/force + pass, twice), one
     // per parity of the ping-pong; captured on a private stream, launched on the attached one
     bool graphs = true;
@@ -152,13 +153,14 @@ int cdiv(int a, int b) { return (a + b - 1) / b; }
 
 void free_small() {
     void* ptrs[] = {G.srow, G.wrow, G.cos_t, G.sin_t, G.ringK, G.ringV, G.rho, G.force, G.rho_m,
-                    G.phi,  G.mpart, G.pkpart, G.mom_dev, G.hist, G.wrow2, G.colpart_f, G.ticket};
+                    G.phi,  G.mpart, G.pkpart, G.mom_dev, G.hist, G.wrow2, G.colpart_f, G.ticket, G.caspart};
     for (void* p : ptrs)
         if (p) cudaFree(p);
     G.srow = nullptr;
     G.wrow = G.cos_t = G.sin_t = G.ringK = G.ringV = G.rho = G.force = G.rho_m = G.phi = G.mpart = G.pkpart =
         G.mom_dev = G.hist = G.wrow2 = G.colpart_f = nullptr;
     G.ticket = nullptr;
+    G.caspart = nullptr;
     G.hist_cap = G.hist_count = 0;
 }
 
@@ -435,6 +437,7 @@ int prepare() {
     int rc = (G.prec == 32) ? configure_all<float>() : configure_all<double>();
     if (rc != 0) return rc;
     CU(cudaMalloc(&G.pkpart, sizeof(double) * 2 * (size_t)G.mbands * cdiv(nt, 256)));
+    CU(cudaMalloc(&G.caspart, sizeof(double) * 4 * ((size_t)G.mbands * cdiv(nt, 256) + 1)));
     if (G.onepass) {
         const size_t nb = (size_t)(G.fbands[2] > G.fbands[1] ? G.fbands[2] : G.fbands[1]) * G.fnw();
         CU(cudaMalloc(&G.colpart_f, sizeof(double) * nb * nt));
@@ -954,6 +957,29 @@ int vlasov_moments(double out[8]) {
     if ((rc = ensure_buffers()) != 0) return rc;
     if ((rc = moments_async(G.mom_dev)) != 0) return rc;
     CU(cudaMemcpyAsync(out, G.mom_dev, sizeof(double) * 8, cudaMemcpyDeviceToHost, G.stream));
+    CU(cudaStreamSynchronize(G.stream));
+    return VLASOV_OK;
+}
+
+int vlasov_casimirs(double out[4]) {
+    int rc = check_ready();
+    if (rc != 0) return rc;
+    if (!out) return fail(VLASOV_EINVAL, "vlasov_casimirs: null");
+    if ((rc = ensure_buffers()) != 0) return rc;
+    const int nblk = G.mbands * cdiv(G.ntheta, 256);
+    const double cell = ((G.xmax - G.xmin) / (double)G.ntheta) * ((G.pmax - G.pmin) / (double)G.np);
+    dim3 grid(cdiv(G.ntheta, 256), G.mbands);
+    if (G.prec == 32)
+        vl::casimir_pass_kernel<float><<<grid, 256, 0, G.stream>>>(static_cast<const float*>(G.f[G.cur]), G.ntheta, G.np,
+                                                                   G.mrpb, G.caspart);
+    else
+        vl::casimir_pass_kernel<double><<<grid, 256, 0, G.stream>>>(static_cast<const double*>(G.f[G.cur]), G.ntheta,
+                                                                    G.np, G.mrpb, G.caspart);
+    LAUNCH_CHECK();
+    double* res = G.caspart + 4 * (size_t)nblk;
+    vl::casimir_final_kernel<<<1, 1024, 0, G.stream>>>(G.caspart, nblk, cell, res);
+    LAUNCH_CHECK();
+    CU(cudaMemcpyAsync(out, res, sizeof(double) * 4, cudaMemcpyDeviceToHost, G.stream));
     CU(cudaStreamSynchronize(G.stream));
     return VLASOV_OK;
 }

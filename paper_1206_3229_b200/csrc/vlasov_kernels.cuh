@@ -712,6 +712,81 @@ __global__ void __launch_bounds__(1024) moments_final_kernel(const double* __res
     }
 }
 
+// ------------------------------------------------------------------------------------------------
+// Casimir invariants, eq (18): C[s] = int s(f) dp dx by the rectangle rule.
+//   s(f) = -f log f (entropy of Fig. 2; nodes with f <= 0 contribute 0, D20),  s(f) = f^2,
+//   negative mass sum min(f, 0), max f.  One read pass over f; block partials, then one CTA adds them over a fixed
+//   tree (deterministic).
+// ------------------------------------------------------------------------------------------------
+template <int NT>
+__device__ __forceinline__ double block_max(double v, double* red /* NT/32 doubles */) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_down_sync(0xffffffffu, v, o));
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    __syncthreads();
+    if (lane == 0) red[warp] = v;
+    __syncthreads();
+    double t = v;
+    if (warp == 0) {
+        t = (lane < NT / 32) ? red[lane] : red[0];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) t = fmax(t, __shfl_down_sync(0xffffffffu, t, o));
+    }
+    return t;  // valid in thread 0
+}
+
+template <typename T>
+__global__ void __launch_bounds__(256) casimir_pass_kernel(const T* __restrict__ f, int ntheta, int np,
+                                                           int rows_per_band,
+                                                           double* __restrict__ part /* [blocks][4] */) {
+    __shared__ double red[8];
+    const int i = blockIdx.x * 256 + threadIdx.x;
+    const int j0 = blockIdx.y * rows_per_band, j1 = min(np, j0 + rows_per_band);
+    double s = 0.0, c2 = 0.0, neg = 0.0, mx = (double)f[0];
+    if (i < ntheta) {
+        for (int j = j0; j < j1; ++j) {
+            const double v = (double)f[(size_t)j * ntheta + i];
+            if (v > 0.0) s -= v * log(v);
+            if (v < 0.0) neg += v;
+            c2 = fma(v, v, c2);
+            mx = fmax(mx, v);
+        }
+    }
+    const double S = block_sum<256>(s, red);
+    const double C = block_sum<256>(c2, red);
+    const double N = block_sum<256>(neg, red);
+    const double M = block_max<256>(mx, red);
+    if (threadIdx.x == 0) {
+        const int b = blockIdx.y * gridDim.x + blockIdx.x;
+        part[4 * b + 0] = S;
+        part[4 * b + 1] = C;
+        part[4 * b + 2] = N;
+        part[4 * b + 3] = M;
+    }
+}
+
+__global__ void __launch_bounds__(1024) casimir_final_kernel(const double* __restrict__ part, int nparts, double cell,
+                                                             double* __restrict__ out) {
+    __shared__ double red[32];
+    double s = 0.0, c2 = 0.0, neg = 0.0, mx = part[3];
+    for (int b = threadIdx.x; b < nparts; b += 1024) {
+        s += part[4 * b + 0];
+        c2 += part[4 * b + 1];
+        neg += part[4 * b + 2];
+        mx = fmax(mx, part[4 * b + 3]);
+    }
+    const double S = block_sum<1024>(s, red);
+    const double C = block_sum<1024>(c2, red);
+    const double N = block_sum<1024>(neg, red);
+    const double M = block_max<1024>(mx, red);
+    if (threadIdx.x == 0) {
+        out[0] = S * cell;
+        out[1] = C * cell;
+        out[2] = N * cell;
+        out[3] = M;
+    }
+}
+
 __global__ void fill_zero_kernel(double* __restrict__ p, int n) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i < n) p[i] = 0.0;

@@ -237,6 +237,38 @@ def test_one_pass_is_reproducible_run_to_run():
     assert np.array_equal(outs[0], outs[1]) and np.array_equal(outs[0], outs[2])
 
 
+@pytest.mark.parametrize("name,kw,steps", [("cfg1", dict(), 40), ("cfg2", dict(n=256), 0), ("cfg3", dict(ntheta=320, npts=256), 25),
+                                           ("cfg4", dict(ntheta=512, npts=300), 25), ("cfg5", dict(ntheta=1500, npts=700), 10)])
+def test_casimirs_match_oracle(name, kw, steps):
+    """Entropy, int f^2, negative mass and max f of eq (18) (L183-L188) of the evolved state: CUDA reduction against
+    the oracle's long-double sums (1e-12 relative: one ulp of log per node, different summation order)."""
+    c = inputs.config(name, **kw)
+    o, g = pair(c["model"], c["grid"], c["domain"], c["dt"], c["f0"], **c["params"])
+    if steps:
+        o.step(steps)
+        g.step(steps)
+    co, cg = o.casimirs(), g.casimirs()
+    scale = np.array([abs(co[0]), co[1], max(abs(co[2]), 1e-3 * co[1]), abs(co[3])])
+    assert np.all(np.abs(cg - co) <= 1e-10 * np.maximum(scale, 1e-300)), (co, cg)
+    if steps:
+        assert co[2] < 0.0 or name == "cfg2"  # the water-bags undershoot at their edges: negative mass is real
+    g.close()
+
+
+def test_casimirs_fp32_state():
+    c = inputs.config("cfg5", ntheta=640, npts=320)
+    g = vb.Vlasov(c["model"], c["grid"], c["domain"], c["dt"], precision=32)
+    f32 = c["f0"].astype(np.float32)
+    g.upload(f32)
+    cg = g.casimirs()
+    g.close()
+    o = Oracle(c["model"], c["grid"], c["domain"], c["dt"], threads=8)
+    o.upload(f32.astype(np.float64))
+    co = o.casimirs()
+    o.close()
+    assert np.allclose(cg, co, rtol=1e-12, atol=0)
+
+
 def test_graph_launches_change_nothing():
     """Steady-state step pairs launched as CUDA graphs (default) and as plain launches: same kernels, same bits."""
     c = inputs.config("cfg5", ntheta=900, npts=500)

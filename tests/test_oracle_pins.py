@@ -626,3 +626,37 @@ def test_p19_casimirs_invariant_under_integer_cell_shifts_and_bounded_drift():
     a2 = o2.casimirs()
     assert a2[1] <= base[1] * (1 + 1e-14)
     assert abs(a2[0] - base[0]) < 1e-6 * abs(base[0]) and abs(a2[1] - base[1]) < 1e-6 * base[1]
+
+
+# ----------------------------------------------------------------------------- the paper's own sheet runs (Table 2)
+def paper_sheet_state(n):
+    """Set-up of PAPER.md L145-L150: x, p in [-2, 2], water-bag of eq (17) with x0 = 1, p0 = 0.5, edges included."""
+    dom = (-2.0, 2.0, -2.0, 2.0)
+    x = inputs.nodes(dom[0], dom[1], n)
+    p = inputs.nodes(dom[2], dom[3], n)
+    f0 = np.where((np.abs(x)[None, :] <= 1.0) & (np.abs(p)[:, None] <= 0.5), 0.5, 0.0)
+    return dom, f0
+
+
+def test_p20_energy_error_of_the_papers_sheet_run_matches_table_2(golden_dir):
+    """Table 2 (L158-L165) prints delta e = 5e-4 for n = 256 at dt = 0.1 with the FD interpolation.  The oracle, run
+    with the paper's own boundary conditions (periodic in x and p, L113) to t = 100, shows 4.9e-4: same value to
+    the one digit the paper prints (the run length is not stated, D13: asserted within a factor 2).  Its norm is
+    conserved to round-off where the paper reports 4e-5 (D14: the telescoping sum is exact)."""
+    rows = [ln.split() for ln in open(os.path.join(golden_dir, "sheet_table2_L158.txt")) if not ln.startswith("#")]
+    table = {int(r[0]): (float(r[1]), float(r[2])) for r in rows}
+    n = 256
+    dom, f0 = paper_sheet_state(n)
+    o = run(MODEL_SHEET, (n, n), dom, 0.1, f0, threads=os.cpu_count() or 4, bc_x=BC_PERIODIC, bc_p=BC_PERIODIC)
+    m0 = o.moments()
+    s0 = o.casimirs()[0]
+    de = dn = 0.0
+    for _ in range(100):
+        o.step(10)
+        m = o.moments()
+        de = max(de, abs(m[7] - m0[7]) / abs(m0[7]))
+        dn = max(dn, abs(m[1] - m0[1]) / m0[1])
+    assert 0.5 * table[n][0] <= de <= 2.0 * table[n][0]
+    assert dn <= 1e-12 <= table[n][1]
+    # Fig. 2 (L180): the entropy rises from its initial plateau once filaments reach the mesh size
+    assert o.casimirs()[0] > s0 + 0.2

@@ -199,7 +199,8 @@ def run_cuda(args):
     c = inputs.config("cfg5", n=n)
     f0 = c["f0"].astype(np.float64 if prec == 64 else np.float32)
     g = vb.Vlasov(c["model"], c["grid"], c["domain"], c["dt"], precision=prec, device="cuda:%d" % local_rank,
-                  fuse=args.fuse, tune_fvariant=args.fvariant, tune_graph=args.graph)
+                  fuse=args.fuse, tune_fvariant=args.fvariant, tune_graph=args.graph,
+                  **({"tune_fbands": args.fbands} if args.fbands > 0 else {}))
     g.upload(f0)
     pts = float(n) * float(n)
 
@@ -335,6 +336,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--fuse", type=int, default=2, choices=[0, 1, 2],
                     help="passes per step: 2 = one (p + theta in one kernel, default), 1 = two, 0 = three")
+    ap.add_argument("--fbands", type=int, default=0, help="bands of rows of the one-pass kernel (0 = automatic)")
     ap.add_argument("--graph", type=int, default=1, choices=[0, 1],
                     help="1 (default): steady-state step pairs are launched as CUDA graphs, 0: plain launches")
     ap.add_argument("--fvariant", type=int, default=0, choices=[0, 1],

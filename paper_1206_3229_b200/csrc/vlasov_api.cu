@@ -279,7 +279,11 @@ int configure_fused() {
         wmin = wd < wmin ? wd : wmin;
     }
     if (wmin < 1) return VLASOV_OK;
-    int bands = G.tune_fbands > 0 ? G.tune_fbands : G.sm_count / cols;
+    // one CTA per SM; but no bands shorter than 32 rows: every band adds 12 rows of density partials for
+    // rho_force_kernel to read and a nine-row halo (sweep on 256^2 .. 2048^2 in profiles/README.md)
+    int bands = G.sm_count / cols;
+    if (bands > np / 32) bands = np / 32;
+    if (G.tune_fbands > 0) bands = G.tune_fbands;
     if (bands < 1) bands = 1;
     if (bands > np) bands = np;
     int rpb = cdiv(np, bands);

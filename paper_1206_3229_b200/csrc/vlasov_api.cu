@@ -65,6 +65,8 @@ struct Ctx {
     // one-pass kernel: composite theta weights, band shift ranges, its own density partials
     double *wrow2 = nullptr, *colpart_f = nullptr;
     unsigned* ticket = nullptr;    // last-CTA counter of rho_force_kernel
+    double* ringpart = nullptr;    // [Ntheta / RING_L][Ntheta] chunk partials of the ring convolution
+    unsigned* ringtick = nullptr;  // [Ntheta / 256] last-CTA counters of its tiles
     double* caspart = nullptr;     // [mbands * column blocks][4] partials of the Casimir pass, then 4 results
     // CUDA graph of two consecutive steady-state steps of the one-pass path (density/force + pass, twice), one
     // per parity of the ping-pong; captured on a private stream, launched on the attached one
@@ -153,7 +155,7 @@ int cdiv(int a, int b) { return (a + b - 1) / b; }
 
 void free_small() {
     void* ptrs[] = {G.srow, G.wrow, G.cos_t, G.sin_t, G.ringK, G.ringV, G.rho, G.force, G.rho_m,
-                    G.phi,  G.mpart, G.pkpart, G.mom_dev, G.hist, G.wrow2, G.colpart_f, G.ticket, G.caspart};
+                    G.phi,  G.mpart, G.pkpart, G.mom_dev, G.hist, G.wrow2, G.colpart_f, G.ticket, G.caspart, G.ringpart, G.ringtick};
     for (void* p : ptrs)
         if (p) cudaFree(p);
     G.srow = nullptr;
@@ -161,6 +163,8 @@ void free_small() {
         G.mom_dev = G.hist = G.wrow2 = G.colpart_f = nullptr;
     G.ticket = nullptr;
     G.caspart = nullptr;
+    G.ringpart = nullptr;
+    G.ringtick = nullptr;
     G.hist_cap = G.hist_count = 0;
 }
 
@@ -426,6 +430,9 @@ int prepare() {
         CU(cudaMalloc(&G.ringV, sizeof(double) * nt));
         CU(cudaMemcpy(G.ringK, K.data(), sizeof(double) * nt, cudaMemcpyHostToDevice));
         CU(cudaMemcpy(G.ringV, V.data(), sizeof(double) * nt, cudaMemcpyHostToDevice));
+        CU(cudaMalloc(&G.ringpart, sizeof(double) * (size_t)cdiv(nt, vl::RING_L) * nt));
+        CU(cudaMalloc(&G.ringtick, sizeof(unsigned) * cdiv(nt, 256)));
+        CU(cudaMemset(G.ringtick, 0, sizeof(unsigned) * cdiv(nt, 256)));
     }
     CU(cudaMalloc(&G.rho, sizeof(double) * nt));
     CU(cudaMalloc(&G.force, sizeof(double) * nt));
@@ -582,16 +589,14 @@ int rho_from_colpart(int bands, double* rho_out, bool hmf_partials, double* colp
     return VLASOV_OK;
 }
 
+// force of the ring, sheet and free models from rho (the HMF force comes out of rho_force_kernel itself)
 int force_from_rho() {
     const int nt = G.ntheta;
     const double dx = (G.xmax - G.xmin) / (double)nt;
     switch (G.model) {
-        case VLASOV_MODEL_HMF:
-            vl::force_hmf_kernel<<<cdiv(nt, 256), 256, 0, G.stream>>>(G.mpart, cdiv(nt, vl::RR_COLS), dx, G.cos_t, G.sin_t,
-                                                                      nt, G.force, nullptr);
-            break;
         case VLASOV_MODEL_RING:
-            vl::ring_convolve_kernel<<<cdiv(nt, 256), 256, 0, G.stream>>>(G.ringK, G.rho, nt, dx, G.force);
+            vl::ring_convolve_kernel<<<dim3(cdiv(nt, 256), cdiv(nt, vl::RING_L)), 256, 0, G.stream>>>(
+                G.ringK, G.rho, nt, dx, G.ringpart, G.ringtick, G.force);
             break;
         case VLASOV_MODEL_SHEET:
             vl::sheet_scan_kernel<<<1, 1024, 0, G.stream>>>(G.rho, nt, dx, 0, G.force);
@@ -632,7 +637,8 @@ int moments_async(double* dev_out8) {
     if ((rc = rho_from_colpart(G.mbands, G.rho_m, false)) != 0) return rc;
     const double* phi = nullptr;
     if (G.model == VLASOV_MODEL_RING) {
-        vl::ring_convolve_kernel<<<cdiv(nt, 256), 256, 0, G.stream>>>(G.ringV, G.rho_m, nt, dx, G.phi);
+        vl::ring_convolve_kernel<<<dim3(cdiv(nt, 256), cdiv(nt, vl::RING_L)), 256, 0, G.stream>>>(
+            G.ringV, G.rho_m, nt, dx, G.ringpart, G.ringtick, G.phi);
         LAUNCH_CHECK();
         phi = G.phi;
     } else if (G.model == VLASOV_MODEL_SHEET) {

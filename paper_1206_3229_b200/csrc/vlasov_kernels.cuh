@@ -343,45 +343,9 @@ __device__ __forceinline__ double block_sum(double v, double* red /* NT/32 doubl
     return t;  // valid in thread 0
 }
 
-// rho_i = dp * sum_b colpart[b][i];  for HMF also per-block partial sums of cos(theta_i) rho_i, sin(theta_i) rho_i
-// zero_after: the partials are accumulated by atomic adds (one-pass kernel) and must be zero for the next pass
-__global__ void __launch_bounds__(256) rho_reduce_kernel(double* __restrict__ colpart, int nbands, int ntheta,
-                                                         double dp, double* __restrict__ rho,
-                                                         const double* __restrict__ cos_t,
-                                                         const double* __restrict__ sin_t,
-                                                         double* __restrict__ mpart /* [gridDim.x][2] */,
-                                                         int zero_after) {
-    __shared__ double red[8];
-    const int i = blockIdx.x * 256 + threadIdx.x;
-    double acc = 0.0;
-    if (i < ntheta) {
-        double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
-        int b = 0;
-        for (; b + 4 <= nbands; b += 4) {
-            a0 += colpart[(size_t)(b + 0) * ntheta + i];
-            a1 += colpart[(size_t)(b + 1) * ntheta + i];
-            a2 += colpart[(size_t)(b + 2) * ntheta + i];
-            a3 += colpart[(size_t)(b + 3) * ntheta + i];
-        }
-        for (; b < nbands; ++b) a0 += colpart[(size_t)b * ntheta + i];
-        if (zero_after)
-            for (b = 0; b < nbands; ++b) colpart[(size_t)b * ntheta + i] = 0.0;
-        acc = ((a0 + a1) + (a2 + a3)) * dp;
-        rho[i] = acc;
-    }
-    if (mpart != nullptr) {
-        const double c = (i < ntheta) ? cos_t[i] * acc : 0.0;
-        const double s = (i < ntheta) ? sin_t[i] * acc : 0.0;
-        const double cs = block_sum<256>(c, red);
-        const double ss = block_sum<256>(s, red);
-        if (threadIdx.x == 0) {
-            mpart[2 * blockIdx.x + 0] = cs;
-            mpart[2 * blockIdx.x + 1] = ss;
-        }
-    }
-}
-
-// The same reduction spread over more CTAs (32 columns x 32 groups of bands per CTA), and for the HMF model fused
+// rho_i = dp * sum_b colpart[b][i]; for HMF also per-CTA partial sums of cos(theta_i) rho_i, sin(theta_i) rho_i.
+// zero_after: the partials of the one-pass kernel are accumulated by atomic adds and must be zero for the next pass.
+// 32 columns x 32 groups of bands per CTA, and for the HMF model fused
 // with the force: the last CTA to finish (ticket counter) adds the per-CTA moment partials over a fixed tree --
 // the tree is fixed, so the result does not depend on which CTA is last -- and writes F_i = -M_x sin(theta_i) + M_y cos(theta_i)
 // (eqs (7)-(8), L56-L63) for every column.
@@ -488,56 +452,55 @@ __global__ void __launch_bounds__(RR_COLS* RR_GROUPS)
     for (int k = tid; k < ntheta; k += RR_COLS * RR_GROUPS) force[k] = -sin_t[k] * mx + cos_t[k] * my;
 }
 
-// HMF, eqs (7)-(8) (L56-L63): F_i = -M_x sin(theta_i) + M_y cos(theta_i)
-__global__ void __launch_bounds__(256) force_hmf_kernel(const double* __restrict__ mpart, int nparts, double dtheta,
-                                                        const double* __restrict__ cos_t,
-                                                        const double* __restrict__ sin_t, int ntheta,
-                                                        double* __restrict__ force, double* __restrict__ mxy) {
-    double mx = 0.0, my = 0.0;
-    for (int b = 0; b < nparts; ++b) {  // same order in every thread: deterministic, identical M everywhere
-        mx += mpart[2 * b + 0];
-        my += mpart[2 * b + 1];
-    }
-    mx *= dtheta;
-    my *= dtheta;
-    const int i = blockIdx.x * 256 + threadIdx.x;
-    if (i < ntheta) force[i] = -sin_t[i] * mx + cos_t[i] * my;
-    if (mxy != nullptr && blockIdx.x == 0 && threadIdx.x == 0) {
-        mxy[0] = mx;
-        mxy[1] = my;
-    }
-}
-
 // ring, eq (2) (L33-L35), reading D9: out_i = scale * sum_{m=0}^{N-1} tab[m] rho[(i - m) mod N].
-// Used with tab = K (force) and tab = V (potential, for the energy).  The table tile and the matching
-// window of rho are staged in shared memory; every thread owns one i.
-constexpr int RING_TM = 1024;
+// Used with tab = K (force) and tab = V (potential, for the energy).  The sum over m is cut into chunks of RING_L
+// terms: CTA (tile of 256 outputs, chunk c) stages its piece of the table and the matching window of rho in shared
+// memory and writes 256 partial sums; the last CTA of a tile to finish (ticket counter per tile) adds the chunks
+// in chunk order -- the result does not depend on which CTA that is.  N = 2048: 8 x 16 CTAs of 128 FMAs per thread
+// instead of 8 CTAs of 2048.
+constexpr int RING_L = 128;
 __global__ void __launch_bounds__(256) ring_convolve_kernel(const double* __restrict__ tab,
                                                             const double* __restrict__ rho, int n, double scale,
+                                                            double* __restrict__ part /* [chunks][n] */,
+                                                            unsigned* __restrict__ tickets /* [tiles], zero */,
                                                             double* __restrict__ out) {
-    __shared__ double sK[RING_TM];
-    __shared__ double sR[RING_TM + 256];
-    const int ib = blockIdx.x * 256;
-    const int i = ib + threadIdx.x;
-    double acc0 = 0.0, acc1 = 0.0;
-    for (int m0 = 0; m0 < n; m0 += RING_TM) {
-        const int tm = min(RING_TM, n - m0);
-        __syncthreads();
-        for (int q = threadIdx.x; q < tm; q += 256) sK[q] = tab[m0 + q];
-        // sR[q] = rho[(ib - m0 - (tm-1) + q) mod n], q in [0, tm + 255)
-        const int lo = wrap_index(ib - m0 - (tm - 1), n);
-        for (int q = threadIdx.x; q < tm + 255; q += 256) sR[q] = rho[(lo + q) % n];
-        __syncthreads();
-        // rho index i - m  ->  sR[(i - ib) + (tm-1) - (m - m0)]
-        const int off = threadIdx.x + tm - 1;
-        int mm = 0;
-        for (; mm + 2 <= tm; mm += 2) {
-            acc0 = fma(sK[mm], sR[off - mm], acc0);
-            acc1 = fma(sK[mm + 1], sR[off - mm - 1], acc1);
-        }
-        if (mm < tm) acc0 = fma(sK[mm], sR[off - mm], acc0);
+    __shared__ double sK[RING_L];
+    __shared__ double sR[RING_L + 256];
+    __shared__ bool last;
+    const int ib = blockIdx.x * 256, i = ib + threadIdx.x;
+    const int m0 = blockIdx.y * RING_L, tm = min(RING_L, n - m0);
+    for (int q = threadIdx.x; q < tm; q += 256) sK[q] = tab[m0 + q];
+    // sR[q] = rho[(ib - m0 - (tm - 1) + q) mod n], q in [0, tm + 255)
+    const int lo = wrap_index(ib - m0 - (tm - 1), n);
+    for (int q = threadIdx.x; q < tm + 255; q += 256) sR[q] = rho[(lo + q) % n];
+    __syncthreads();
+    // rho index i - m  ->  sR[(i - ib) + (tm - 1) - (m - m0)]
+    const int off = threadIdx.x + tm - 1;
+    double acc0 = 0.0, acc1 = 0.0, acc2 = 0.0, acc3 = 0.0;
+    int mm = 0;
+    for (; mm + 4 <= tm; mm += 4) {
+        acc0 = fma(sK[mm], sR[off - mm], acc0);
+        acc1 = fma(sK[mm + 1], sR[off - mm - 1], acc1);
+        acc2 = fma(sK[mm + 2], sR[off - mm - 2], acc2);
+        acc3 = fma(sK[mm + 3], sR[off - mm - 3], acc3);
     }
-    if (i < n) out[i] = (acc0 + acc1) * scale;
+    for (; mm < tm; ++mm) acc0 = fma(sK[mm], sR[off - mm], acc0);
+    if (i < n) __stcg(part + (size_t)blockIdx.y * n + i, (acc0 + acc1) + (acc2 + acc3));
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        const bool l = (atomicAdd(tickets + blockIdx.x, 1u) == gridDim.y - 1);
+        if (l) tickets[blockIdx.x] = 0u;
+        last = l;
+    }
+    __syncthreads();
+    if (!last) return;
+    __threadfence();
+    if (i < n) {
+        double t = 0.0;
+        for (unsigned c = 0; c < gridDim.y; ++c) t += __ldcg(part + (size_t)c * n + i);
+        out[i] = t * scale;
+    }
 }
 
 // sheet, eq (4) (L41-L45), reading D11: F_i = -dx (sum_{k<i} rho_k - sum_{k>i} rho_k) = -dx (2 C_i + rho_i - S)

@@ -582,9 +582,10 @@ int rho_from_colpart(int bands, double* rho_out, bool hmf_partials, double* colp
                      bool fuse_force = false) {
     const double dp = (G.pmax - G.pmin) / (double)G.np;
     const double dx = (G.xmax - G.xmin) / (double)G.ntheta;
+    const bool sheet = fuse_force && G.model == VLASOV_MODEL_SHEET;
     vl::rho_force_kernel<<<cdiv(G.ntheta, vl::RR_COLS), vl::RR_COLS * vl::RR_GROUPS, 0, G.stream>>>(
         colpart ? colpart : G.colpart, bands, G.ntheta, dp, rho_out, G.cos_t, G.sin_t, hmf_partials ? G.mpart : nullptr,
-        zero_after ? 1 : 0, G.ticket, dx, (fuse_force && hmf_partials) ? G.force : nullptr);
+        zero_after ? 1 : 0, G.ticket, dx, (fuse_force && (hmf_partials || sheet)) ? G.force : nullptr, sheet ? 1 : 0);
     LAUNCH_CHECK();
     return VLASOV_OK;
 }
@@ -613,7 +614,7 @@ int force_from_rho() {
 int rho_and_force(int bands, double* colpart, bool zero_after) {
     const bool hmf = (G.model == VLASOV_MODEL_HMF);
     int rc = rho_from_colpart(bands, G.rho, hmf, colpart, zero_after, true);
-    if (rc != 0 || hmf) return rc;
+    if (rc != 0 || hmf || G.model == VLASOV_MODEL_SHEET) return rc;  // those two forces come out of the same kernel
     return force_from_rho();
 }
 

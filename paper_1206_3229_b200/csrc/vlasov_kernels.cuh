@@ -343,6 +343,108 @@ __device__ __forceinline__ double block_sum(double v, double* red /* NT/32 doubl
     return t;  // valid in thread 0
 }
 
+// sheet, eq (4) (L41-L45), reading D11: F_i = -dx (sum_{k<i} rho_k - sum_{k>i} rho_k) = -dx (2 C_i + rho_i - S)
+// with C the exclusive prefix sum and S the total.  One CTA of 1024 threads scans the whole vector.
+// With mode = 1 writes instead the potential phi_i = dx sum_k |x_i - x_k| rho_k (for the energy):
+// phi_i = dx * dxnode * (i (2 C_i - S + rho_i) ... ) evaluated from the two prefix sums of rho_k and k rho_k.
+// (device body: also the tail of rho_force_kernel's last CTA; rho is read through L2, it may just have been written
+// by other CTAs)
+__device__ __forceinline__ void sheet_scan_body(const double* rho, int n, double dx, int mode, double* out) {
+    __shared__ double wsum0[32], wsum1[32];
+    __shared__ double carry0, carry1, tot0, tot1;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    // pass 1: totals S0 = sum rho_k, S1 = sum k rho_k
+    {
+        double a0 = 0.0, a1 = 0.0;
+        for (int k = threadIdx.x; k < n; k += 1024) {
+            const double rk = __ldcg(rho + k);
+            a0 += rk;
+            a1 += (double)k * rk;
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            a0 += __shfl_down_sync(0xffffffffu, a0, o);
+            a1 += __shfl_down_sync(0xffffffffu, a1, o);
+        }
+        if (lane == 0) {
+            wsum0[warp] = a0;
+            wsum1[warp] = a1;
+        }
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            double t0 = 0.0, t1 = 0.0;
+            for (int q = 0; q < 32; ++q) {
+                t0 += wsum0[q];
+                t1 += wsum1[q];
+            }
+            tot0 = t0;
+            tot1 = t1;
+            carry0 = 0.0;
+            carry1 = 0.0;
+        }
+        __syncthreads();
+    }
+    // pass 2: chunked inclusive scan with carry
+    for (int base = 0; base < n; base += 1024) {
+        const int k = base + threadIdx.x;
+        const double r = (k < n) ? __ldcg(rho + k) : 0.0;
+        double x0 = r, x1 = (double)k * r;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const double y0 = __shfl_up_sync(0xffffffffu, x0, o);
+            const double y1 = __shfl_up_sync(0xffffffffu, x1, o);
+            if (lane >= o) {
+                x0 += y0;
+                x1 += y1;
+            }
+        }
+        __syncthreads();
+        if (lane == 31) {
+            wsum0[warp] = x0;
+            wsum1[warp] = x1;
+        }
+        __syncthreads();
+        if (warp == 0) {
+            double z0 = wsum0[lane], z1 = wsum1[lane];
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const double y0 = __shfl_up_sync(0xffffffffu, z0, o);
+                const double y1 = __shfl_up_sync(0xffffffffu, z1, o);
+                if (lane >= o) {
+                    z0 += y0;
+                    z1 += y1;
+                }
+            }
+            wsum0[lane] = z0;
+            wsum1[lane] = z1;
+        }
+        __syncthreads();
+        const double inc0 = carry0 + (warp > 0 ? wsum0[warp - 1] : 0.0) + x0;  // inclusive prefix of rho
+        const double inc1 = carry1 + (warp > 0 ? wsum1[warp - 1] : 0.0) + x1;  // inclusive prefix of k rho
+        if (k < n) {
+            const double C0 = inc0 - r;                  // sum_{q<k} rho_q
+            const double C1 = inc1 - (double)k * r;      // sum_{q<k} q rho_q
+            if (mode == 0) {
+                out[k] = -dx * (2.0 * C0 + r - tot0);
+            } else {
+                // sum_q |k - q| rho_q = k C0 - C1 + (S1 - C1 - k r) - k (S0 - C0 - r)
+                const double right0 = tot0 - C0 - r, right1 = tot1 - C1 - (double)k * r;
+                out[k] = dx * dx * (((double)k * C0 - C1) + (right1 - (double)k * right0));
+            }
+        }
+        __syncthreads();
+        if (threadIdx.x == 1023) {
+            carry0 = inc0;
+            carry1 = inc1;
+        }
+        __syncthreads();
+    }
+}
+
+__global__ void __launch_bounds__(1024) sheet_scan_kernel(const double* rho, int n, double dx, int mode, double* out) {
+    sheet_scan_body(rho, n, dx, mode, out);
+}
+
 // rho_i = dp * sum_b colpart[b][i]; for HMF also per-CTA partial sums of cos(theta_i) rho_i, sin(theta_i) rho_i.
 // zero_after: the partials of the one-pass kernel are accumulated by atomic adds and must be zero for the next pass.
 // 32 columns x 32 groups of bands per CTA, and for the HMF model fused
@@ -354,7 +456,8 @@ __global__ void __launch_bounds__(RR_COLS* RR_GROUPS)
     rho_force_kernel(double* __restrict__ colpart, int nbands, int ntheta, double dp, double* __restrict__ rho,
                      const double* __restrict__ cos_t, const double* __restrict__ sin_t,
                      double* __restrict__ mpart /* [gridDim.x][2] or null */, int zero_after,
-                     unsigned* __restrict__ ticket, double dtheta, double* __restrict__ force /* null: no force */) {
+                     unsigned* __restrict__ ticket, double dtheta, double* __restrict__ force /* null: no force */,
+                     int sheet /* 1: the last CTA writes the sheet force (prefix scan of rho) instead */) {
     __shared__ double part[RR_GROUPS][RR_COLS];
     __shared__ double2 mp[RR_COLS * RR_GROUPS];
     __shared__ bool last;
@@ -406,22 +509,28 @@ __global__ void __launch_bounds__(RR_COLS* RR_GROUPS)
             if (tid == 0) {
                 mpart[2 * blockIdx.x + 0] = cs;
                 mpart[2 * blockIdx.x + 1] = ss;
-                bool l = false;
-                if (force != nullptr) {
-                    __threadfence();
-                    l = (atomicAdd(ticket, 1u) == gridDim.x - 1);
-                    if (l) *ticket = 0u;
-                }
-                last = l;
             }
         }
+        if (tid == 0) {
+            bool l = false;
+            if (force != nullptr) {
+                __threadfence();
+                l = (atomicAdd(ticket, 1u) == gridDim.x - 1);
+                if (l) *ticket = 0u;
+            }
+            last = l;
+        }
     }
-    if (mpart == nullptr) return;
+    if (force == nullptr) return;
     __syncthreads();
     if (!last) return;
+    __threadfence();
+    if (sheet) {  // eq (4), D11: F_i = -dx (2 C_i + rho_i - S) from the prefix sums of the rho every CTA has written
+        sheet_scan_body(rho, ntheta, dtheta, 0, force);
+        return;
+    }
     // last CTA: M = dtheta * (sum of the partials over a fixed tree: thread t adds partials t, t + 1024, ...; then
     // shuffles inside each warp, then across the warps), the same whichever CTA happens to be last; then the force
-    __threadfence();
     double mx = 0.0, my = 0.0;
     for (unsigned b = tid; b < gridDim.x; b += RR_COLS * RR_GROUPS) {
         mx += __ldcg(mpart + 2 * b);
@@ -500,102 +609,6 @@ __global__ void __launch_bounds__(256) ring_convolve_kernel(const double* __rest
         double t = 0.0;
         for (unsigned c = 0; c < gridDim.y; ++c) t += __ldcg(part + (size_t)c * n + i);
         out[i] = t * scale;
-    }
-}
-
-// sheet, eq (4) (L41-L45), reading D11: F_i = -dx (sum_{k<i} rho_k - sum_{k>i} rho_k) = -dx (2 C_i + rho_i - S)
-// with C the exclusive prefix sum and S the total.  One CTA of 1024 threads scans the whole vector.
-// With mode = 1 writes instead the potential phi_i = dx sum_k |x_i - x_k| rho_k (for the energy):
-// phi_i = dx * dxnode * (i (2 C_i - S + rho_i) ... ) evaluated from the two prefix sums of rho_k and k rho_k.
-__global__ void __launch_bounds__(1024) sheet_scan_kernel(const double* __restrict__ rho, int n, double dx, int mode,
-                                                          double* __restrict__ out) {
-    __shared__ double wsum0[32], wsum1[32];
-    __shared__ double carry0, carry1, tot0, tot1;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    // pass 1: totals S0 = sum rho_k, S1 = sum k rho_k
-    {
-        double a0 = 0.0, a1 = 0.0;
-        for (int k = threadIdx.x; k < n; k += 1024) {
-            a0 += rho[k];
-            a1 += (double)k * rho[k];
-        }
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) {
-            a0 += __shfl_down_sync(0xffffffffu, a0, o);
-            a1 += __shfl_down_sync(0xffffffffu, a1, o);
-        }
-        if (lane == 0) {
-            wsum0[warp] = a0;
-            wsum1[warp] = a1;
-        }
-        __syncthreads();
-        if (threadIdx.x == 0) {
-            double t0 = 0.0, t1 = 0.0;
-            for (int q = 0; q < 32; ++q) {
-                t0 += wsum0[q];
-                t1 += wsum1[q];
-            }
-            tot0 = t0;
-            tot1 = t1;
-            carry0 = 0.0;
-            carry1 = 0.0;
-        }
-        __syncthreads();
-    }
-    // pass 2: chunked inclusive scan with carry
-    for (int base = 0; base < n; base += 1024) {
-        const int k = base + threadIdx.x;
-        const double r = (k < n) ? rho[k] : 0.0;
-        double x0 = r, x1 = (double)k * r;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            const double y0 = __shfl_up_sync(0xffffffffu, x0, o);
-            const double y1 = __shfl_up_sync(0xffffffffu, x1, o);
-            if (lane >= o) {
-                x0 += y0;
-                x1 += y1;
-            }
-        }
-        __syncthreads();
-        if (lane == 31) {
-            wsum0[warp] = x0;
-            wsum1[warp] = x1;
-        }
-        __syncthreads();
-        if (warp == 0) {
-            double z0 = wsum0[lane], z1 = wsum1[lane];
-#pragma unroll
-            for (int o = 1; o < 32; o <<= 1) {
-                const double y0 = __shfl_up_sync(0xffffffffu, z0, o);
-                const double y1 = __shfl_up_sync(0xffffffffu, z1, o);
-                if (lane >= o) {
-                    z0 += y0;
-                    z1 += y1;
-                }
-            }
-            wsum0[lane] = z0;
-            wsum1[lane] = z1;
-        }
-        __syncthreads();
-        const double inc0 = carry0 + (warp > 0 ? wsum0[warp - 1] : 0.0) + x0;  // inclusive prefix of rho
-        const double inc1 = carry1 + (warp > 0 ? wsum1[warp - 1] : 0.0) + x1;  // inclusive prefix of k rho
-        if (k < n) {
-            const double C0 = inc0 - r;                  // sum_{q<k} rho_q
-            const double C1 = inc1 - (double)k * r;      // sum_{q<k} q rho_q
-            if (mode == 0) {
-                out[k] = -dx * (2.0 * C0 + r - tot0);
-            } else {
-                // sum_q |k - q| rho_q = k C0 - C1 + (S1 - C1 - k r) - k (S0 - C0 - r)
-                const double right0 = tot0 - C0 - r, right1 = tot1 - C1 - (double)k * r;
-                out[k] = dx * dx * (((double)k * C0 - C1) + (right1 - (double)k * right0));
-            }
-        }
-        __syncthreads();
-        if (threadIdx.x == 1023) {
-            carry0 = inc0;
-            carry1 = inc1;
-        }
-        __syncthreads();
     }
 }
 

@@ -4,7 +4,7 @@
 //   p warps (4, one warpgroup, setmaxnreg 152)
 //       thread t owns the three source columns t, t + 128, t + 256 of the CTA.  For each column a register window
 //       slides down (one new value + ten FMAs per row, eq (11)); new values arrive by per-thread cp.async
-//       into a ring of NSTG groups of 12 rows; the shifted value overwrites the tap in place.  After every 4 rows
+//       into a ring of NSTG groups of 12 rows; the shifted value overwrites the tap in place.  After every 2 rows
 //       ("sub-slot") the warp arrives on the sub-slot's READY mbarrier.  Before refilling a group it waits for
 //       the EMPTY mbarriers of its three sub-slots.
 //   theta warps (NTW = 12, three warpgroups, setmaxnreg 120; 8 at 176 registers also builds)
@@ -42,7 +42,10 @@ struct FusedWsCfg {
     static constexpr int CPT = 3;                       // columns per p thread
     static constexpr int PITCH = NPT * CPT;             // columns of a ring row
     static constexpr int RG = 12;                       // rows per group = length of the register ring
-    static constexpr int SUB = 4;                       // rows per sub-slot (granularity of READY / EMPTY)
+#ifndef VL_FW_SUB
+#define VL_FW_SUB 2
+#endif
+    static constexpr int SUB = VL_FW_SUB;               // rows per sub-slot (granularity of READY / EMPTY)
     static constexpr int SPG = RG / SUB;                // sub-slots per group
     static constexpr int NSUB = NSTG * SPG;
     static constexpr int NTAP = NST == 2 ? 19 : 10;

@@ -45,6 +45,9 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, unsigned parity) {
 __device__ __forceinline__ void mbar_arrive_u32(uint32_t bar) {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
+#ifndef VL_MBAR_HINT_NS
+#define VL_MBAR_HINT_NS 100000
+#endif
 __device__ __forceinline__ void mbar_wait_u32(uint32_t bar, unsigned parity) {
     asm volatile(
         "{\n"
@@ -55,7 +58,7 @@ __device__ __forceinline__ void mbar_wait_u32(uint32_t bar, unsigned parity) {
         "bra LAB_WAIT;\n"
         "DONE:\n"
         "}\n" ::"r"(bar),
-        "r"(parity), "r"(100000u)
+        "r"(parity), "r"((unsigned)VL_MBAR_HINT_NS)
         : "memory");
 }
 

@@ -64,7 +64,11 @@ struct FusedWsCfg {
     static_assert(R & 1, "lane stride R must be odd (shared-memory banks)");
     static_assert(NTW % SUB == 0 && NTW <= RG, "a sub-slot is released by SUB different theta warps");
     // registers per thread after setmaxnreg: 128*152 + 384*120 = 65536; 128*152 + 256*176 = 64512
-    static constexpr int P_REGS = 152, T_REGS = NTW == 12 ? 120 : 176;
+#ifndef VL_FW_PREGS
+#define VL_FW_PREGS 152
+#define VL_FW_TREGS 120
+#endif
+    static constexpr int P_REGS = VL_FW_PREGS, T_REGS = NTW == 12 ? VL_FW_TREGS : 176;
     static constexpr int LAUNCH_REGS = 65536 / NT / 8 * 8;
     static_assert(NPW * 32 * P_REGS + NTW * 32 * T_REGS <= 65536 && P_REGS % 8 == 0 && T_REGS % 8 == 0, "");
     static_assert(RING_BYTES % 16 == 0 && O_BYTES % 16 == 0 && W_BYTES % 16 == 0, "");

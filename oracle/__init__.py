@@ -14,13 +14,17 @@ from .vlasov_oracle import (  # noqa: F401
     KEY_BC_P,
     KEY_BC_X,
     KEY_EPS,
+    KEY_SPLINE,
     MODEL_FREE,
     MODEL_HMF,
     MODEL_RING,
     MODEL_SHEET,
     Oracle,
+    SPLINE_FD,
+    SPLINE_GS,
     build,
     fd8_second_derivative,
     force_from_rho,
+    gs_second_derivative,
     shift_line,
 )

@@ -49,6 +49,16 @@
  * periodic.  Parity unpinned: none of the functions below; the long-time
  * nonlinear curves of Figs 1-5 (images absent) are not reproduced.
  *
+ * Global-spline variant (the paper's comparator "GS",
+ * L100-L104, Tables 1-2): with oracle_set_param(KEY_SPLINE, 1) the second
+ * derivatives are the solution of the tridiagonal system (15) of every line
+ * instead of eq (16); everything else is unchanged.  Periodic lines: the
+ * cyclic system.  Zero extension (D4, D21): the line is the infinite
+ * sequence that is 0 outside [0,n) and f'' its bounded solution of (15),
+ * obtained as the cyclic solution on the line padded by GS_EXT zeros on each
+ * side (the influence of a value decays by |sqrt(3)-2| = 0.268 per node:
+ * 0.268^64 = 2.6e-37).  Pins G1-G7 in tests/test_oracle_pins.py.
+ *
  * Sums that define integrals are accumulated in long double; everything else
  * is IEEE double.  Optional OpenMP over independent lines (off unless
  * oracle_set_threads(n>1) is called); it does not change any result.
@@ -67,7 +77,8 @@
 
 enum { MODEL_FREE = 0, MODEL_HMF = 1, MODEL_RING = 2, MODEL_SHEET = 3 };
 enum { BC_PERIODIC = 0, BC_ZERO = 1 };
-enum { KEY_EPS = 1, KEY_PRECISION = 2, KEY_BC_X = 3, KEY_BC_P = 4, KEY_HISTORY = 5 };
+enum { KEY_EPS = 1, KEY_PRECISION = 2, KEY_BC_X = 3, KEY_BC_P = 4, KEY_HISTORY = 5, KEY_SPLINE = 6 };
+enum { SPLINE_FD = 0, SPLINE_GS = 1 };
 
 /* eq (16): coefficients of f(u_{i-4}) ... f(u_{i+4}). */
 static const double C16[9] = {
@@ -75,6 +86,7 @@ static const double C16[9] = {
     8.0 / 5.0,    -1.0 / 5.0,  8.0 / 315.0, -1.0 / 560.0};
 
 #define EXT 5 /* zero extension: f'' can be non-zero for -4 <= k < n+4; we keep k in [-5, n+5) */
+#define GS_EXT 64 /* zero extension, system (15): f'' decays by 0.268 per node outside [0,n); kept on [-64, n+64) */
 
 static int g_threads = 1;
 
@@ -111,9 +123,67 @@ void oracle_fd8_second_derivative(const double* u, long n, double h, int bc, dou
     }
 }
 
-static double d2_at(const double* d2, long n, int bc, long k) {
+static double d2_at_ext(const double* d2, long n, int bc, long k, long ext) {
     if (bc == BC_PERIODIC) return d2[wrap(k, n)];
-    return (k >= -EXT && k < n + EXT) ? d2[k + EXT] : 0.0;
+    return (k >= -ext && k < n + ext) ? d2[k + ext] : 0.0;
+}
+
+/*
+ * System (15) (L100-L102) with periodic closure, i = 0..n-1, indices mod n:
+ *     (d2[i+1]/6 + (2/3) d2[i] + d2[i-1]/6) = rhs[i],   rhs[i] = (u[i+1] - 2u[i] + u[i-1]) / h^2.
+ * Reading D22: the paper prints the middle coefficient as 1/3.  Continuity of the first derivative of
+ * eq (13) across the knot x_i (the condition the text states, L100) gives h/6 d2[i-1] + (h/3 + h/3) d2[i] +
+ * h/6 d2[i+1]: each of the two intervals that meet at x_i contributes h/3, so the coefficient is 2/3 (the
+ * form of ref. [37]).  With 1/3 a constant f'' would come out 3/2 too large and the system is singular
+ * on the mode (-1)^i.  Solved directly: Thomas elimination of the tridiagonal part plus the
+ * Sherman-Morrison correction for the two corner entries.  n >= 3.  scratch: 3n doubles.
+ */
+static void cyclic_spline_system(const double* rhs, long n, double* x, double* scratch) {
+    const double lo = 1.0 / 6.0, di = 2.0 / 3.0, up = 1.0 / 6.0;
+    double* cp = scratch;         /* modified upper diagonal */
+    double* y = scratch + n;      /* solution of T y = rhs   */
+    double* z = scratch + 2 * n;  /* solution of T z = u     */
+    /* A = T + u v^T, T tridiagonal with T[0][0] = di - gamma, T[n-1][n-1] = di - up*lo/gamma,
+       u = (gamma, 0, .., 0, up)^T, v = (1, 0, .., 0, lo/gamma)^T;  x = y - z (v.y)/(1 + v.z) */
+    const double gamma = -di;
+    for (int pass = 0; pass < 2; ++pass) {
+        double* out = pass == 0 ? y : z;
+        double b0 = di - gamma, bn = di - up * lo / gamma;
+        double r0 = pass == 0 ? rhs[0] : gamma;
+        cp[0] = up / b0;
+        out[0] = r0 / b0;
+        for (long i = 1; i < n; ++i) {
+            double b = (i == n - 1) ? bn : di;
+            double r = pass == 0 ? rhs[i] : (i == n - 1 ? up : 0.0);
+            double m = b - lo * cp[i - 1];
+            cp[i] = up / m;
+            out[i] = (r - lo * out[i - 1]) / m;
+        }
+        for (long i = n - 2; i >= 0; --i) out[i] -= cp[i] * out[i + 1];
+    }
+    double vy = y[0] + lo / gamma * y[n - 1];
+    double vz = z[0] + lo / gamma * z[n - 1];
+    double fac = vy / (1.0 + vz);
+    for (long i = 0; i < n; ++i) x[i] = y[i] - fac * z[i];
+}
+
+/*
+ * Second derivatives of the global cubic spline, system (15).
+ * periodic: d2 has n entries.  zero ext: d2 has n + 2*GS_EXT entries, d2[k + GS_EXT] = f''(u_k).
+ * Returns 0, or ORACLE_ENOMEM / ORACLE_EINVAL (n < 3).
+ */
+int oracle_gs_second_derivative(const double* u, long n, double h, int bc, double* d2) {
+    long lo = (bc == BC_PERIODIC) ? 0 : -GS_EXT;
+    long hi = (bc == BC_PERIODIC) ? n : n + GS_EXT;
+    long N = hi - lo;
+    if (N < 3) return ORACLE_EINVAL;
+    double* rhs = (double*)malloc((size_t)N * 4 * sizeof(double));
+    if (!rhs) return ORACLE_ENOMEM;
+    for (long k = lo; k < hi; ++k)
+        rhs[k - lo] = (line_at(u, n, bc, k + 1) - 2.0 * line_at(u, n, bc, k) + line_at(u, n, bc, k - 1)) / (h * h);
+    cyclic_spline_system(rhs, N, d2, rhs + N);
+    free(rhs);
+    return ORACLE_OK;
 }
 
 /*
@@ -123,11 +193,19 @@ static double d2_at(const double* d2, long n, int bc, long k) {
  * k = i + s, s = floor(-disp/h); in the paper's symbols
  *   alpha = (x_{k+1} - x)/h = 1 - a,  beta = 1 - alpha = a,
  *   gamma = (alpha^3 - alpha) h^2/6,  delta = (beta^3 - beta) h^2/6.
- * d2 is scratch of n + 2*EXT doubles.
+ * kind = SPLINE_FD: f'' from eq (16); SPLINE_GS: f'' from system (15).
+ * d2 is scratch of n + 2*GS_EXT doubles.
  */
-void oracle_shift_line(const double* in, long n, double h, double disp, int bc, double* out,
-                       double* d2) {
-    oracle_fd8_second_derivative(in, n, h, bc, d2);
+int oracle_shift_line_kind(const double* in, long n, double h, double disp, int bc, int kind, double* out,
+                           double* d2) {
+    long ext = EXT;
+    if (kind == SPLINE_GS) {
+        int rc = oracle_gs_second_derivative(in, n, h, bc, d2);
+        if (rc != ORACLE_OK) return rc;
+        ext = GS_EXT;
+    } else {
+        oracle_fd8_second_derivative(in, n, h, bc, d2);
+    }
     double u = -disp / h;
     double sf = floor(u);
     double a = u - sf;
@@ -142,20 +220,32 @@ void oracle_shift_line(const double* in, long n, double h, double disp, int bc, 
     for (long i = 0; i < n; ++i) {
         long k = i + s;
         out[i] = alpha * line_at(in, n, bc, k) + beta * line_at(in, n, bc, k + 1) +
-                 gamma * d2_at(d2, n, bc, k) + delta * d2_at(d2, n, bc, k + 1);
+                 gamma * d2_at_ext(d2, n, bc, k, ext) + delta * d2_at_ext(d2, n, bc, k + 1, ext);
     }
+    return ORACLE_OK;
+}
+
+/* eq (16) variant (the paper's method); d2 is scratch of n + 2*GS_EXT doubles */
+void oracle_shift_line(const double* in, long n, double h, double disp, int bc, double* out,
+                       double* d2) {
+    (void)oracle_shift_line_kind(in, n, h, disp, bc, SPLINE_FD, out, d2);
 }
 
 /* convenience for the pins: allocates its own scratch */
-int oracle_shift_line_alloc(const double* in, long n, double h, double disp, int bc, double* out) {
-    double* d2 = (double*)malloc((size_t)(n + 2 * EXT) * sizeof(double));
+int oracle_shift_line_kind_alloc(const double* in, long n, double h, double disp, int bc, int kind,
+                                 double* out) {
+    double* d2 = (double*)malloc((size_t)(n + 2 * GS_EXT) * sizeof(double));
     double* tmp = (double*)malloc((size_t)n * sizeof(double));
     if (!d2 || !tmp) { free(d2); free(tmp); return ORACLE_ENOMEM; }
-    oracle_shift_line(in, n, h, disp, bc, tmp, d2);
-    memcpy(out, tmp, (size_t)n * sizeof(double));
+    int rc = oracle_shift_line_kind(in, n, h, disp, bc, kind, tmp, d2);
+    if (rc == ORACLE_OK) memcpy(out, tmp, (size_t)n * sizeof(double));
     free(d2);
     free(tmp);
-    return ORACLE_OK;
+    return rc;
+}
+
+int oracle_shift_line_alloc(const double* in, long n, double h, double disp, int bc, double* out) {
+    return oracle_shift_line_kind_alloc(in, n, h, disp, bc, SPLINE_FD, out);
 }
 
 /* pair potentials, eqs (2)-(4) (L33-L45), and K = -dV/dx for the ring */
@@ -220,6 +310,7 @@ typedef struct {
     long nx, np;
     double xmin, xmax, pmin, pmax, dt, eps, t;
     int bc_x, bc_p;
+    int spline; /* SPLINE_FD (eq 16, default) or SPLINE_GS (system 15) */
     double* f;
 } ctx_t;
 
@@ -247,6 +338,7 @@ int oracle_init(int model, const int grid[2], const double domain[4], double dt)
     G.t = 0.0;
     G.bc_x = (model == MODEL_SHEET) ? BC_ZERO : BC_PERIODIC;
     G.bc_p = BC_ZERO;
+    G.spline = SPLINE_FD;
     G.f = (double*)calloc((size_t)G.nx * (size_t)G.np, sizeof(double));
     if (!G.f) return ORACLE_ENOMEM;
     G.ready = 1;
@@ -261,6 +353,7 @@ int oracle_set_param(int key, double value) {
         case KEY_BC_X: if (value != 0.0 && value != 1.0) return ORACLE_EINVAL; G.bc_x = (int)value; break;
         case KEY_BC_P: if (value != 0.0 && value != 1.0) return ORACLE_EINVAL; G.bc_p = (int)value; break;
         case KEY_HISTORY: break;
+        case KEY_SPLINE: if (value != 0.0 && value != 1.0) return ORACLE_EINVAL; G.spline = (int)value; break;
         default: return ORACLE_EINVAL;
     }
     return ORACLE_OK;
@@ -292,11 +385,11 @@ int oracle_theta_sweep(double tau) {
 #pragma omp parallel num_threads(g_threads)
     {
         double* out = (double*)malloc((size_t)nx * sizeof(double));
-        double* d2 = (double*)malloc((size_t)(nx + 2 * EXT) * sizeof(double));
+        double* d2 = (double*)malloc((size_t)(nx + 2 * GS_EXT) * sizeof(double));
 #pragma omp for schedule(static)
         for (long j = 0; j < np; ++j) {
             double* row = G.f + (size_t)j * (size_t)nx;
-            oracle_shift_line(row, nx, h, p_at(j) * tau, G.bc_x, out, d2);
+            (void)oracle_shift_line_kind(row, nx, h, p_at(j) * tau, G.bc_x, G.spline, out, d2);
             memcpy(row, out, (size_t)nx * sizeof(double));
         }
         free(out);
@@ -337,11 +430,11 @@ int oracle_p_sweep_with_force(const double* F, double dt) {
     {
         double* col = (double*)malloc((size_t)np * sizeof(double));
         double* out = (double*)malloc((size_t)np * sizeof(double));
-        double* d2 = (double*)malloc((size_t)(np + 2 * EXT) * sizeof(double));
+        double* d2 = (double*)malloc((size_t)(np + 2 * GS_EXT) * sizeof(double));
 #pragma omp for schedule(static)
         for (long i = 0; i < nx; ++i) {
             for (long j = 0; j < np; ++j) col[j] = G.f[(size_t)j * (size_t)nx + (size_t)i];
-            oracle_shift_line(col, np, h, F[i] * dt, G.bc_p, out, d2);
+            (void)oracle_shift_line_kind(col, np, h, F[i] * dt, G.bc_p, G.spline, out, d2);
             for (long j = 0; j < np; ++j) G.f[(size_t)j * (size_t)nx + (size_t)i] = out[j];
         }
         free(col);

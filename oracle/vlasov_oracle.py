@@ -18,7 +18,9 @@ _LIB = os.path.join(_HERE, "libvlasov_oracle.so")
 
 MODEL_FREE, MODEL_HMF, MODEL_RING, MODEL_SHEET = 0, 1, 2, 3
 BC_PERIODIC, BC_ZERO = 0, 1
-KEY_EPS, KEY_PRECISION, KEY_BC_X, KEY_BC_P, KEY_HISTORY = 1, 2, 3, 4, 5
+KEY_EPS, KEY_PRECISION, KEY_BC_X, KEY_BC_P, KEY_HISTORY, KEY_SPLINE = 1, 2, 3, 4, 5, 6
+SPLINE_FD, SPLINE_GS = 0, 1
+GS_EXT = 64
 
 _lock = threading.Lock()
 _lib = None
@@ -62,6 +64,8 @@ def _load():
             lib.oracle_fd8_second_derivative.argtypes = [_dp, ctypes.c_long, ctypes.c_double, ctypes.c_int, _dp]
             lib.oracle_fd8_second_derivative.restype = None
             lib.oracle_shift_line_alloc.argtypes = [_dp, ctypes.c_long, ctypes.c_double, ctypes.c_double, ctypes.c_int, _dp]
+            lib.oracle_gs_second_derivative.argtypes = [_dp, ctypes.c_long, ctypes.c_double, ctypes.c_int, _dp]
+            lib.oracle_shift_line_kind_alloc.argtypes = [_dp, ctypes.c_long, ctypes.c_double, ctypes.c_double, ctypes.c_int, ctypes.c_int, _dp]
             lib.oracle_force_from_rho.argtypes = [ctypes.c_int, _dp, ctypes.c_long, ctypes.c_double, ctypes.c_double, ctypes.c_double, _dp]
             lib.oracle_force_from_rho.restype = None
             _lib = lib
@@ -89,11 +93,21 @@ def fd8_second_derivative(u, h: float, bc: int = BC_PERIODIC) -> np.ndarray:
     return out
 
 
-def shift_line(u, h: float, disp: float, bc: int = BC_PERIODIC) -> np.ndarray:
-    """out_i = f(x_i - disp) by eqs (13)-(14) with f'' from eq (16)."""
+def gs_second_derivative(u, h: float, bc: int = BC_PERIODIC) -> np.ndarray:
+    """System (15).  Periodic: n values.  Zero extension: n+128 values for k=-64..n+63."""
+    u = np.ascontiguousarray(u, dtype=np.float64)
+    n = u.shape[0]
+    out = np.empty(n if bc == BC_PERIODIC else n + 2 * GS_EXT, dtype=np.float64)
+    _check(_load().oracle_gs_second_derivative(_ptr(u), n, float(h), int(bc), _ptr(out)), "gs_second_derivative")
+    return out
+
+
+def shift_line(u, h: float, disp: float, bc: int = BC_PERIODIC, spline: int = SPLINE_FD) -> np.ndarray:
+    """out_i = f(x_i - disp) by eqs (13)-(14) with f'' from eq (16) (or system (15) for SPLINE_GS)."""
     u = np.ascontiguousarray(u, dtype=np.float64)
     out = np.empty_like(u)
-    _check(_load().oracle_shift_line_alloc(_ptr(u), u.shape[0], float(h), float(disp), int(bc), _ptr(out)), "shift_line")
+    _check(_load().oracle_shift_line_kind_alloc(_ptr(u), u.shape[0], float(h), float(disp), int(bc), int(spline),
+                                                _ptr(out)), "shift_line")
     return out
 
 
@@ -121,7 +135,7 @@ class Oracle:
         _check(self.lib.oracle_init(int(model), g, d, float(dt)), "init")
         self.lib.oracle_set_threads(int(threads))
         for k, v in params.items():
-            key = {"eps": KEY_EPS, "bc_x": KEY_BC_X, "bc_p": KEY_BC_P}[k]
+            key = {"eps": KEY_EPS, "bc_x": KEY_BC_X, "bc_p": KEY_BC_P, "spline": KEY_SPLINE}[k]
             _check(self.lib.oracle_set_param(key, float(v)), "set_param")
 
     @property

@@ -132,14 +132,14 @@ def max_over_ranks(value: float, world: int, backend_device=None) -> float:
 
 
 # ------------------------------------------------------------------------------------------ oracle legs
-def oracle_throughput(n: int, steps: int, warmup: int = 0, min_seconds: float = 0.0):
+def oracle_throughput(n: int, steps: int, warmup: int = 0, min_seconds: float = 0.0, spline: int = 0):
     """Gpts/s of the CPU oracle on the cfg-5 workload at grid n x n, all host cores."""
     import oracle
     from paper_1206_3229_b200 import inputs
 
     cores = os.cpu_count() or 1
     c = inputs.config("cfg5", n=n)
-    o = oracle.Oracle(c["model"], c["grid"], c["domain"], c["dt"], threads=cores)
+    o = oracle.Oracle(c["model"], c["grid"], c["domain"], c["dt"], threads=cores, **({"spline": spline} if spline else {}))
     o.upload(c["f0"])
     if warmup:
         o.step(warmup)
@@ -161,7 +161,7 @@ def run_reference(args):
         return 0
     n_ref = args.ref_n
     t0 = time.perf_counter()
-    val, el, done, threads = oracle_throughput(n_ref, args.steps, warmup=args.warmup)
+    val, el, done, threads = oracle_throughput(n_ref, args.steps, warmup=args.warmup, spline=int(args.spline == "gs"))
     sample = "CPU oracle (oracle/vlasov_oracle.c, OpenMP over lines), cfg5 HMF water-bag at %dx%d (bounded sample of the %dx%d workload), %d Strang steps" % (
         n_ref, n_ref, args.n, args.n, done)
     line = {
@@ -200,6 +200,7 @@ def run_cuda(args):
     f0 = c["f0"].astype(np.float64 if prec == 64 else np.float32)
     g = vb.Vlasov(c["model"], c["grid"], c["domain"], c["dt"], precision=prec, device="cuda:%d" % local_rank,
                   fuse=args.fuse, tune_fvariant=args.fvariant, tune_graph=args.graph,
+                  **({"spline": vb.SPLINE_GS} if args.spline == "gs" else {}),
                   **({"tune_fbands": args.fbands} if args.fbands > 0 else {}))
     g.upload(f0)
     pts = float(n) * float(n)
@@ -264,6 +265,16 @@ def run_cuda(args):
                     "step_frac": (step_bytes * pts * K / (ms_local * 1e-3) / 1e9) / peak,
                     "step_bytes_per_point": step_bytes,
                     "two_pass_step_frac": (4 * eb * pts * K / (ms_local * 1e-3) / 1e9) / peak}
+        if args.spline == "gs":
+            # 60 FMAs per point and pass: bound by the fp64 pipe.  Peak = the measured fp64 FMA rate of this B200,
+            # 17.0 TFMA/s = 34.0 TFLOP/s (profiles/fp64_probe.txt; csrc/fp64_probe.cu), DESIGN.md section 7.
+            gs_names = {"theta1": "gs_theta_sweep_kernel", "p": "gs_p_sweep_kernel"}
+            flops = 2.0 * 60.0 * pts
+            ach_tf = flops / (kern[dom]["avg_ms"] * 1e-3) / 1e12
+            roofline = {"bound": "alu", "kernel": gs_names.get(dom, dom), "achieved": ach_tf, "peak": 34.0,
+                        "unit": "TFLOP/s", "frac": ach_tf / 34.0, "traffic": None,
+                        "peak_source": "measured fp64 FMA rate, profiles/fp64_probe.txt (17.0 TFMA/s)",
+                        "algorithmic_flops_per_launch": flops, "hbm_gbs": ach, "hbm_frac": ach / peak}
 
     # ---- end to end through the C ABI with host buffers
     Ke = min(K, args.e2e_steps)
@@ -301,7 +312,7 @@ def run_cuda(args):
     cpu = None
     if not args.no_cpu_baseline:
         nb = args.cpu_n
-        val, el, done, threads = oracle_throughput(nb, 1, warmup=0, min_seconds=args.cpu_seconds)
+        val, el, done, threads = oracle_throughput(nb, 1, warmup=0, min_seconds=args.cpu_seconds, spline=int(args.spline == "gs"))
         cpu = {"value": val, "unit": UNIT, "cores": threads, "kind": "oracle",
                "sample": "%d Strang step(s) of cfg5 HMF water-bag on a %dx%d grid (%.1f s of wall time), oracle/vlasov_oracle.c with OpenMP over lines" % (done, nb, nb, el)}
 
@@ -309,7 +320,8 @@ def run_cuda(args):
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64" if prec == 64 else "f32", "data": "synthetic",
-        "config": {"workload": "cfg5 HMF water-bag %dx%d %s, dt=0.1, theta periodic, p zero-extended, seeded 1e-6 noise" % (n, n, "fp64" if prec == 64 else "fp32"),
+        "config": {"workload": "cfg5 HMF water-bag %dx%d %s, dt=0.1, theta periodic, p zero-extended, seeded 1e-6 noise%s" % (
+                       n, n, "fp64" if prec == 64 else "fp32", ", global-spline variant (system 15)" if args.spline == "gs" else ""),
                    "grid": [n, n], "passes_per_step": passes / K, "fuse": args.fuse,
                    "l2": "state (%.0f MiB x 2 buffers) exceeds the 126 MB L2; no flush needed" % (pts * eb / 2 ** 20)
                    if pts * eb > 126e6 else "state fits L2: DRAM roofline not claimed",
@@ -339,6 +351,9 @@ def main():
     ap.add_argument("--fbands", type=int, default=0, help="bands of rows of the one-pass kernel (0 = automatic)")
     ap.add_argument("--graph", type=int, default=1, choices=[0, 1],
                     help="1 (default): steady-state step pairs are launched as CUDA graphs, 0: plain launches")
+    ap.add_argument("--spline", default="fd", choices=["fd", "gs"],
+                    help="fd: f'' by eq (16), the paper's method and the headline workload; gs: the Global Spline "
+                         "comparator, system (15) (SURVEY 8(f) NEXT #2; three 60-tap passes per step, fp64-ALU bound)")
     ap.add_argument("--fvariant", type=int, default=0, choices=[0, 1],
                     help="one-pass kernel: 0 = warp-specialised (default), 1 = every warp does both stages")
     args = ap.parse_args()

@@ -57,6 +57,11 @@ extern "C" {
                                   (p shift, both half theta shifts and the density of the next step share a pass;
                                   needs periodic x, otherwise behaves like 1)                                   */
 #define VLASOV_KEY_PROFILE 7   /* 1: bracket every sweep launch of vlasov_step with CUDA events (any time)   */
+#define VLASOV_KEY_SPLINE 8    /* which f'' enters eq (13): 0 (default) the local eighth-order difference of eq (16),
+                                  L106-L111, the paper's method; 1 the GLOBAL SPLINE, f'' = solution of the
+                                  tridiagonal system (15), L100-L102 (the paper's comparator "GS", Tables 1-2;
+                                  diagonal 2/3, D22).  Three passes per step, 60 taps per shift instead
+                                  of 10; both axes need >= 32 nodes                                             */
 /* keys 101..108 (launch-shape overrides: warps, bands, segment lengths, kernel variant) exist for the tests and
  * the tuning sweeps only; see binding.py KEY_TUNE_*.  Results never depend on them beyond rounding order.   */
 

@@ -18,6 +18,7 @@
 #include "vlasov_theta_bulk.cuh"
 #include "vlasov_fused.cuh"
 #include "vlasov_fused_ws.cuh"
+#include "vlasov_gs.cuh"
 
 namespace {
 
@@ -44,6 +45,9 @@ struct Ctx {
     int model = 0, ntheta = 0, np = 0;
     double xmin = 0, xmax = 0, pmin = 0, pmax = 0, dt = 0, eps = 0.01, t = 0;
     int bc_x = 0, bc_p = 1, prec = 64;
+    int spline = 0;  // 0: f'' by eq (16) (the paper's method), 1: global spline, system (15) (vlasov_gs.cuh)
+    double *gsw = nullptr, *gsH6 = nullptr;  // [Np][GS_NT] row weights of a half theta shift; H/6 table
+    int gs_bands = 0, gs_rpb = 0, gs_pseg = 0, gs_pnseg = 0, gs_tbd = 128;
     bool history = false;
     int fuse = 2;  // 0: p and theta passes apart, 1: adjacent half theta shifts in one pass, 2: p + theta in one pass
     cudaStream_t stream = nullptr;
@@ -155,13 +159,15 @@ int cdiv(int a, int b) { return (a + b - 1) / b; }
 
 void free_small() {
     void* ptrs[] = {G.srow, G.wrow, G.cos_t, G.sin_t, G.ringK, G.ringV, G.rho, G.force, G.rho_m,
-                    G.phi,  G.mpart, G.pkpart, G.mom_dev, G.hist, G.wrow2, G.colpart_f, G.ticket, G.caspart, G.ringpart, G.ringtick};
+                    G.phi,  G.mpart, G.pkpart, G.mom_dev, G.hist, G.wrow2, G.colpart_f, G.ticket, G.caspart, G.ringpart, G.ringtick,
+                    G.gsw, G.gsH6};
     for (void* p : ptrs)
         if (p) cudaFree(p);
     G.srow = nullptr;
     G.wrow = G.cos_t = G.sin_t = G.ringK = G.ringV = G.rho = G.force = G.rho_m = G.phi = G.mpart = G.pkpart =
         G.mom_dev = G.hist = G.wrow2 = G.colpart_f = nullptr;
     G.ticket = nullptr;
+    G.gsw = G.gsH6 = nullptr;
     G.caspart = nullptr;
     G.ringpart = nullptr;
     G.ringtick = nullptr;
@@ -447,6 +453,50 @@ int prepare() {
 
     int rc = (G.prec == 32) ? configure_all<float>() : configure_all<double>();
     if (rc != 0) return rc;
+    if (G.spline == 1) {
+        // global spline (system (15), L100-L102): 60-tap row weights of a half theta shift, H/6 for the p shift
+        if (nt < vl::GS_MIN_N || np < vl::GS_MIN_N)
+            return fail(VLASOV_EINVAL, "SPLINE = 1 (global spline) needs at least 32 nodes on both axes");
+        std::vector<double> H6(2 * vl::GS_Q + 3);
+        vl::gs_H_over_6(H6.data());
+        std::vector<double> gsw((size_t)np * vl::GS_NT);
+        for (int j = 0; j < np; ++j) {
+            const double p = G.pmin + (double)j * dp;
+            double sf, a;
+            vl::split_shift(-(p * tau) / dx, &sf, &a);
+            vl::gs_weights(a, H6.data(), &gsw[(size_t)j * vl::GS_NT]);
+        }
+        CU(cudaMalloc(&G.gsw, sizeof(double) * gsw.size()));
+        CU(cudaMalloc(&G.gsH6, sizeof(double) * H6.size()));
+        CU(cudaMemcpy(G.gsw, gsw.data(), sizeof(double) * gsw.size(), cudaMemcpyHostToDevice));
+        CU(cudaMemcpy(G.gsH6, H6.data(), sizeof(double) * H6.size(), cudaMemcpyHostToDevice));
+        G.onepass = false;
+        // theta: threads per CTA (64 .. 256) with the least idle columns in the last chunk; bands of rows so that
+        // all CTAs are resident at once (one full wave).  p: segments of 64 rows, many small CTAs
+        int best_bd = 128;
+        long best_cols = -1;
+        for (int bd = 256; bd >= 64; bd -= 32) {
+            const long cols = (long)cdiv(nt, vl::GS_TR * bd) * vl::GS_TR * bd;
+            if (best_cols < 0 || cols < best_cols) {
+                best_cols = cols;
+                best_bd = bd;
+            }
+        }
+        G.gs_tbd = best_bd;
+        int occ = 1;
+        if (G.prec == 32) CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, vl::gs_theta_sweep_kernel<float>, best_bd, 0));
+        else CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, vl::gs_theta_sweep_kernel<double>, best_bd, 0));
+        if (occ < 1) occ = 1;
+        const int nch = cdiv(nt, vl::GS_TR * best_bd);
+        int bands = (G.sm_count * occ) / nch;
+        if (bands < 1) bands = 1;
+        if (bands > max_bands_bound()) bands = max_bands_bound();
+        if (bands > np) bands = np;
+        G.gs_rpb = cdiv(np, bands);
+        G.gs_bands = cdiv(np, G.gs_rpb);
+        G.gs_pseg = 2 * vl::GS_PG * vl::GS_PR;
+        G.gs_pnseg = cdiv(np, G.gs_pseg);
+    }
     CU(cudaMalloc(&G.pkpart, sizeof(double) * 2 * (size_t)G.mbands * cdiv(nt, 256)));
     CU(cudaMalloc(&G.caspart, sizeof(double) * 4 * ((size_t)G.mbands * cdiv(nt, 256) + 1)));
     if (G.onepass) {
@@ -506,9 +556,36 @@ int launch_theta(bool want_colsums) {
     return VLASOV_OK;
 }
 
-int theta_bands(int nstage) { return G.theta_bulk ? G.bgrid[nstage].nbands : G.nbands[nstage]; }
+template <typename T>
+int launch_gs_theta(bool want_colsums) {
+    vl::GsThetaArgs<T> a;
+    a.fin = static_cast<const T*>(G.f[G.cur]);
+    a.fout = static_cast<T*>(G.f[G.cur ^ 1]);
+    a.srow = G.srow;
+    a.gsw = G.gsw;
+    a.colpart = want_colsums ? G.colpart : nullptr;
+    a.ntheta = G.ntheta;
+    a.np = G.np;
+    a.bc_x = G.bc_x;
+    a.rows_per_band = G.gs_rpb;
+    prof_begin(0);
+    vl::gs_theta_sweep_kernel<T><<<dim3(cdiv(G.ntheta, vl::GS_TR * G.gs_tbd), G.gs_bands), G.gs_tbd, 0, G.stream>>>(a);
+    prof_end(0);
+    LAUNCH_CHECK();
+    G.cur ^= 1;
+    return VLASOV_OK;
+}
+
+int theta_bands(int nstage) {
+    if (G.spline == 1) return G.gs_bands;
+    return G.theta_bulk ? G.bgrid[nstage].nbands : G.nbands[nstage];
+}
 
 int theta_pass(int nstage, bool want_colsums) {
+    if (G.spline == 1) {  // global spline: half shifts one at a time (the composite of two would have 119 taps)
+        if (nstage != 1) return fail(VLASOV_EINVAL, "SPLINE = 1 has no fused pair of half theta shifts");
+        return G.prec == 32 ? launch_gs_theta<float>(want_colsums) : launch_gs_theta<double>(want_colsums);
+    }
     if (G.prec == 32)
         return nstage == 2 ? launch_theta<float, 2>(want_colsums) : launch_theta<float, 1>(want_colsums);
     return nstage == 2 ? launch_theta<double, 2>(want_colsums) : launch_theta<double, 1>(want_colsums);
@@ -535,7 +612,31 @@ int launch_p() {
     return VLASOV_OK;
 }
 
-int p_pass() { return G.prec == 32 ? launch_p<float>() : launch_p<double>(); }
+template <typename T>
+int launch_gs_p() {
+    vl::GsPArgs<T> a;
+    a.fin = static_cast<const T*>(G.f[G.cur]);
+    a.fout = static_cast<T*>(G.f[G.cur ^ 1]);
+    a.force = G.force;
+    a.H6 = G.gsH6;
+    a.ntheta = G.ntheta;
+    a.np = G.np;
+    a.bc_p = G.bc_p;
+    a.seg_len = G.gs_pseg;
+    a.dt = G.dt;
+    a.dp = (G.pmax - G.pmin) / (double)G.np;
+    prof_begin(2);
+    vl::gs_p_sweep_kernel<T><<<dim3(cdiv(G.ntheta, vl::GS_PTX), G.gs_pnseg), vl::GS_PTX * vl::GS_PG, 0, G.stream>>>(a);
+    prof_end(2);
+    LAUNCH_CHECK();
+    G.cur ^= 1;
+    return VLASOV_OK;
+}
+
+int p_pass() {
+    if (G.spline == 1) return G.prec == 32 ? launch_gs_p<float>() : launch_gs_p<double>();
+    return G.prec == 32 ? launch_p<float>() : launch_p<double>();
+}
 
 // one pass: momentum shift with the stored force, then NST theta half shifts, then (optionally) the density
 // partials of the result in colpart_f (eqs (11), (12), (9), (10))
@@ -766,6 +867,10 @@ int vlasov_set_param(int key, double value) {
             G.bc_p = (int)value;
             break;
         case VLASOV_KEY_HISTORY: G.history = (value != 0.0); break;
+        case VLASOV_KEY_SPLINE:
+            if (value != 0.0 && value != 1.0) return fail(VLASOV_EINVAL, "SPLINE must be 0 (eq 16) or 1 (system 15)");
+            G.spline = (int)value;
+            break;
         case VLASOV_KEY_FUSE:
             if (value != 0.0 && value != 1.0 && value != 2.0) return fail(VLASOV_EINVAL, "FUSE must be 0, 1 or 2");
             G.fuse = (int)value;
@@ -879,7 +984,7 @@ int vlasov_step(int n) {
             ++k;
         }
         G.t += (double)n * G.dt;
-    } else if (G.fuse >= 1 && !G.history) {
+    } else if (G.fuse >= 1 && !G.history && G.spline == 0) {
         if ((rc = theta_pass(1, true)) != 0) return rc;                       // eq (9)
         for (int k = 0; k < n; ++k) {
             prof_begin(3);
@@ -919,7 +1024,12 @@ int vlasov_substep(int which) {
     if ((rc = ensure_buffers()) != 0) return rc;
     switch (which) {
         case VLASOV_SUB_THETA_HALF: return theta_pass(1, true);
-        case VLASOV_SUB_THETA_TWICE: return theta_pass(2, true);
+        case VLASOV_SUB_THETA_TWICE:
+            if (G.spline == 1) {  // two half shifts, two passes
+                if ((rc = theta_pass(1, false)) != 0) return rc;
+                return theta_pass(1, true);
+            }
+            return theta_pass(2, true);
         case VLASOV_SUB_FORCE:
             if ((rc = moments_pass()) != 0) return rc;
             return rho_and_force(G.mbands, nullptr, false);

@@ -475,7 +475,11 @@ int prepare() {
         // all CTAs are resident at once (one full wave).  p: segments of 64 rows, many small CTAs
         int best_bd = 128;
         long best_cols = -1;
-        for (int bd = 256; bd >= 64; bd -= 32) {
+#ifndef VL_GS_TBD_LO
+#define VL_GS_TBD_LO 64
+#define VL_GS_TBD_HI 128
+#endif
+        for (int bd = VL_GS_TBD_HI; bd >= VL_GS_TBD_LO; bd -= 32) {
             const long cols = (long)cdiv(nt, vl::GS_TR * bd) * vl::GS_TR * bd;
             if (best_cols < 0 || cols < best_cols) {
                 best_cols = cols;
@@ -494,7 +498,9 @@ int prepare() {
         if (bands > np) bands = np;
         G.gs_rpb = cdiv(np, bands);
         G.gs_bands = cdiv(np, G.gs_rpb);
-        G.gs_pseg = 2 * vl::GS_PG * vl::GS_PR;
+        G.gs_pseg = vl::GS_PSEG;
+        CU(cudaFuncSetAttribute(vl::gs_p_sweep_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)vl::gs_p_smem<float>()));
+        CU(cudaFuncSetAttribute(vl::gs_p_sweep_kernel<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)vl::gs_p_smem<double>()));
         G.gs_pnseg = cdiv(np, G.gs_pseg);
     }
     CU(cudaMalloc(&G.pkpart, sizeof(double) * 2 * (size_t)G.mbands * cdiv(nt, 256)));
@@ -622,11 +628,10 @@ int launch_gs_p() {
     a.ntheta = G.ntheta;
     a.np = G.np;
     a.bc_p = G.bc_p;
-    a.seg_len = G.gs_pseg;
     a.dt = G.dt;
     a.dp = (G.pmax - G.pmin) / (double)G.np;
     prof_begin(2);
-    vl::gs_p_sweep_kernel<T><<<dim3(cdiv(G.ntheta, vl::GS_PTX), G.gs_pnseg), vl::GS_PTX * vl::GS_PG, 0, G.stream>>>(a);
+    vl::gs_p_sweep_kernel<T><<<dim3(cdiv(G.ntheta, vl::GS_PTX), G.gs_pnseg), vl::GS_PTX * vl::GS_PG, vl::gs_p_smem<T>(), G.stream>>>(a);
     prof_end(2);
     LAUNCH_CHECK();
     G.cur ^= 1;

@@ -24,6 +24,7 @@
 //       column (they depend on the force there, eq (11)) sit in shared memory [tap][column] and serve 4 row groups.
 // Arithmetic is fp64 for both storage precisions.
 #pragma once
+#include "vlasov_fused.cuh"  // ptx::cp_async
 #include "vlasov_kernels.cuh"
 
 namespace vl {
@@ -48,11 +49,13 @@ __host__ __device__ inline void gs_H_over_6(double* H) {
 }
 
 // the GS_NT weights of a shift with fraction a from the table H/6 (host: rows; device: columns)
-__host__ __device__ inline void gs_weights(double a, const double* H6, double* w, int stride = 1) {
+// taps n = n0, n0 + nstep, ..
+__host__ __device__ inline void gs_weights(double a, const double* H6, double* w, int stride = 1, int n0 = 0,
+                                           int nstep = 1) {
     const double al = 1.0 - a;
     const double A = al * (al * al - 1.0);
     const double B = a * (a * a - 1.0);
-    for (int n = 0; n < GS_NT; ++n) {
+    for (int n = n0; n < GS_NT; n += nstep) {
         const int m = n - GS_M0;  // -(Q+1) .. Q+2
         double v = 0.0;
         if (m <= GS_Q + 1) v += A * H6[m + GS_Q + 1];
@@ -68,6 +71,9 @@ __host__ __device__ inline void gs_weights(double a, const double* H6, double* w
 // ------------------------------------------------------------------------------------------------
 constexpr int GS_TR = 9;                       // consecutive outputs per thread (odd: conflict-free lane stride)
 constexpr int GS_TMAXT = 256;                  // most threads per CTA (the host picks 64 .. 256 by the row length)
+#ifndef VL_GS_TMINB
+#define VL_GS_TMINB 3  // <= 85 registers: 8 CTAs of 96 threads per SM (sweep in profiles/README.md)
+#endif
 constexpr int GS_TKPRE = GS_TR + 1;            // window values a thread prefetches: ceil((9 bd + 59) / bd), bd >= 64
 
 template <typename T>
@@ -82,7 +88,7 @@ struct GsThetaArgs {
 
 // Arithmetic is fp64 whatever the storage type T (60 taps in fp32 would not keep 1e-4 over 100 steps).
 template <typename T>
-__global__ void __launch_bounds__(GS_TMAXT) gs_theta_sweep_kernel(const GsThetaArgs<T> arg) {
+__global__ void __launch_bounds__(GS_TMAXT, VL_GS_TMINB) gs_theta_sweep_kernel(const GsThetaArgs<T> arg) {
     __shared__ double xs[GS_TR * GS_TMAXT + GS_NT];
     __shared__ double ws[GS_NT];
     const int tid = threadIdx.x, bd = blockDim.x;
@@ -169,10 +175,37 @@ __global__ void __launch_bounds__(GS_TMAXT) gs_theta_sweep_kernel(const GsThetaA
 
 // ------------------------------------------------------------------------------------------------
 // momentum shift, eq (11) with the global spline
+//
+// A CTA owns GS_PTX adjacent columns and a segment of GS_PSEG rows.  The source rows of the segment go through a
+// shared-memory tile ONCE: tile[k][c] = f[jA + s_c - 29 + k][i0 + c], k < GS_PSEG + 59, each column at its own
+// integer shift s_c, so that inside the tile every column's window starts at the same k.  (Re-reading the window
+// from global memory through L1 does not work: rows are a power-of-two stride apart and evict each other.)
+// Thread (column c, row group g) produces GS_PR consecutive rows at a time from a sliding register window.
 // ------------------------------------------------------------------------------------------------
-constexpr int GS_PTX = 64;  // columns per CTA
-constexpr int GS_PG = 4;    // row groups per CTA: thread (column c, group g) takes the row blocks g, g + GS_PG, ..
-constexpr int GS_PR = 8;    // consecutive output rows per thread and block
+#ifndef VL_GS_PG
+#define VL_GS_PG 4
+#endif
+#ifndef VL_GS_PR
+#define VL_GS_PR 16
+#endif
+#ifndef VL_GS_PSEGMUL
+#define VL_GS_PSEGMUL 4
+#endif
+#ifndef VL_GS_PMINB
+#define VL_GS_PMINB 2
+#endif
+#ifndef VL_GS_PTX
+#define VL_GS_PTX 32
+#endif
+constexpr int GS_PTX = VL_GS_PTX;   // columns per CTA
+constexpr int GS_PG = VL_GS_PG;     // row groups per CTA
+constexpr int GS_PR = VL_GS_PR;     // consecutive output rows per thread and block
+constexpr int GS_PSEG = VL_GS_PSEGMUL * GS_PG * GS_PR;  // rows per CTA
+constexpr int GS_PROWS = GS_PSEG + GS_NT - 1;           // rows of the tile
+template <typename T>
+constexpr size_t gs_p_smem() {
+    return sizeof(double) * ((size_t)GS_NT * GS_PTX + 2 * GS_Q + 4) + sizeof(T) * (size_t)GS_PROWS * GS_PTX;
+}
 
 template <typename T>
 struct GsPArgs {
@@ -180,67 +213,75 @@ struct GsPArgs {
     T* fout;
     const double* force;  // [Ntheta]
     const double* H6;     // [2 GS_Q + 3]
-    int ntheta, np, bc_p, seg_len;  // seg_len: rows per CTA, a multiple of GS_PR
+    int ntheta, np, bc_p;
     double dt, dp;
 };
 
 template <typename T>
-__global__ void __launch_bounds__(GS_PTX * GS_PG) gs_p_sweep_kernel(const GsPArgs<T> arg) {
-    __shared__ double wsm[GS_NT * GS_PTX];  // [tap][column]
-    __shared__ double H6s[2 * GS_Q + 3];
-    __shared__ int ssm[GS_PTX];
+__global__ void __launch_bounds__(GS_PTX * GS_PG, VL_GS_PMINB) gs_p_sweep_kernel(const GsPArgs<T> arg) {
+    extern __shared__ __align__(16) unsigned char gs_smem[];
+    double* wsm = reinterpret_cast<double*>(gs_smem);       // [GS_NT][GS_PTX]
+    double* H6s = wsm + (size_t)GS_NT * GS_PTX;             // [2 GS_Q + 3] (+ 1 pad)
+    T* tile = reinterpret_cast<T*>(H6s + 2 * GS_Q + 4);     // [GS_PROWS][GS_PTX], storage type
     const int tid = threadIdx.x, c = tid % GS_PTX, g = tid / GS_PTX;
     const int ntheta = arg.ntheta, np = arg.np;
     const int i = blockIdx.x * GS_PTX + c;
     const bool act = i < ntheta;
     const bool periodic = (arg.bc_p == BC_PERIODIC);
     if (tid < 2 * GS_Q + 3) H6s[tid] = arg.H6[tid];
-    __syncthreads();
+    const int jA = blockIdx.y * GS_PSEG;
+    const int jB = min(np, jA + GS_PSEG);
+    const size_t pitch = (size_t)ntheta;
 
-    if (g == 0) {
-        // eta = F dt / dp cells; the foot of row j is row j + s + a
-        double sf, a;
-        split_shift(-((act ? arg.force[i] : 0.0) * arg.dt) / arg.dp, &sf, &a);
-        int s;
-        if (periodic) {
-            sf = fmod(sf, (double)np);
-            s = (int)sf;
-        } else {
-            const double lim = (double)np + 64.0;
-            s = (int)fmin(fmax(sf, -lim), lim);
-        }
-        ssm[c] = s;
-        gs_weights(a, H6s, wsm + c, GS_PTX);
+    // integer shift and fraction of the column: eta = F dt / dp cells; the foot of row j is row j + s + a
+    double sf, a;
+    split_shift(-((act ? arg.force[i] : 0.0) * arg.dt) / arg.dp, &sf, &a);
+    int s;
+    if (periodic) {
+        sf = fmod(sf, (double)np);
+        s = (int)sf;
+    } else {
+        const double lim = (double)np + 64.0;
+        s = (int)fmin(fmax(sf, -lim), lim);
     }
+
+    // the tile: rows jA + s - 29 + k of this thread's column, k = g, g + GS_PG, ..; all copies in flight at once
+    {
+        const T* __restrict__ col = arg.fin + (act ? i : 0);
+        const int nrows = (jB - jA) + GS_NT - 1;
+        int y = jA + s - GS_M0 + g;
+        if (periodic) y = wrap_index(y, np);
+        uint32_t dst = ptx::smem_u32(tile + g * GS_PTX + c);
+        for (int k = g; k < nrows; k += GS_PG) {
+            const bool ok = act && (periodic || (unsigned)y < (unsigned)np);
+            const T* src = ok ? col + (size_t)y * pitch : arg.fin;
+            ptx::cp_async_zfill<(int)sizeof(T)>(dst, src, ok ? (unsigned)sizeof(T) : 0u);
+            dst += (uint32_t)(GS_PG * GS_PTX * sizeof(T));
+            y += GS_PG;
+            if (periodic && y >= np) y -= np;
+        }
+        ptx::cp_async_commit();
+    }
+    __syncthreads();  // H6s
+    gs_weights(a, H6s, wsm + c, GS_PTX, g, GS_PG);  // while the copies fly: group g takes the taps g, g + GS_PG, ..
+    ptx::cp_async_wait<0>();
     __syncthreads();
     if (!act) return;
-    const int s = ssm[c];
 
-    const T* __restrict__ col = arg.fin + i;
     T* __restrict__ ocol = arg.fout + i;
-    const size_t pitch = (size_t)ntheta;
-    const int jA = blockIdx.y * arg.seg_len;
-    const int jB = min(np, jA + arg.seg_len);
-
+    const double* __restrict__ wc = wsm + c;
     for (int jb = jA + g * GS_PR; jb < jB; jb += GS_PG * GS_PR) {
-        const int y0 = jb + s - GS_M0;  // source row of window element 0
-        auto load = [&](int k) -> double {
-            int y = y0 + k;
-            if (periodic) {
-                y = wrap_index(y, np);
-                return (double)__ldg(col + (size_t)y * pitch);
-            }
-            return ((unsigned)y < (unsigned)np) ? (double)__ldg(col + (size_t)y * pitch) : 0.0;
-        };
+        const T* __restrict__ tc = tile + (size_t)(jb - jA) * GS_PTX + c;
         double x[GS_PR], out[GS_PR];
 #pragma unroll
-        for (int r = 0; r < GS_PR - 1; ++r) x[r] = load(r);
+        for (int r = 0; r < GS_PR - 1; ++r) x[r] = (double)tc[r * GS_PTX];
 #pragma unroll
         for (int r = 0; r < GS_PR; ++r) out[r] = 0.0;
 #pragma unroll
         for (int n = 0; n < GS_NT; ++n) {
-            x[(n + GS_PR - 1) % GS_PR] = load(n + GS_PR - 1);
-            const double w = wsm[n * GS_PTX + c];
+            // rows past the end of a short last block read stale tile rows: their outputs are not stored
+            x[(n + GS_PR - 1) % GS_PR] = (double)tc[(n + GS_PR - 1) * GS_PTX];
+            const double w = wc[n * GS_PTX];
 #pragma unroll
             for (int r = 0; r < GS_PR; ++r) out[r] = fma(w, x[(n + r) % GS_PR], out[r]);
         }

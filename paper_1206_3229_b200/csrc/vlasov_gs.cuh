@@ -176,23 +176,23 @@ __global__ void __launch_bounds__(GS_TMAXT, VL_GS_TMINB) gs_theta_sweep_kernel(c
 // ------------------------------------------------------------------------------------------------
 // momentum shift, eq (11) with the global spline
 //
-// A CTA owns GS_PTX adjacent columns and a segment of GS_PSEG rows.  The source rows of the segment go through a
-// shared-memory tile ONCE: tile[k][c] = f[jA + s_c - 29 + k][i0 + c], k < GS_PSEG + 59, each column at its own
+// A CTA owns GS_PTX = 32 adjacent columns and a segment of GS_PSEG = 256 rows.  The source rows of the segment go
+// through a shared-memory tile ONCE (per-thread cp.async, one commit group per chunk of 128 output rows): tile[k][c] = f[jA + s_c - 29 + k][i0 + c], k < GS_PSEG + 59, each column at its own
 // integer shift s_c, so that inside the tile every column's window starts at the same k.  (Re-reading the window
 // from global memory through L1 does not work: rows are a power-of-two stride apart and evict each other.)
 // Thread (column c, row group g) produces GS_PR consecutive rows at a time from a sliding register window.
 // ------------------------------------------------------------------------------------------------
 #ifndef VL_GS_PG
-#define VL_GS_PG 4
+#define VL_GS_PG 8
 #endif
 #ifndef VL_GS_PR
 #define VL_GS_PR 16
 #endif
 #ifndef VL_GS_PSEGMUL
-#define VL_GS_PSEGMUL 4
+#define VL_GS_PSEGMUL 2
 #endif
 #ifndef VL_GS_PMINB
-#define VL_GS_PMINB 2
+#define VL_GS_PMINB 1
 #endif
 #ifndef VL_GS_PTX
 #define VL_GS_PTX 32
@@ -245,32 +245,52 @@ __global__ void __launch_bounds__(GS_PTX * GS_PG, VL_GS_PMINB) gs_p_sweep_kernel
         s = (int)fmin(fmax(sf, -lim), lim);
     }
 
-    // the tile: rows jA + s - 29 + k of this thread's column, k = g, g + GS_PG, ..; all copies in flight at once
+    // the tile: rows jA + s - 29 + k of this thread's column, k = g, g + GS_PG, ..  All copies are issued at once, in
+    // one commit group per chunk of GS_PG * GS_PR output rows (chunk 0 also carries the 59 halo rows), so that the
+    // first chunk can be computed while the others are still in flight.
+    constexpr int CH = GS_PG * GS_PR, NCH = VL_GS_PSEGMUL;
     {
         const T* __restrict__ col = arg.fin + (act ? i : 0);
         const int nrows = (jB - jA) + GS_NT - 1;
         int y = jA + s - GS_M0 + g;
         if (periodic) y = wrap_index(y, np);
         uint32_t dst = ptx::smem_u32(tile + g * GS_PTX + c);
-        for (int k = g; k < nrows; k += GS_PG) {
-            const bool ok = act && (periodic || (unsigned)y < (unsigned)np);
-            const T* src = ok ? col + (size_t)y * pitch : arg.fin;
-            ptx::cp_async_zfill<(int)sizeof(T)>(dst, src, ok ? (unsigned)sizeof(T) : 0u);
-            dst += (uint32_t)(GS_PG * GS_PTX * sizeof(T));
-            y += GS_PG;
-            if (periodic && y >= np) y -= np;
+        int k = g;
+#pragma unroll
+        for (int m = 0; m < NCH; ++m) {
+            const int hi = min(nrows, (m + 1) * CH + GS_NT - 1);
+            for (; k < hi; k += GS_PG) {
+                const bool ok = act && (periodic || (unsigned)y < (unsigned)np);
+                const T* src = ok ? col + (size_t)y * pitch : arg.fin;
+                ptx::cp_async_zfill<(int)sizeof(T)>(dst, src, ok ? (unsigned)sizeof(T) : 0u);
+                dst += (uint32_t)(GS_PG * GS_PTX * sizeof(T));
+                y += GS_PG;
+                if (periodic && y >= np) y -= np;
+            }
+            ptx::cp_async_commit();
         }
-        ptx::cp_async_commit();
     }
     __syncthreads();  // H6s
     gs_weights(a, H6s, wsm + c, GS_PTX, g, GS_PG);  // while the copies fly: group g takes the taps g, g + GS_PG, ..
-    ptx::cp_async_wait<0>();
-    __syncthreads();
-    if (!act) return;
 
-    T* __restrict__ ocol = arg.fout + i;
+    T* __restrict__ ocol = arg.fout + (act ? i : 0);
     const double* __restrict__ wc = wsm + c;
-    for (int jb = jA + g * GS_PR; jb < jB; jb += GS_PG * GS_PR) {
+#pragma unroll 1
+    for (int m = 0; m < NCH; ++m) {
+        const int jb = jA + m * CH + g * GS_PR;
+        // this thread's copies of chunks 0..m have landed; after the barrier everybody's have (and the weights)
+        switch (NCH - 1 - m) {
+            case 0: ptx::cp_async_wait<0>(); break;
+            case 1: ptx::cp_async_wait<1>(); break;
+            case 2: ptx::cp_async_wait<2>(); break;
+            case 3: ptx::cp_async_wait<3>(); break;
+            case 4: ptx::cp_async_wait<4>(); break;
+            case 5: ptx::cp_async_wait<5>(); break;
+            case 6: ptx::cp_async_wait<6>(); break;
+            default: ptx::cp_async_wait<7>(); break;
+        }
+        __syncthreads();
+        if (!act || jb >= jB) continue;
         const T* __restrict__ tc = tile + (size_t)(jb - jA) * GS_PTX + c;
         double x[GS_PR], out[GS_PR];
 #pragma unroll

@@ -272,7 +272,7 @@ def run_cuda(args):
             flops = 2.0 * 60.0 * pts
             ach_tf = flops / (kern[dom]["avg_ms"] * 1e-3) / 1e12
             roofline = {"bound": "alu", "kernel": gs_names.get(dom, dom), "achieved": ach_tf, "peak": 34.0,
-                        "unit": "TFLOP/s", "frac": ach_tf / 34.0, "traffic": None,
+                        "unit": "TFLOP/s", "frac": ach_tf / 34.0, "traffic": committed_traffic("gs_" + dom, n, prec),
                         "peak_source": "measured fp64 FMA rate, profiles/fp64_probe.txt (17.0 TFMA/s)",
                         "algorithmic_flops_per_launch": flops, "hbm_gbs": ach, "hbm_frac": ach / peak}
 

@@ -589,7 +589,10 @@ int theta_bands(int nstage) {
 
 int theta_pass(int nstage, bool want_colsums) {
     if (G.spline == 1) {  // global spline: half shifts one at a time (the composite of two would have 119 taps)
-        if (nstage != 1) return fail(VLASOV_EINVAL, "SPLINE = 1 has no fused pair of half theta shifts");
+        if (nstage == 2) {
+            int rc = G.prec == 32 ? launch_gs_theta<float>(false) : launch_gs_theta<double>(false);
+            if (rc != 0) return rc;
+        }
         return G.prec == 32 ? launch_gs_theta<float>(want_colsums) : launch_gs_theta<double>(want_colsums);
     }
     if (G.prec == 32)
@@ -1029,12 +1032,7 @@ int vlasov_substep(int which) {
     if ((rc = ensure_buffers()) != 0) return rc;
     switch (which) {
         case VLASOV_SUB_THETA_HALF: return theta_pass(1, true);
-        case VLASOV_SUB_THETA_TWICE:
-            if (G.spline == 1) {  // two half shifts, two passes
-                if ((rc = theta_pass(1, false)) != 0) return rc;
-                return theta_pass(1, true);
-            }
-            return theta_pass(2, true);
+        case VLASOV_SUB_THETA_TWICE: return theta_pass(2, true);
         case VLASOV_SUB_FORCE:
             if ((rc = moments_pass()) != 0) return rc;
             return rho_and_force(G.mbands, nullptr, false);

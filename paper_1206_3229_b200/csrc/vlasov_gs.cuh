@@ -69,7 +69,10 @@ __host__ __device__ inline void gs_weights(double a, const double* H6, double* w
 // ------------------------------------------------------------------------------------------------
 // theta shift, eq (9) / (12) with the global spline
 // ------------------------------------------------------------------------------------------------
-constexpr int GS_TR = 9;                       // consecutive outputs per thread (odd: conflict-free lane stride)
+#ifndef VL_GS_TR
+#define VL_GS_TR 9
+#endif
+constexpr int GS_TR = VL_GS_TR;                // consecutive outputs per thread (odd: conflict-free lane stride)
 constexpr int GS_TMAXT = 256;                  // most threads per CTA (the host picks 64 .. 256 by the row length)
 #ifndef VL_GS_TMINB
 #define VL_GS_TMINB 3  // <= 85 registers: 8 CTAs of 96 threads per SM (sweep in profiles/README.md)

@@ -74,6 +74,25 @@ def test_gs_p_sweep_with_given_force(grid, bc_p, amp):
     g.close()
 
 
+@pytest.mark.parametrize("which,nhalf", [(vb.SUB_THETA_TWICE, 2), (vb.SUB_P_THETA_HALF, 1), (vb.SUB_P_THETA_TWICE, 2)])
+def test_gs_composite_substeps(which, nhalf):
+    """the composite test hooks run as separate passes with the global spline and leave density and force behind"""
+    c = inputs.config("cfg1", ntheta=300, npts=200)
+    o, g = pair(c["model"], c["grid"], c["domain"], c["dt"], c["f0"])
+    th = inputs.nodes(c["domain"][0], c["domain"][1], 300)
+    F = 0.7 * np.sin(th + 0.2)
+    if which != vb.SUB_THETA_TWICE:
+        o.p_sweep(c["dt"], force=F)
+        g.set_force(F)
+    for _ in range(nhalf):
+        o.theta_sweep(0.5 * c["dt"])
+    g.substep(which)
+    assert rel_err(g.download(), o.download()) < 1e-13
+    if which != vb.SUB_THETA_TWICE:
+        assert np.max(np.abs(g.force() - o.force())) <= 1e-12 * np.max(np.abs(o.force()))
+    g.close()
+
+
 def test_gs_integer_cell_shifts_are_exact_copies():
     """a = 0: w = (.., 0, 1, 0, ..) exactly, so the shifted line is a bit-exact copy (P2 holds for any f'')."""
     nt, npp = 128, 64

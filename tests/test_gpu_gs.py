@@ -182,3 +182,39 @@ def test_gs_at_2048_first_steps_then_22_steps():
     assert rel_err(g.download(), o.download()) <= 1e-11
     assert np.max(np.abs(g.moments() - o.moments())) <= 1e-11
     g.close()
+
+
+# ----------------------------------------------------------------------------- full sizes of BASELINE.json's configs
+def run_both_gs(c, steps):
+    import os
+
+    o = Oracle(c["model"], c["grid"], c["domain"], c["dt"], threads=os.cpu_count() or 8, spline=SPLINE_GS, **c["params"])
+    o.upload(c["f0"])
+    o.step(steps)
+    fo, mo = o.download(), o.moments()
+    o.close()
+    g = vb.Vlasov(c["model"], c["grid"], c["domain"], c["dt"], spline=vb.SPLINE_GS, **c["params"])
+    g.upload(c["f0"])
+    g.step(steps)
+    fg, mg = g.download(), g.moments()
+    g.close()
+    return fo, mo, fg, mg
+
+
+@pytest.mark.parametrize("name,kw,steps", [("cfg2", {}, 100), ("cfg3", {}, 100), ("cfg4", {}, 100),
+                                           ("cfg5", dict(n=4096), 40)])
+def test_gs_full_size_steps_match_oracle(name, kw, steps):
+    """cfg 2 (1024^2), cfg 3 (ring, 2048^2), cfg 4 (sheet, 4096^2, zero-extended x) for 100 steps and cfg 5 at 4096^2
+    for 40, global spline on both sides, element by element (north_star: 1e-10 max|f|, moments 1e-10)."""
+    c = inputs.config(name, **kw)
+    fo, mo, fg, mg = run_both_gs(c, steps)
+    assert rel_err(fg, fo) <= 1e-10
+    assert np.max(np.abs(mg - mo)) <= 1e-10 * max(1.0, np.max(np.abs(mo)))
+
+
+def test_gs_bench_size_first_steps_match_oracle():
+    """8192^2 in the configuration bench.py --spline gs times: two steps element by element"""
+    c = inputs.config("cfg5", n=8192)
+    fo, mo, fg, mg = run_both_gs(c, 2)
+    assert rel_err(fg, fo) <= 1e-12
+    assert np.max(np.abs(mg - mo)) <= 1e-11

@@ -19,6 +19,10 @@ theta half shift).  Prints ONE JSON line (rank 0).
              point of the two-pass minimum north_star names
   cpu_baseline  the CPU oracle (oracle/, as it stands) timed on this box's host cores on a bounded sample
 
+--spline gs times the Global Spline variant instead (system (15), the paper's comparator): three
+60-tap passes per step, roofline.bound = "alu" against the measured fp64 FMA rate; the oracle legs then run with
+KEY_SPLINE = GS too.  The default (fd) is the paper's method and the headline workload.
+
 --impl reference times the oracle (there is no other reference implementation: the paper ships no code).
 N > 1: independent replicas (the path does not shard in this build): one process per
 GPU, no data-path collective, value = all replicas' grid points / max time.

@@ -204,7 +204,7 @@ def run_cuda(args):
     f0 = c["f0"].astype(np.float64 if prec == 64 else np.float32)
     g = vb.Vlasov(c["model"], c["grid"], c["domain"], c["dt"], precision=prec, device="cuda:%d" % local_rank,
                   fuse=args.fuse, tune_fvariant=args.fvariant, tune_graph=args.graph,
-                  **({"spline": vb.SPLINE_GS} if args.spline == "gs" else {}),
+                  **({"spline": vb.SPLINE_GS, "tune_gsfir": args.gsfir} if args.spline == "gs" else {}),
                   **({"tune_fbands": args.fbands} if args.fbands > 0 else {}))
     g.upload(f0)
     pts = float(n) * float(n)
@@ -358,6 +358,8 @@ def main():
     ap.add_argument("--spline", default="fd", choices=["fd", "gs"],
                     help="fd: f'' by eq (16), the paper's method and the headline workload; gs: the Global Spline "
                          "comparator, system (15) (SURVEY 8(f) NEXT #2; three 60-tap passes per step, fp64-ALU bound)")
+    ap.add_argument("--gsfir", type=int, default=0, choices=[0, 1],
+                    help="with --spline gs: 1 = the 60-tap filter kernels instead of the recursive ones (A/B partner)")
     ap.add_argument("--fvariant", type=int, default=0, choices=[0, 1],
                     help="one-pass kernel: 0 = warp-specialised (default), 1 = every warp does both stages")
     args = ap.parse_args()

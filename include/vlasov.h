@@ -62,7 +62,7 @@ extern "C" {
                                   tridiagonal system (15), L100-L102 (the paper's comparator "GS", Tables 1-2;
                                   diagonal 2/3, D22).  Three passes per step, 60 taps per shift instead
                                   of 10; both axes need >= 32 nodes                                             */
-/* keys 101..108 (launch-shape overrides: warps, bands, segment lengths, kernel variant) exist for the tests and
+/* keys 101..110 (launch-shape overrides: warps, bands, segment lengths, kernel variant) exist for the tests and
  * the tuning sweeps only; see binding.py KEY_TUNE_*.  Results never depend on them beyond rounding order.   */
 
 /* sub-steps for vlasov_substep (parity tests of single stages; same kernels as vlasov_step) */

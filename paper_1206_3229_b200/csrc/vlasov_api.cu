@@ -31,7 +31,7 @@ constexpr int FU_R = 11;         // consecutive outputs per lane in its theta st
 constexpr int FU_NSTG = 3;       // cp.async ring depth (phases of 12 rows)
 constexpr int FU_NW = FU_NT / 32;  // density partial rows per band of the one-pass kernel, variant 1 (all warps alike)
 constexpr int FW_NSTG = 3;       // ring depth (groups of 12 rows) of the warp-specialised one-pass kernel (variant 0)
-constexpr int KEY_TUNE_FVARIANT = 108, KEY_TUNE_GRAPH = 109;
+constexpr int KEY_TUNE_FVARIANT = 108, KEY_TUNE_GRAPH = 109, KEY_TUNE_GSFIR = 110;
 constexpr int FU_PAD = 12;       // rows of padding of the theta weight tables (the last phase of a band reads on)
 constexpr int NCLS = 6;          // profiled kernel classes: theta x1, theta x2, p, rho+force, p+theta x2, p+theta x1
 constexpr int KEY_TUNE_FBANDS = 107;
@@ -46,7 +46,9 @@ struct Ctx {
     double xmin = 0, xmax = 0, pmin = 0, pmax = 0, dt = 0, eps = 0.01, t = 0;
     int bc_x = 0, bc_p = 1, prec = 64;
     int spline = 0;  // 0: f'' by eq (16) (the paper's method), 1: global spline, system (15) (vlasov_gs.cuh)
-    double *gsw = nullptr, *gsH6 = nullptr;  // [Np][GS_NT] row weights of a half theta shift; H/6 table
+    double *gsw = nullptr, *gsH6 = nullptr, *gsab = nullptr;  // gsab: [Np][4] = 1-a, a, A/6, B/6 of a half theta shift
+    int gs_fir = 0;                  // KEY_TUNE_GSFIR: 1 = the 60-tap filter kernels instead of the recursive ones
+    int gs_rbands = 0, gs_rrpb = 0;  // bands of the recursive theta kernel  // [Np][GS_NT] row weights of a half theta shift; H/6 table
     int gs_bands = 0, gs_rpb = 0, gs_pseg = 0, gs_pnseg = 0, gs_tbd = 128;
     bool history = false;
     int fuse = 2;  // 0: p and theta passes apart, 1: adjacent half theta shifts in one pass, 2: p + theta in one pass
@@ -160,14 +162,14 @@ int cdiv(int a, int b) { return (a + b - 1) / b; }
 void free_small() {
     void* ptrs[] = {G.srow, G.wrow, G.cos_t, G.sin_t, G.ringK, G.ringV, G.rho, G.force, G.rho_m,
                     G.phi,  G.mpart, G.pkpart, G.mom_dev, G.hist, G.wrow2, G.colpart_f, G.ticket, G.caspart, G.ringpart, G.ringtick,
-                    G.gsw, G.gsH6};
+                    G.gsw, G.gsH6, G.gsab};
     for (void* p : ptrs)
         if (p) cudaFree(p);
     G.srow = nullptr;
     G.wrow = G.cos_t = G.sin_t = G.ringK = G.ringV = G.rho = G.force = G.rho_m = G.phi = G.mpart = G.pkpart =
         G.mom_dev = G.hist = G.wrow2 = G.colpart_f = nullptr;
     G.ticket = nullptr;
-    G.gsw = G.gsH6 = nullptr;
+    G.gsw = G.gsH6 = G.gsab = nullptr;
     G.caspart = nullptr;
     G.ringpart = nullptr;
     G.ringtick = nullptr;
@@ -459,13 +461,20 @@ int prepare() {
             return fail(VLASOV_EINVAL, "SPLINE = 1 (global spline) needs at least 32 nodes on both axes");
         std::vector<double> H6(2 * vl::GS_Q + 3);
         vl::gs_H_over_6(H6.data());
-        std::vector<double> gsw((size_t)np * vl::GS_NT);
+        std::vector<double> gsw((size_t)np * vl::GS_NT), gsab((size_t)np * 4);
         for (int j = 0; j < np; ++j) {
             const double p = G.pmin + (double)j * dp;
             double sf, a;
             vl::split_shift(-(p * tau) / dx, &sf, &a);
             vl::gs_weights(a, H6.data(), &gsw[(size_t)j * vl::GS_NT]);
+            const double al = 1.0 - a;
+            gsab[(size_t)j * 4 + 0] = al;
+            gsab[(size_t)j * 4 + 1] = a;
+            gsab[(size_t)j * 4 + 2] = al * (al * al - 1.0) / 6.0;
+            gsab[(size_t)j * 4 + 3] = a * (a * a - 1.0) / 6.0;
         }
+        CU(cudaMalloc(&G.gsab, sizeof(double) * gsab.size()));
+        CU(cudaMemcpy(G.gsab, gsab.data(), sizeof(double) * gsab.size(), cudaMemcpyHostToDevice));
         CU(cudaMalloc(&G.gsw, sizeof(double) * gsw.size()));
         CU(cudaMalloc(&G.gsH6, sizeof(double) * H6.size()));
         CU(cudaMemcpy(G.gsw, gsw.data(), sizeof(double) * gsw.size(), cudaMemcpyHostToDevice));
@@ -498,6 +507,19 @@ int prepare() {
         if (bands > np) bands = np;
         G.gs_rpb = cdiv(np, bands);
         G.gs_bands = cdiv(np, G.gs_rpb);
+        {   // recursive theta kernel: 4 warps x 216 columns per CTA, bands for one resident wave
+            int occ2 = 1;
+            if (G.prec == 32) CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ2, vl::gs_theta_rec_kernel<float>, vl::GS_RWARPS * 32, 0));
+            else CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ2, vl::gs_theta_rec_kernel<double>, vl::GS_RWARPS * 32, 0));
+            if (occ2 < 1) occ2 = 1;
+            const int nchr = cdiv(cdiv(nt, vl::GS_ROUT), vl::GS_RWARPS);
+            int b2 = (G.sm_count * occ2) / nchr;
+            if (b2 < 1) b2 = 1;
+            if (b2 > max_bands_bound()) b2 = max_bands_bound();
+            if (b2 > np) b2 = np;
+            G.gs_rrpb = cdiv(np, b2);
+            G.gs_rbands = cdiv(np, G.gs_rrpb);
+        }
         G.gs_pseg = vl::GS_PSEG;
         CU(cudaFuncSetAttribute(vl::gs_p_sweep_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)vl::gs_p_smem<float>()));
         CU(cudaFuncSetAttribute(vl::gs_p_sweep_kernel<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)vl::gs_p_smem<double>()));
@@ -563,7 +585,28 @@ int launch_theta(bool want_colsums) {
 }
 
 template <typename T>
+int launch_gs_theta_rec(bool want_colsums) {
+    vl::GsThetaRecArgs<T> a;
+    a.fin = static_cast<const T*>(G.f[G.cur]);
+    a.fout = static_cast<T*>(G.f[G.cur ^ 1]);
+    a.srow = G.srow;
+    a.gsab = G.gsab;
+    a.colpart = want_colsums ? G.colpart : nullptr;
+    a.ntheta = G.ntheta;
+    a.np = G.np;
+    a.bc_x = G.bc_x;
+    a.rows_per_band = G.gs_rrpb;
+    prof_begin(0);
+    vl::gs_theta_rec_kernel<T><<<dim3(cdiv(cdiv(G.ntheta, vl::GS_ROUT), vl::GS_RWARPS), G.gs_rbands), vl::GS_RWARPS * 32, 0, G.stream>>>(a);
+    prof_end(0);
+    LAUNCH_CHECK();
+    G.cur ^= 1;
+    return VLASOV_OK;
+}
+
+template <typename T>
 int launch_gs_theta(bool want_colsums) {
+    if (!G.gs_fir) return launch_gs_theta_rec<T>(want_colsums);
     vl::GsThetaArgs<T> a;
     a.fin = static_cast<const T*>(G.f[G.cur]);
     a.fout = static_cast<T*>(G.f[G.cur ^ 1]);
@@ -583,7 +626,7 @@ int launch_gs_theta(bool want_colsums) {
 }
 
 int theta_bands(int nstage) {
-    if (G.spline == 1) return G.gs_bands;
+    if (G.spline == 1) return G.gs_fir ? G.gs_bands : G.gs_rbands;
     return G.theta_bulk ? G.bgrid[nstage].nbands : G.nbands[nstage];
 }
 
@@ -886,6 +929,7 @@ int vlasov_set_param(int key, double value) {
         case KEY_TUNE_FBANDS: G.tune_fbands = (int)value; break;
         case KEY_TUNE_FVARIANT: G.fvariant = (value == 1.0) ? 1 : 0; break;
         case KEY_TUNE_GRAPH: G.graphs = (value != 0.0); break;
+        case KEY_TUNE_GSFIR: G.gs_fir = (value != 0.0) ? 1 : 0; break;
         case VLASOV_KEY_PROFILE: G.profile = (value != 0.0); break;
         case KEY_TUNE_NW1: G.tune_nw1 = (int)value; break;
         case KEY_TUNE_NW2: G.tune_nw2 = (int)value; break;

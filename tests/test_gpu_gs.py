@@ -34,10 +34,21 @@ def rough_state(nt, npp, dom, seed=1):
     return f + 0.1 * rng.random((npp, nt))
 
 
+GSFIR = 0  # which GPU kernels: 0 = the recursive ones (default), 1 = the 60-tap filter kernels (tune_gsfir)
+
+
+@pytest.fixture(autouse=True, params=[0, 1], ids=["recursive", "fir"])
+def gs_kernel_variant(request):
+    global GSFIR
+    GSFIR = request.param
+    yield
+    GSFIR = 0
+
+
 def pair(model, grid, dom, dt, f0, threads=8, precision=64, **params):
     o = Oracle(model, grid, dom, dt, threads=threads, spline=SPLINE_GS, **params)
     o.upload(f0)
-    g = vb.Vlasov(model, grid, dom, dt, precision=precision, spline=vb.SPLINE_GS, **params)
+    g = vb.Vlasov(model, grid, dom, dt, precision=precision, spline=vb.SPLINE_GS, tune_gsfir=GSFIR, **params)
     g.upload(f0)
     return o, g
 
@@ -98,7 +109,7 @@ def test_gs_integer_cell_shifts_are_exact_copies():
     nt, npp = 128, 64
     dom = (0.0, float(nt), -4.0, 4.0)          # dx = 1; p_j tau integer for tau = 8: p_j = -4 + j/8
     f0 = rough_state(nt, npp, dom, seed=7)
-    g = vb.Vlasov(MODEL_FREE, (nt, npp), dom, 16.0, spline=vb.SPLINE_GS)
+    g = vb.Vlasov(MODEL_FREE, (nt, npp), dom, 16.0, spline=vb.SPLINE_GS, tune_gsfir=GSFIR)
     g.upload(f0)
     g.substep(vb.SUB_THETA_HALF)
     out = g.download()
@@ -140,7 +151,7 @@ def test_gs_differs_from_fd_and_history_matches():
     gf.step(10)
     f_fd = gf.download()
     gf.close()
-    g2 = vb.Vlasov(c["model"], c["grid"], c["domain"], c["dt"], spline=vb.SPLINE_GS, history=1)
+    g2 = vb.Vlasov(c["model"], c["grid"], c["domain"], c["dt"], spline=vb.SPLINE_GS, history=1, tune_gsfir=GSFIR)
     g2.upload(c["f0"])
     g2.step(10)
     hist = g2.history(10)
@@ -193,7 +204,7 @@ def run_both_gs(c, steps):
     o.step(steps)
     fo, mo = o.download(), o.moments()
     o.close()
-    g = vb.Vlasov(c["model"], c["grid"], c["domain"], c["dt"], spline=vb.SPLINE_GS, **c["params"])
+    g = vb.Vlasov(c["model"], c["grid"], c["domain"], c["dt"], spline=vb.SPLINE_GS, tune_gsfir=GSFIR, **c["params"])
     g.upload(c["f0"])
     g.step(steps)
     fg, mg = g.download(), g.moments()

@@ -520,6 +520,8 @@ int prepare() {
             G.gs_rrpb = cdiv(np, b2);
             G.gs_rbands = cdiv(np, G.gs_rrpb);
         }
+        CU(cudaFuncSetAttribute(vl::gs_p_rec_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)vl::gs_p_rec_smem<float>()));
+        CU(cudaFuncSetAttribute(vl::gs_p_rec_kernel<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)vl::gs_p_rec_smem<double>()));
         G.gs_pseg = vl::GS_PSEG;
         CU(cudaFuncSetAttribute(vl::gs_p_sweep_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)vl::gs_p_smem<float>()));
         CU(cudaFuncSetAttribute(vl::gs_p_sweep_kernel<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)vl::gs_p_smem<double>()));
@@ -677,6 +679,9 @@ int launch_gs_p() {
     a.dt = G.dt;
     a.dp = (G.pmax - G.pmin) / (double)G.np;
     prof_begin(2);
+    if (!G.gs_fir)
+        vl::gs_p_rec_kernel<T><<<dim3(cdiv(G.ntheta, vl::GS_PRX), cdiv(G.np, vl::GS_PRSEG)), vl::GS_PRX * vl::GS_PRG, vl::gs_p_rec_smem<T>(), G.stream>>>(a);
+    else
     vl::gs_p_sweep_kernel<T><<<dim3(cdiv(G.ntheta, vl::GS_PTX), G.gs_pnseg), vl::GS_PTX * vl::GS_PG, vl::gs_p_smem<T>(), G.stream>>>(a);
     prof_end(2);
     LAUNCH_CHECK();

@@ -186,8 +186,8 @@ __global__ void __launch_bounds__(GS_TMAXT, VL_GS_TMINB) gs_theta_sweep_kernel(c
 // the carries travel between lanes by shuffles: the true carry into a lane is C(l) = P0_8(l-1) + r^9 C(l-1), and
 // four rounds of shuffle resolve it to r^36 = 1e-21.  The first and last four lanes (36 nodes) are warm-up only:
 // lanes 4..27 produce the warp's 216 outputs.  About 17 fp64 operations per output instead of 60, 11 shared-memory
-// loads per lane and row instead of 98; no block-wide barrier: every warp has its own ring of four row windows in
-// shared memory, filled by per-lane cp.async three rows ahead (the pass is bound by bytes in flight, not by flops).
+// loads per lane and row instead of 98; no block-wide barrier: every warp has its own ring of three row windows in
+// shared memory, filled by per-lane cp.async two rows ahead (the pass is bound by bytes in flight, not by flops).
 // ------------------------------------------------------------------------------------------------
 constexpr int GS_RL = 9;                       // nodes per lane
 constexpr int GS_RWL = 4;                      // warm-up lanes on each side (4 * 9 = 36 nodes, r^36 = 1e-21)
@@ -207,10 +207,10 @@ struct GsThetaRecArgs {
 };
 
 #ifndef VL_GS_RSTG
-#define VL_GS_RSTG 4
+#define VL_GS_RSTG 3
 #endif
 #ifndef VL_GS_RMINB
-#define VL_GS_RMINB 4
+#define VL_GS_RMINB 5  // <= 102 registers: 20 warps per SM (sweep: 4 -> 0.337 ms, 5 -> 0.322)
 #endif
 constexpr int GS_RSTG = VL_GS_RSTG;            // rows in flight per warp (cp.async ring of windows)
 constexpr int GS_RWINP = GS_RWIN + 6;          // padded window: a multiple of 16 bytes for both storage types
@@ -478,6 +478,136 @@ __global__ void __launch_bounds__(GS_PTX * GS_PG, VL_GS_PMINB) gs_p_sweep_kernel
 #pragma unroll
         for (int r = 0; r < GS_PR; ++r)
             if (jb + r < jB) ocol[(size_t)(jb + r) * pitch] = (T)out[r];
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// momentum shift with the global spline, RECURSIVE form (default): same tile as gs_p_sweep_kernel (each column at
+// its own integer shift, 37 halo rows on each side), but a thread runs the two recursions of gs_theta_rec_kernel
+// down and up its column over a run of GS_PRUN rows: 36 warm-up rows, the causal values P of the run kept in
+// registers, then the anti-causal pass from 36 rows below the run upwards, which emits eq (13) row by row.
+// About 18 fp64 operations per point instead of 60; no weight table.
+// ------------------------------------------------------------------------------------------------
+#ifndef VL_GS_PRUN
+#define VL_GS_PRUN 32
+#endif
+#ifndef VL_GS_PRG
+#define VL_GS_PRG 8
+#endif
+#ifndef VL_GS_PRMINB
+#define VL_GS_PRMINB 2
+#endif
+constexpr int GS_PRUN = VL_GS_PRUN;              // rows per thread
+constexpr int GS_PRG = VL_GS_PRG;                // row groups per CTA
+constexpr int GS_PRX = 32;                       // columns per CTA
+constexpr int GS_PRW = GS_RWL * GS_RL;           // warm-up rows: 36
+constexpr int GS_PRSEG = GS_PRUN * GS_PRG;       // rows per CTA
+constexpr int GS_PRROWS = GS_PRSEG + 2 * (GS_PRW + 1) + 1;  // rows of the tile: t = -37 .. SEG + 37
+template <typename T>
+constexpr size_t gs_p_rec_smem() {
+    return sizeof(T) * (size_t)GS_PRROWS * GS_PRX;
+}
+
+template <typename T>
+__global__ void __launch_bounds__(GS_PRX * GS_PRG, VL_GS_PRMINB) gs_p_rec_kernel(const GsPArgs<T> arg) {
+    extern __shared__ __align__(16) unsigned char gs_smem[];
+    T* tile = reinterpret_cast<T*>(gs_smem);  // [GS_PRROWS][GS_PRX]; row 0 is source row jA + s - 37 of the column
+    constexpr double SQ3 = 1.7320508075688772;
+    constexpr double r = SQ3 - 2.0;
+    const int tid = threadIdx.x, c = tid % GS_PRX, g = tid / GS_PRX;
+    const int ntheta = arg.ntheta, np = arg.np;
+    const int i = blockIdx.x * GS_PRX + c;
+    const bool act = i < ntheta;
+    const bool periodic = (arg.bc_p == BC_PERIODIC);
+    const int jA = blockIdx.y * GS_PRSEG;
+    const int jB = min(np, jA + GS_PRSEG);
+    const size_t pitch = (size_t)ntheta;
+
+    double sf, a;
+    split_shift(-((act ? arg.force[i] : 0.0) * arg.dt) / arg.dp, &sf, &a);
+    int s;
+    if (periodic) {
+        sf = fmod(sf, (double)np);
+        s = (int)sf;
+    } else {
+        const double lim = (double)np + 64.0;
+        s = (int)fmin(fmax(sf, -lim), lim);
+    }
+    {
+        const T* __restrict__ col = arg.fin + (act ? i : 0);
+        const int nrows = (jB - jA) + 2 * (GS_PRW + 1) + 1;  // rows past it (ragged last segment) are zero-filled
+        int y = jA + s - (GS_PRW + 1) + g;
+        if (periodic) y = wrap_index(y, np);
+        uint32_t dst = ptx::smem_u32(tile + g * GS_PRX + c);
+        for (int k = g; k < GS_PRROWS; k += GS_PRG) {
+            const bool ok = act && k < nrows && (periodic || (unsigned)y < (unsigned)np);
+            const T* src = ok ? col + (size_t)y * pitch : arg.fin;
+            ptx::cp_async_zfill<(int)sizeof(T)>(dst, src, ok ? (unsigned)sizeof(T) : 0u);
+            dst += (uint32_t)(GS_PRG * GS_PRX * sizeof(T));
+            y += GS_PRG;
+            if (periodic && y >= np) y -= np;
+        }
+        ptx::cp_async_commit();
+    }
+    const double al = 1.0 - a, be = a;
+    const double A6 = al * (al * al - 1.0) / 6.0, B6 = a * (a * a - 1.0) / 6.0;
+    ptx::cp_async_wait<0>();
+    __syncthreads();
+    const int jlo = jA + g * GS_PRUN;
+    if (!act || jlo >= jB) return;
+
+    // x(t) = value at the foot cell of output row jlo + t: tile row g * GS_PRUN + 37 + t
+    const T* __restrict__ xcol = tile + (size_t)(g * GS_PRUN + GS_PRW + 1) * GS_PRX + c;
+    auto X = [&](int t) -> double { return (double)xcol[t * GS_PRX]; };
+
+    // causal pass: warm-up over t = -36 .. -1, then the run
+    double xm = X(-GS_PRW - 1), x0 = X(-GS_PRW), P = 0.0;
+#pragma unroll 6
+    for (int t = -GS_PRW; t < 0; ++t) {
+        const double xp = X(t + 1);
+        P = fma(r, P, (xp - 2.0 * x0) + xm);
+        xm = x0;
+        x0 = xp;
+    }
+    double Pv[GS_PRUN];
+#pragma unroll
+    for (int t = 0; t < GS_PRUN; ++t) {
+        const double xp = X(t + 1);
+        P = fma(r, P, (xp - 2.0 * x0) + xm);
+        Pv[t] = P;
+        xm = x0;
+        x0 = xp;
+    }
+    // here x0 = x(RUN), xm = x(RUN - 1): P at RUN for the f'' that the last row needs
+    const double dR = (X(GS_PRUN + 1) - 2.0 * x0) + xm;
+    const double PR = fma(r, P, dR);
+
+    // anti-causal pass: warm-up over t = RUN + 36 .. RUN + 1, then upwards through the run
+    double xp = X(GS_PRUN + GS_PRW + 1), N = 0.0;
+    x0 = X(GS_PRUN + GS_PRW);
+#pragma unroll 6
+    for (int t = GS_PRUN + GS_PRW; t > GS_PRUN; --t) {
+        const double xl = X(t - 1);
+        N = fma(r, N, (xp - 2.0 * x0) + xl);
+        xp = x0;
+        x0 = xl;
+    }
+    // here x0 = x(RUN), xp = x(RUN + 1)
+    N = fma(r, N, dR);
+    double Dn = SQ3 * ((PR + N) - dR);  // f'' h^2 at RUN
+    T* __restrict__ ocol = arg.fout + i + (size_t)jlo * pitch;
+    double xh = x0, xc = xm;  // x(t + 1), x(t) for t = RUN - 1 (xm is still x(RUN - 1) from the causal pass)
+#pragma unroll
+    for (int t = GS_PRUN - 1; t >= 0; --t) {
+        const double xl = X(t - 1);
+        const double d = (xh - 2.0 * xc) + xl;
+        N = fma(r, N, d);
+        const double D = SQ3 * ((Pv[t] + N) - d);
+        const double o = fma(B6, Dn, fma(A6, D, fma(be, xh, al * xc)));
+        if (jlo + t < jB) ocol[(size_t)t * pitch] = (T)o;
+        Dn = D;
+        xh = xc;
+        xc = xl;
     }
 }
 

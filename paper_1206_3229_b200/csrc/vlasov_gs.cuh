@@ -484,12 +484,12 @@ __global__ void __launch_bounds__(GS_PTX * GS_PG, VL_GS_PMINB) gs_p_sweep_kernel
 // ------------------------------------------------------------------------------------------------
 // momentum shift with the global spline, RECURSIVE form (default): same tile as gs_p_sweep_kernel (each column at
 // its own integer shift, 37 halo rows on each side), but a thread runs the two recursions of gs_theta_rec_kernel
-// down and up its column over a run of GS_PRUN rows: 36 warm-up rows, the causal values P of the run kept in
+// down and up its column over a run of GS_PRUN = 24 rows: 36 warm-up rows, the causal values P of the run kept in
 // registers, then the anti-causal pass from 36 rows below the run upwards, which emits eq (13) row by row.
 // About 18 fp64 operations per point instead of 60; no weight table.
 // ------------------------------------------------------------------------------------------------
 #ifndef VL_GS_PRUN
-#define VL_GS_PRUN 32
+#define VL_GS_PRUN 24
 #endif
 #ifndef VL_GS_PRG
 #define VL_GS_PRG 8

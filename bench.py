@@ -20,7 +20,8 @@ theta half shift).  Prints ONE JSON line (rank 0).
   cpu_baseline  the CPU oracle (oracle/, as it stands) timed on this box's host cores on a bounded sample
 
 --spline gs times the Global Spline variant instead (system (15), the paper's comparator): three
-60-tap passes per step, roofline.bound = "alu" against the measured fp64 FMA rate; the oracle legs then run with
+passes per step with the recursive kernels (roofline against HBM like the FD path); --gsfir 1 selects the 60-tap
+filter kernels (roofline.bound = "alu" against the measured fp64 FMA rate).  The oracle legs then run with
 KEY_SPLINE = GS too.  The default (fd) is the paper's method and the headline workload.
 
 --impl reference times the oracle (there is no other reference implementation: the paper ships no code).
@@ -269,9 +270,15 @@ def run_cuda(args):
                     "step_frac": (step_bytes * pts * K / (ms_local * 1e-3) / 1e9) / peak,
                     "step_bytes_per_point": step_bytes,
                     "two_pass_step_frac": (4 * eb * pts * K / (ms_local * 1e-3) / 1e9) / peak}
-        if args.spline == "gs":
-            # 60 FMAs per point and pass: bound by the fp64 pipe.  Peak = the measured fp64 FMA rate of this B200,
-            # 17.0 TFMA/s = 34.0 TFLOP/s (profiles/fp64_probe.txt; csrc/fp64_probe.cu), DESIGN.md section 7.
+        if args.spline == "gs" and args.gsfir == 0:
+            # recursive global-spline kernels: ~18 fp64 operations per point and pass, one read + one write of f:
+            # HBM-bound like the FD kernels
+            gs_names = {"theta1": "gs_theta_rec_kernel", "p": "gs_p_rec_kernel"}
+            roofline["kernel"] = gs_names.get(dom, dom)
+            roofline["traffic"] = committed_traffic("gsrec_" + dom, n, prec)
+        elif args.spline == "gs":
+            # 60-tap filter kernels (A/B partner): 60 FMAs per point and pass, bound by the fp64 pipe.  Peak = the
+            # measured fp64 FMA rate of this B200, 17.0 TFMA/s = 34.0 TFLOP/s (profiles/fp64_probe.txt).
             gs_names = {"theta1": "gs_theta_sweep_kernel", "p": "gs_p_sweep_kernel"}
             flops = 2.0 * 60.0 * pts
             ach_tf = flops / (kern[dom]["avg_ms"] * 1e-3) / 1e12

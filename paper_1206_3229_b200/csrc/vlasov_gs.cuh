@@ -1,6 +1,9 @@
 // vlasov_gs.cuh -- the GLOBAL SPLINE variant of the shifts (system (15);
 // the paper's accuracy comparator "GS" of Tables 1-2), as CUDA kernels for sm_100a.
 //
+// Two sets of kernels: the RECURSIVE ones (gs_theta_rec_kernel, gs_p_rec_kernel: the default, further down) and the
+// 60-TAP FILTER ones (gs_theta_sweep_kernel, gs_p_sweep_kernel: tune_gsfir = 1, the A/B partner), described first.
+//
 // The paper solves the tridiagonal system (15) for f'' on the CPU and calls it "not effective enough" in parallel
 // (L104).  Here it is not solved at all.  The system has constant coefficients (1/6, 2/3, 1/6; DESIGN.md reading
 // D22), so its inverse on a periodic (or infinite, zero-extended) line is the convolution with the two-sided
@@ -20,8 +23,8 @@
 //   gs_theta_sweep_kernel: a CTA owns a chunk of blockDim * 9 columns and walks down a band of rows; each lane owns 9
 //       consecutive columns (lane stride 9: conflict-free) and keeps their column sums (density partials, eq (10));
 //       the next row's window is prefetched into registers while the current one is computed.  One wave of CTAs.
-//   gs_p_sweep_kernel: a thread owns one column and produces 8 consecutive rows at a time; the 60 weights of a
-//       column (they depend on the force there, eq (11)) sit in shared memory [tap][column] and serve 4 row groups.
+//   gs_p_sweep_kernel: a thread owns one column and produces 16 consecutive rows at a time; the 60 weights of a
+//       column (they depend on the force there, eq (11)) sit in shared memory [tap][column] and serve 8 row groups.
 // Arithmetic is fp64 for both storage precisions.
 #pragma once
 #include "vlasov_fused.cuh"  // ptx::cp_async

@@ -60,8 +60,9 @@ extern "C" {
 #define VLASOV_KEY_SPLINE 8    /* which f'' enters eq (13): 0 (default) the local eighth-order difference of eq (16),
                                   L106-L111, the paper's method; 1 the GLOBAL SPLINE, f'' = solution of the
                                   tridiagonal system (15), L100-L102 (the paper's comparator "GS", Tables 1-2;
-                                  diagonal 2/3, D22).  Three passes per step, 60 taps per shift instead
-                                  of 10; both axes need >= 32 nodes                                             */
+                                  diagonal 2/3, D22).  Three passes per step; the solve is replaced by
+                                  its closed-form inverse (two first-order recursions per line; or, with tuning
+                                  key 110, a 60-tap filter); both axes need >= 32 nodes                          */
 /* keys 101..110 (launch-shape overrides: warps, bands, segment lengths, kernel variant) exist for the tests and
  * the tuning sweeps only; see binding.py KEY_TUNE_*.  Results never depend on them beyond rounding order.   */
 

@@ -542,6 +542,17 @@ __global__ void __launch_bounds__(GS_PRX * GS_PRG, VL_GS_PRMINB) gs_p_rec_kernel
         int y = jA + s - (GS_PRW + 1) + g;
         if (periodic) y = wrap_index(y, np);
         uint32_t dst = ptx::smem_u32(tile + g * GS_PRX + c);
+        const int ylast = y + (GS_PRROWS - 1 - g) / GS_PRG * GS_PRG;  // last row this thread copies
+        if (act && nrows == GS_PRROWS && y >= 0 && ylast < np) {       // every row exists: no per-row tests
+            const T* __restrict__ src = col + (size_t)y * pitch;
+            const size_t step = (size_t)GS_PRG * pitch;
+#pragma unroll 4
+            for (int k = g; k < GS_PRROWS; k += GS_PRG) {
+                ptx::cp_async<(int)sizeof(T)>(dst, src);
+                dst += (uint32_t)(GS_PRG * GS_PRX * sizeof(T));
+                src += step;
+            }
+        } else
         for (int k = g; k < GS_PRROWS; k += GS_PRG) {
             const bool ok = act && k < nrows && (periodic || (unsigned)y < (unsigned)np);
             const T* src = ok ? col + (size_t)y * pitch : arg.fin;

@@ -1,38 +1,44 @@
 #!/usr/bin/env python
 """bench.py -- throughput of the Strang semi-Lagrangian Vlasov step on B200.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl cuda|reference] [--n GRID] [--precision 64|32]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl cuda|reference]
+                    [--config cfg1..cfg5] [--grid N] [--precision 64|32] [--spline fd|gs] [--order 2|4]
 
-Workload (BASELINE.json cfg 5 / north_star): HMF model, water-bag + seeded noise, N x N grid (default
-8192 x 8192, fp64), dt = 0.1.  A "step" is one full Strang step (theta half shift, density, force, p shift,
-theta half shift).  Prints ONE JSON line (rank 0).
+Workload (BASELINE.json cfg 5 / north_star, the default): HMF model, water-bag + seeded noise, N x N grid (default
+8192 x 8192, fp64), dt = 0.1.  --config cfg1 .. cfg4 runs the other BASELINE.json configurations at their own sizes
+(their state fits the 126 MB L2 -- cfg 4 nearly -- so no DRAM roofline is claimed for them).  A "step" is one full
+Strang step (theta half shift, density, force, p shift, theta half shift).  Prints ONE JSON line (rank 0).
 
-  value      grid-point updates per second per Strang step (Gpts/s), whole job, state resident in HBM,
-             K steps timed as one vlasov_step(K) call with CUDA events
+  value      grid-point updates per second per Strang step (Gpts/s), whole job, state resident in HBM.  K steps are
+             timed as ONE vlasov_step(K) call between CUDA events on the launch stream; the call is repeated (at
+             least 3 times) and the MEDIAN repetition is reported; reps_ms lists all of them.
+             A call of K steps makes K + 1 passes over f (the first half theta shift is a pass of its own and the
+             last pass applies one half shift instead of two): ms_per_step carries that 1/K overhead.
   e2e        same metric through the C ABI with HOST buffers: every step uploads f from pinned host memory,
              runs vlasov_step(1) and downloads f back to pinned host memory
   roofline   dominant kernel (the one-pass kernel: p shift + two theta half shifts + density) against the
              measured HBM peak; algorithmic bytes = 16 B per grid point per launch in fp64 (one read + one
-             write of f); its duration comes from CUDA events around every launch in a second run of the
+             write of f); its duration comes from CUDA events around every launch in a further run of the
              same K steps (the timed region itself carries no per-kernel events); step_frac is the whole
              step against the bytes this run's passes must move, two_pass_step_frac against the 32 B per
-             point of the two-pass minimum north_star names
+             point of the two-pass minimum north_star names; target = north_star's 0.70 per Strang step.
+             traffic is NOT measured by this run: it is the DRAM byte count of the committed ncu capture named in
+             traffic_source (profiles/traffic.txt), refreshed with every kernel change.
   cpu_baseline  the CPU oracle (oracle/, as it stands) timed on this box's host cores on a bounded sample
 
---spline gs times the Global Spline variant instead (system (15), the paper's comparator): three
-passes per step with the recursive kernels (roofline against HBM like the FD path); --gsfir 1 selects the 60-tap
-filter kernels (roofline.bound = "alu" against the measured fp64 FMA rate).  The oracle legs then run with
-KEY_SPLINE = GS too.  The default (fd) is the paper's method and the headline workload.
-
---impl reference times the oracle (there is no other reference implementation: the paper ships no code).
+--spline gs times the Global Spline variant instead (system (15), the paper's comparator).
+--impl reference times the oracle (there is no other reference implementation: the paper ships no code) on the SAME
+grid as the CUDA arm; the number of steps it really runs is capped so that the run ends within --ref-seconds.
 N > 1: independent replicas (the path does not shard in this build): one process per
-GPU, no data-path collective, value = all replicas' grid points / max time.
+GPU, no data-path collective, value = all replicas' grid points / max time.  `python bench.py --gpus N` without
+torchrun re-executes itself under torch.distributed.run with N processes.
 """
 from __future__ import annotations
 
 import argparse
 import json
 import os
+import socket
 import sys
 import threading
 import time
@@ -45,6 +51,9 @@ sys.path.insert(0, ROOT)
 METRIC = "vlasov_grid_point_updates_per_second_per_strang_step"
 UNIT = "Gpts/s"
 HBM_FALLBACK_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md fallback
+L2_BYTES = 126e6
+TARGET_STEP_FRAC = 0.70    # north_star: >= 70 % of the HBM roofline per Strang step at 8192^2
+MODEL_NAMES = {0: "free streaming", 1: "HMF", 2: "ring", 3: "sheet"}
 
 
 def measured_peak():
@@ -57,21 +66,28 @@ def measured_peak():
 
 
 def committed_traffic(kernel: str, n: int, precision: int):
-    """DRAM bytes per launch of the dominant kernel from the committed ncu capture (profiles/), or None."""
+    """(DRAM bytes per launch, provenance) of the dominant kernel from the committed ncu capture, or (None, None).
+    profiles/traffic.txt: `<kernel>_n<N>_fp<P>_dram_bytes_per_launch = <bytes>  # ...` and a `source = ...` line."""
     path = os.path.join(ROOT, "profiles", "traffic.txt")
     key = "%s_n%d_fp%d_dram_bytes_per_launch" % (kernel, n, precision)
+    val, src = None, None
     try:
         with open(path) as fh:
             for line in fh:
                 if line.startswith(key):
-                    return float(line.split("=")[1].split()[0])
+                    val = float(line.split("=")[1].split()[0])
+                    if "@" in line:
+                        src = line.split("@", 1)[1].strip()
     except Exception:
         pass
-    return None
+    if val is None:
+        return None, None
+    return val, "profiles/traffic.txt (committed ncu --set full capture%s); not measured in this run" % (
+        ", " + src if src else "")
 
 
 class ClockSampler(threading.Thread):
-    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+    """Samples SM clock and throttle reasons through NVML from the warm-up to the end of the timed repetitions."""
 
     def __init__(self, index: int):
         super().__init__(daemon=True)
@@ -110,7 +126,7 @@ class ClockSampler(threading.Thread):
                         self.reasons.add(name)
             except Exception:
                 pass
-            time.sleep(0.002)
+            time.sleep(0.0005)
 
     def stop(self):
         self._stop_evt.set()
@@ -136,18 +152,53 @@ def max_over_ranks(value: float, world: int, backend_device=None) -> float:
     return float(t.item())
 
 
-# ------------------------------------------------------------------------------------------ oracle legs
-def oracle_throughput(n: int, steps: int, warmup: int = 0, min_seconds: float = 0.0, spline: int = 0):
-    """Gpts/s of the CPU oracle on the cfg-5 workload at grid n x n, all host cores."""
-    import oracle
+def median_rep(reps_ms):
+    """the median repetition (an actually measured one: the upper median for an even count)"""
+    s = sorted(reps_ms)
+    return s[len(s) // 2]
+
+
+# ------------------------------------------------------------------------------------------ the workload
+def workload(args, with_f0=True):
+    """the BASELINE.json configuration this run uses and the `config` object both arms print (identical)"""
     from paper_1206_3229_b200 import inputs
 
+    kw = {}
+    if args.n:
+        kw["n"] = args.n
+    c = inputs.config(args.config, with_f0=with_f0, **kw)
+    nt, npp = c["grid"]
+    eb = 8 if args.precision == 64 else 4
+    fits = nt * npp * eb <= L2_BYTES
+    bc = "x zero-extended (open)" if c["model"] == inputs.MODEL_SHEET else "theta periodic"
+    cfg = {
+        "workload": "%s %s %dx%d %s, dt=%g, %s, p zero-extended%s" % (
+            args.config, MODEL_NAMES[c["model"]], nt, npp, "fp64" if eb == 8 else "fp32", c["dt"], bc,
+            ", global-spline variant (system 15)" if args.spline == "gs" else ""),
+        "cfg": args.config, "grid": [nt, npp], "precision": args.precision, "spline": args.spline,
+        "l2": "state fits L2: DRAM roofline not claimed" if fits else
+              "state (%.0f MiB x 2 buffers) exceeds the 126 MB L2; no flush needed" % (nt * npp * eb / 2 ** 20),
+    }
+    return c, cfg
+
+
+# ------------------------------------------------------------------------------------------ oracle legs
+def make_oracle(c, spline: int):
+    import oracle
+
     cores = os.cpu_count() or 1
-    c = inputs.config("cfg5", n=n)
-    o = oracle.Oracle(c["model"], c["grid"], c["domain"], c["dt"], threads=cores, **({"spline": spline} if spline else {}))
+    params = dict(c["params"])
+    if spline:
+        params["spline"] = spline
+    o = oracle.Oracle(c["model"], c["grid"], c["domain"], c["dt"], threads=cores, **params)
     o.upload(c["f0"])
-    if warmup:
-        o.step(warmup)
+    return o
+
+
+def oracle_throughput(c, steps: int, min_seconds: float = 0.0, spline: int = 0):
+    """Gpts/s of the CPU oracle on the workload c, all host cores: `steps` at a time until min_seconds have passed"""
+    o = make_oracle(c, spline)
+    pts = float(c["grid"][0]) * float(c["grid"][1])
     done, t0 = 0, time.perf_counter()
     while True:
         o.step(steps)
@@ -157,37 +208,62 @@ def oracle_throughput(n: int, steps: int, warmup: int = 0, min_seconds: float = 
             break
     threads = o.threads
     o.close()
-    return n * n * done / el / 1e9, el, done, threads
+    return pts * done / el / 1e9, el, done, threads
 
 
 def run_reference(args):
+    """The oracle as it stands on the host cores, on the CUDA arm's grid.  The driver's --steps K --warmup W would take
+    K x 2 s at 8192^2, so the steps really run are capped: the first step is timed, then as many warm-up and timed
+    steps as fit --ref-seconds (at least one timed step)."""
     rank, _, world = dist_env()
     if rank != 0:
         return 0
-    n_ref = args.ref_n
+    c, cfg = workload(args)
+    pts = float(c["grid"][0]) * float(c["grid"][1])
+    t_wall = time.perf_counter()
+    o = make_oracle(c, int(args.spline == "gs"))
     t0 = time.perf_counter()
-    val, el, done, threads = oracle_throughput(n_ref, args.steps, warmup=args.warmup, spline=int(args.spline == "gs"))
-    sample = "CPU oracle (oracle/vlasov_oracle.c, OpenMP over lines), cfg5 HMF water-bag at %dx%d (bounded sample of the %dx%d workload), %d Strang steps" % (
-        n_ref, n_ref, args.n, args.n, done)
+    o.step(1)                      # first step: untimed warm-up (page faults of the oracle's arrays) and the estimate
+    t1 = time.perf_counter() - t0
+    budget = max(args.ref_seconds - t1, 0.0)
+    w_eff = min(max(args.warmup - 1, 0), int(0.1 * budget / t1))
+    k_eff = max(1, min(args.steps, int(0.9 * budget / t1)))
+    if w_eff:
+        o.step(w_eff)
+    t0 = time.perf_counter()
+    o.step(k_eff)
+    el = time.perf_counter() - t0
+    threads = o.threads
+    o.close()
+    val = pts * k_eff / el / 1e9
+    sample = ("CPU oracle (oracle/vlasov_oracle.c, OpenMP over lines) on the full %dx%d grid of the workload; %d timed "
+              "Strang steps after %d warm-up steps (the requested %d + %d capped to fit %.0f s)" % (
+                  c["grid"][0], c["grid"][1], k_eff, 1 + w_eff, args.steps, args.warmup, args.ref_seconds))
     line = {
         "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
-        "warmup": args.warmup, "ms_per_step": el / done * 1e3, "higher_is_better": True, "scaling": "weak",
-        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": "cfg5 HMF water-bag %dx%d fp64, dt=0.1" % (args.n, args.n), "sample_grid": n_ref},
+        "warmup": args.warmup, "ms_per_step": el / k_eff * 1e3, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": cfg,
+        "steps_timed": k_eff, "warmup_done": 1 + w_eff,
         "cpu_baseline": {"value": val, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
-        "gpu_launches": 0, "wall_s": time.perf_counter() - t0,
+        "gpu_launches": 0, "wall_s": time.perf_counter() - t_wall,
     }
     print(json.dumps(line))
     return 0
 
 
 # ------------------------------------------------------------------------------------------ CUDA arm
+KERNEL_NAMES = {
+    "theta2": "theta_sweep_bulk_kernel<2 shifts>", "theta1": "theta_sweep_bulk_kernel<1 shift>",
+    "p": "p_sweep_kernel", "ptheta2": "strang_fused_ws_kernel<p shift + 2 theta half shifts + density>",
+    "ptheta1": "strang_fused_ws_kernel<p shift + 1 theta half shift>"}
+GS_KERNEL_NAMES = {"theta1": "gs_theta_rec_kernel", "p": "gs_p_rec_kernel"}
+
+
 def run_cuda(args):
     import torch
 
     from paper_1206_3229_b200 import binding as vb
-    from paper_1206_3229_b200 import inputs
 
     rank, local_rank, world = dist_env()
     if not torch.cuda.is_available():
@@ -199,16 +275,20 @@ def run_cuda(args):
 
         dist.init_process_group("nccl", device_id=dev)
 
-    n, prec, K, W = args.n, args.precision, args.steps, max(args.warmup, 0)
+    prec, K, W = args.precision, args.steps, max(args.warmup, 0)
     eb = 8 if prec == 64 else 4
-    c = inputs.config("cfg5", n=n)
+    c, cfg = workload(args)
+    nt, npp = c["grid"]
     f0 = c["f0"].astype(np.float64 if prec == 64 else np.float32)
-    g = vb.Vlasov(c["model"], c["grid"], c["domain"], c["dt"], precision=prec, device="cuda:%d" % local_rank,
-                  fuse=args.fuse, tune_fvariant=args.fvariant, tune_graph=args.graph,
-                  **({"spline": vb.SPLINE_GS, "tune_gsfir": args.gsfir} if args.spline == "gs" else {}),
-                  **({"tune_fbands": args.fbands} if args.fbands > 0 else {}))
+    params = dict(c["params"])
+    params.update(fuse=args.fuse, tune_graph=args.graph)
+    if args.spline == "gs":
+        params["spline"] = vb.SPLINE_GS
+    if args.fbands > 0:
+        params["tune_fbands"] = args.fbands
+    g = vb.Vlasov(c["model"], c["grid"], c["domain"], c["dt"], precision=prec, device="cuda:%d" % local_rank, **params)
     g.upload(f0)
-    pts = float(n) * float(n)
+    pts = float(nt) * float(npp)
 
     def barrier():
         if world > 1:
@@ -217,21 +297,28 @@ def run_cuda(args):
             dist.barrier()
         torch.cuda.synchronize()
 
-    # ---- device-resident timing: W warm-up steps, then exactly K steps (no per-kernel events in this region)
+    # ---- device-resident timing: W warm-up steps, then repetitions of exactly K steps as one vlasov_step(K) call
+    # (no per-kernel events in this region); the clock sampler runs from the warm-up to the last repetition
+    sampler = ClockSampler(local_rank)
+    sampler.start()
     if W:
         g.step(W)
-    sampler = ClockSampler(local_rank)
     barrier()
-    launches0 = vb.vlasov_launch_count()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    sampler.start()
-    e0.record()
-    g.step(K)
-    e1.record()
-    barrier()
+    reps_ms, launches = [], 0
+    t_load = time.perf_counter()
+    while len(reps_ms) < args.reps or (time.perf_counter() - t_load < args.min_load_seconds and len(reps_ms) < 50):
+        launches0 = vb.vlasov_launch_count()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        e0.record()
+        g.step(K)
+        e1.record()
+        barrier()
+        reps_ms.append(max_over_ranks(e0.elapsed_time(e1), world, dev))
+        launches = vb.vlasov_launch_count() - launches0
     clocks = sampler.stop()
-    ms_local = e0.elapsed_time(e1)
-    launches = vb.vlasov_launch_count() - launches0
+    ms = median_rep(reps_ms)
+    value = world * pts * K / (ms * 1e-3) / 1e9
 
     # ---- the same K steps again with a CUDA-event pair around every launch: per-kernel durations for the roofline
     vb.vlasov_set_param(vb.KEY_PROFILE, 1)
@@ -239,11 +326,9 @@ def run_cuda(args):
     g.step(K)
     ktimes = vb.vlasov_kernel_times()
     vb.vlasov_set_param(vb.KEY_PROFILE, 0)
-    ms = max_over_ranks(ms_local, world, dev)
-    value = world * pts * K / (ms * 1e-3) / 1e9
     mom = g.moments()
 
-    # ---- roofline of the dominant kernel (CUDA-event durations recorded inside the timed region)
+    # ---- roofline of the dominant kernel
     peak, peak_src = measured_peak()
     kern = {}
     for name, d in ktimes.items():
@@ -260,36 +345,22 @@ def run_cuda(args):
     roofline = None
     if dom is not None:
         ach = kern[dom]["achieved_gbs"]
-        names = {"theta2": "theta_sweep_bulk_kernel<2 shifts>", "theta1": "theta_sweep_bulk_kernel<1 shift>",
-                 "p": "p_sweep_kernel", "ptheta2": "strang_fused_ws_kernel<p shift + 2 theta half shifts + density>",
-                 "ptheta1": "strang_fused_ws_kernel<p shift + 1 theta half shift>"}
-        roofline = {"bound": "hbm", "kernel": names[dom],
+        gs = args.spline == "gs"
+        traffic, traffic_src = committed_traffic(("gsrec_" if gs else "") + dom, nt, prec) if nt == npp else (None, None)
+        step_frac = (step_bytes * pts * K / (ms * 1e-3) / 1e9) / peak
+        roofline = {"bound": "hbm", "kernel": (GS_KERNEL_NAMES if gs else KERNEL_NAMES).get(dom, dom),
                     "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
-                    "traffic": committed_traffic(dom, n, prec),
+                    "traffic": traffic, "traffic_source": traffic_src,
                     "peak_source": peak_src, "algorithmic_bytes_per_launch": 2 * eb * pts,
-                    "step_frac": (step_bytes * pts * K / (ms_local * 1e-3) / 1e9) / peak,
-                    "step_bytes_per_point": step_bytes,
-                    "two_pass_step_frac": (4 * eb * pts * K / (ms_local * 1e-3) / 1e9) / peak}
-        if args.spline == "gs" and args.gsfir == 0:
-            # recursive global-spline kernels: ~18 fp64 operations per point and pass, one read + one write of f:
-            # HBM-bound like the FD kernels
-            gs_names = {"theta1": "gs_theta_rec_kernel", "p": "gs_p_rec_kernel"}
-            roofline["kernel"] = gs_names.get(dom, dom)
-            roofline["traffic"] = committed_traffic("gsrec_" + dom, n, prec)
-        elif args.spline == "gs":
-            # 60-tap filter kernels (A/B partner): 60 FMAs per point and pass, bound by the fp64 pipe.  Peak = the
-            # measured fp64 FMA rate of this B200, 17.0 TFMA/s = 34.0 TFLOP/s (profiles/fp64_probe.txt).
-            gs_names = {"theta1": "gs_theta_sweep_kernel", "p": "gs_p_sweep_kernel"}
-            flops = 2.0 * 60.0 * pts
-            ach_tf = flops / (kern[dom]["avg_ms"] * 1e-3) / 1e12
-            roofline = {"bound": "alu", "kernel": gs_names.get(dom, dom), "achieved": ach_tf, "peak": 34.0,
-                        "unit": "TFLOP/s", "frac": ach_tf / 34.0, "traffic": committed_traffic("gs_" + dom, n, prec),
-                        "peak_source": "measured fp64 FMA rate, profiles/fp64_probe.txt (17.0 TFMA/s)",
-                        "algorithmic_flops_per_launch": flops, "hbm_gbs": ach, "hbm_frac": ach / peak}
+                    "step_frac": step_frac, "step_bytes_per_point": step_bytes,
+                    "two_pass_step_frac": (4 * eb * pts * K / (ms * 1e-3) / 1e9) / peak,
+                    "target_step_frac": TARGET_STEP_FRAC, "meets_target": bool(step_frac >= TARGET_STEP_FRAC)}
+        if nt * npp * eb <= L2_BYTES:
+            roofline["note"] = "state fits L2: the fractions above are NOT a DRAM roofline claim"
 
     # ---- end to end through the C ABI with host buffers
     Ke = min(K, args.e2e_steps)
-    host = torch.empty((n, n), dtype=torch.float64 if prec == 64 else torch.float32).pin_memory()
+    host = torch.empty((npp, nt), dtype=torch.float64 if prec == 64 else torch.float32).pin_memory()
     host.numpy()[:] = f0
     hp = host.data_ptr()
     for _ in range(2):
@@ -319,29 +390,40 @@ def run_cuda(args):
     if rank != 0:
         return 0
 
-    # ---- oracle on the host cores (bounded sample), rank 0 only
+    # ---- oracle on the host cores (bounded sample of the same workload), rank 0 only
     cpu = None
     if not args.no_cpu_baseline:
-        nb = args.cpu_n
-        val, el, done, threads = oracle_throughput(nb, 1, warmup=0, min_seconds=args.cpu_seconds, spline=int(args.spline == "gs"))
+        val, el, done, threads = oracle_throughput(c, 1, min_seconds=args.cpu_seconds, spline=int(args.spline == "gs"))
         cpu = {"value": val, "unit": UNIT, "cores": threads, "kind": "oracle",
-               "sample": "%d Strang step(s) of cfg5 HMF water-bag on a %dx%d grid (%.1f s of wall time), oracle/vlasov_oracle.c with OpenMP over lines" % (done, nb, nb, el)}
+               "sample": "%d Strang step(s) of the same workload on its full %dx%d grid (%.1f s of wall time), "
+                         "oracle/vlasov_oracle.c with OpenMP over lines" % (done, nt, npp, el)}
 
+    cfg = dict(cfg)
+    cfg.update({"passes_per_step": passes / K, "fuse": args.fuse,
+                "parallelism": "replicas x%d" % world if world > 1 else "single GPU"})
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": "f64" if prec == 64 else "f32", "data": "synthetic",
-        "config": {"workload": "cfg5 HMF water-bag %dx%d %s, dt=0.1, theta periodic, p zero-extended, seeded 1e-6 noise%s" % (
-                       n, n, "fp64" if prec == 64 else "fp32", ", global-spline variant (system 15)" if args.spline == "gs" else ""),
-                   "grid": [n, n], "passes_per_step": passes / K, "fuse": args.fuse,
-                   "l2": "state (%.0f MiB x 2 buffers) exceeds the 126 MB L2; no flush needed" % (pts * eb / 2 ** 20)
-                   if pts * eb > 126e6 else "state fits L2: DRAM roofline not claimed",
-                   "parallelism": "replicas x%d" % world if world > 1 else "single GPU", "launch": info},
-        "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "kernels": kern,
+        "dtype": "f64" if prec == 64 else "f32", "data": "synthetic", "config": cfg,
+        "timing": {"reps": len(reps_ms), "reps_ms": reps_ms, "statistic": "median repetition of vlasov_step(K)",
+                   "note": "K steps = K + 1 passes (first half theta shift + last pass with one half shift)"},
+        "launch": info, "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "kernels": kern,
         "cpu_baseline": cpu, "final_moments": {"t": mom[0], "mass": mom[1], "E": mom[7], "Mx": mom[5]},
     }
     print(json.dumps(line))
     return 0
+
+
+def relaunch_under_torchrun(args) -> int:
+    """`python bench.py --gpus N` without torchrun: run N ranks of this script under torch.distributed.run"""
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus),
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + [
+               "--grid" if a == "--n" else a for a in sys.argv[1:]]
+    os.execv(sys.executable, cmd)
+    return 1  # not reached
 
 
 def main():
@@ -350,12 +432,18 @@ def main():
     ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=20)
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
-    ap.add_argument("--n", type=int, default=8192, help="grid size N (N x N)")
+    ap.add_argument("--config", default="cfg5", choices=["cfg1", "cfg2", "cfg3", "cfg4", "cfg5"],
+                    help="BASELINE.json configuration (cfg5 = the throughput workload the metric is quoted on)")
+    ap.add_argument("--grid", "--n", dest="n", type=int, default=0,
+                    help="grid size N (N x N); default: the configuration's own (cfg5: 8192).  Under torchrun write "
+                         "--grid (torchrun's own parser finds --n ambiguous)")
     ap.add_argument("--precision", type=int, default=64, choices=[64, 32])
+    ap.add_argument("--reps", type=int, default=3, help="repetitions of the timed vlasov_step(K) call (median reported)")
+    ap.add_argument("--min-load-seconds", type=float, default=0.06,
+                    help="keep repeating (up to 50 times) until the GPU has been under load this long (clock samples)")
     ap.add_argument("--e2e-steps", type=int, default=10)
-    ap.add_argument("--cpu-n", type=int, default=8192, help="grid of the cpu_baseline sample")
     ap.add_argument("--cpu-seconds", type=float, default=10.0)
-    ap.add_argument("--ref-n", type=int, default=1024, help="grid of the --impl reference sample")
+    ap.add_argument("--ref-seconds", type=float, default=120.0, help="wall-time cap of the --impl reference run")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--fuse", type=int, default=2, choices=[0, 1, 2],
                     help="passes per step: 2 = one (p + theta in one kernel, default), 1 = two, 0 = three")
@@ -364,12 +452,14 @@ def main():
                     help="1 (default): steady-state step pairs are launched as CUDA graphs, 0: plain launches")
     ap.add_argument("--spline", default="fd", choices=["fd", "gs"],
                     help="fd: f'' by eq (16), the paper's method and the headline workload; gs: the Global Spline "
-                         "comparator, system (15) (SURVEY 8(f) NEXT #2; three 60-tap passes per step, fp64-ALU bound)")
-    ap.add_argument("--gsfir", type=int, default=0, choices=[0, 1],
-                    help="with --spline gs: 1 = the 60-tap filter kernels instead of the recursive ones (A/B partner)")
-    ap.add_argument("--fvariant", type=int, default=0, choices=[0, 1],
-                    help="one-pass kernel: 0 = warp-specialised (default), 1 = every warp does both stages")
+                         "comparator, system (15) (SURVEY 8(f) NEXT #2)")
     args = ap.parse_args()
+    _, _, world = dist_env()
+    if args.gpus != world:
+        if world == 1 and args.gpus > 1 and "RANK" not in os.environ:
+            return relaunch_under_torchrun(args)
+        raise SystemExit("bench.py: --gpus %d but WORLD_SIZE is %d (launch with torch.distributed.run "
+                         "--nproc-per-node %d)" % (args.gpus, world, args.gpus))
     if args.impl == "reference":
         return run_reference(args)
     return run_cuda(args)

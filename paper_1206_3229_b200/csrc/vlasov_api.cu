@@ -26,12 +26,10 @@ constexpr int R_THETA = 9;       // consecutive outputs per lane in the theta ke
 constexpr int TB_NS = 3;         // rows in flight per warp in the bulk-copy theta kernel
 constexpr int TB_WARPS = 4;      // warps per CTA (independent pipelines)
 constexpr int TB_MINB = 3;       // CTAs per SM the register budget is set for
-constexpr int FU_NT = 384;       // threads per CTA of the one-pass kernel (one per source column)
-constexpr int FU_R = 11;         // consecutive outputs per lane in its theta stage (odd)
-constexpr int FU_NSTG = 3;       // cp.async ring depth (phases of 12 rows)
-constexpr int FU_NW = FU_NT / 32;  // density partial rows per band of the one-pass kernel, variant 1 (all warps alike)
-constexpr int FW_NSTG = 3;       // ring depth (groups of 12 rows) of the warp-specialised one-pass kernel (variant 0)
-constexpr int KEY_TUNE_FVARIANT = 108, KEY_TUNE_GRAPH = 109, KEY_TUNE_GSFIR = 110;
+constexpr int FU_R = 11;         // consecutive outputs per lane in the theta stage of the one-pass kernel (odd)
+constexpr int FW_NSTG = 3;       // ring depth (groups of 12 rows) of the one-pass kernel
+constexpr int FW_NTW = 12;       // its theta warps = density partial rows per band
+constexpr int KEY_TUNE_GRAPH = 109;
 constexpr int FU_PAD = 12;       // rows of padding of the theta weight tables (the last phase of a band reads on)
 constexpr int NCLS = 6;          // profiled kernel classes: theta x1, theta x2, p, rho+force, p+theta x2, p+theta x1
 constexpr int KEY_TUNE_FBANDS = 107;
@@ -46,10 +44,8 @@ struct Ctx {
     double xmin = 0, xmax = 0, pmin = 0, pmax = 0, dt = 0, eps = 0.01, t = 0;
     int bc_x = 0, bc_p = 1, prec = 64;
     int spline = 0;  // 0: f'' by eq (16) (the paper's method), 1: global spline, system (15) (vlasov_gs.cuh)
-    double *gsw = nullptr, *gsH6 = nullptr, *gsab = nullptr;  // gsab: [Np][4] = 1-a, a, A/6, B/6 of a half theta shift
-    int gs_fir = 0;                  // KEY_TUNE_GSFIR: 1 = the 60-tap filter kernels instead of the recursive ones
-    int gs_rbands = 0, gs_rrpb = 0;  // bands of the recursive theta kernel  // [Np][GS_NT] row weights of a half theta shift; H/6 table
-    int gs_bands = 0, gs_rpb = 0, gs_pseg = 0, gs_pnseg = 0, gs_tbd = 128;
+    double* gsab = nullptr;          // [Np][4] = 1-a, a, A/6, B/6 of a half theta shift
+    int gs_rbands = 0, gs_rrpb = 0;  // bands of the global-spline theta kernel
     bool history = false;
     int fuse = 2;  // 0: p and theta passes apart, 1: adjacent half theta shifts in one pass, 2: p + theta in one pass
     cudaStream_t stream = nullptr;
@@ -78,13 +74,13 @@ struct Ctx {
     // per parity of the ping-pong; captured on a private stream, launched on the attached one
     bool graphs = true;
     cudaGraphExec_t gexec[2] = {nullptr, nullptr};
+    unsigned graph_kernels[2] = {0, 0};
     cudaStream_t cap_stream = nullptr;
     int fbands[3] = {0, 0, 0}, frpb[3] = {0, 0, 0}, fcols[3] = {0, 0, 0};
     bool onepass = false;
     int tune_fbands = 0;
-    int fvariant = 0;              // 0: warp-specialised one-pass kernel, 1: every warp does both stages
-    int fnw() const { return fvariant == 1 ? FU_NW : 12; }
-    int fgran(size_t elem) const { return fvariant == 1 ? 1 : (int)(16 / elem); }  // lanes per column-block granule
+    int fnw() const { return FW_NTW; }
+    int fgran(size_t elem) const { return (int)(16 / elem); }  // lanes per column-block granule
     std::vector<int> h_srow;
 
     // launch configuration
@@ -162,14 +158,14 @@ int cdiv(int a, int b) { return (a + b - 1) / b; }
 void free_small() {
     void* ptrs[] = {G.srow, G.wrow, G.cos_t, G.sin_t, G.ringK, G.ringV, G.rho, G.force, G.rho_m,
                     G.phi,  G.mpart, G.pkpart, G.mom_dev, G.hist, G.wrow2, G.colpart_f, G.ticket, G.caspart, G.ringpart, G.ringtick,
-                    G.gsw, G.gsH6, G.gsab};
+                    G.gsab};
     for (void* p : ptrs)
         if (p) cudaFree(p);
     G.srow = nullptr;
     G.wrow = G.cos_t = G.sin_t = G.ringK = G.ringV = G.rho = G.force = G.rho_m = G.phi = G.mpart = G.pkpart =
         G.mom_dev = G.hist = G.wrow2 = G.colpart_f = nullptr;
     G.ticket = nullptr;
-    G.gsw = G.gsH6 = G.gsab = nullptr;
+    G.gsab = nullptr;
     G.caspart = nullptr;
     G.ringpart = nullptr;
     G.ringtick = nullptr;
@@ -272,11 +268,8 @@ int configure_theta_bulk() {
 // of the density partials).  Sets G.fbands[NST] = 0 when the grid does not qualify.
 template <typename T, int NST>
 int configure_fused() {
-    using C = vl::FusedCfg<T, NST, FU_NT, FU_R, FU_NSTG>;
-    CU(cudaFuncSetAttribute(vl::strang_fused_kernel<T, NST, FU_NT, FU_R, FU_NSTG>,
-                            cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM_BYTES));
-    CU(cudaFuncSetAttribute(vl::strang_fused_ws_kernel<T, NST, FU_R, FW_NSTG, 12>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                            (int)vl::FusedWsCfg<T, NST, FU_R, FW_NSTG, 12>::SMEM_BYTES));
+    CU(cudaFuncSetAttribute(vl::strang_fused_ws_kernel<T, NST, FU_R, FW_NSTG, FW_NTW>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                            (int)vl::FusedWsCfg<T, NST, FU_R, FW_NSTG, FW_NTW>::SMEM_BYTES));
     const int np = G.np, nt = G.ntheta;
     G.fbands[NST] = 0;
     for (int j = 1; j < np; ++j)
@@ -371,8 +364,7 @@ size_t workspace_bytes() {
     return round256(state_bytes()) + round256((size_t)max_bands_bound() * G.ntheta * sizeof(double));
 }
 
-int prepare() {
-    if (G.prepared) return VLASOV_OK;
+int prepare_tables() {
     const int nt = G.ntheta, np = G.np;
     const double dx = (G.xmax - G.xmin) / (double)nt, dp = (G.pmax - G.pmin) / (double)np;
     const double tau = 0.5 * G.dt;
@@ -397,16 +389,32 @@ int prepare() {
     }
     G.h_srow = srow;
     // composite weights of two equal half shifts, W = w * w (19 taps): the one-pass kernel applies both at once
-    std::vector<double> wrow2((size_t)(np + FU_PAD) * 20, 0.0);
+    constexpr int W2 = 20;  // FusedWsCfg<T, 2, ...>::WST
+    std::vector<double> wrow2((size_t)(np + FU_PAD) * W2, 0.0);
     for (int j = 0; j < np; ++j) {
         const double* w = &wrow[(size_t)j * vl::WROW_STRIDE];
-        double* W = &wrow2[(size_t)j * 20];
+        double* W = &wrow2[(size_t)j * W2];
         for (int n = 0; n < 19; ++n) {
             double acc = 0.0;
             for (int m = (n > 9 ? n - 9 : 0); m <= (n < 9 ? n : 9); ++m) acc += w[m] * w[n - m];
             W[n] = acc;
         }
         W[19] = 2.0 * (double)srow[j];  // integer part of the two half shifts together
+        if (G.prec == 32) {  // fp32 arithmetic: both tables hold the difference-form weights (vl::diff_form_weights)
+            double U[18];
+            vl::diff_form_weights(W, 19, 2 * vl::FD_C + 1, U);
+            for (int n = 0; n < 18; ++n) W[n] = U[n];
+            W[18] = 0.0;
+        }
+    }
+    if (G.prec == 32) {
+        for (int j = 0; j < np; ++j) {
+            double* w = &wrow[(size_t)j * vl::WROW_STRIDE];
+            double U[9];
+            vl::diff_form_weights(w, 10, vl::FD_C, U);
+            for (int m = 0; m < 9; ++m) w[m] = U[m];
+            w[9] = 0.0;
+        }
     }
     CU(cudaMalloc(&G.wrow2, sizeof(double) * wrow2.size()));
     CU(cudaMemcpy(G.wrow2, wrow2.data(), sizeof(double) * wrow2.size(), cudaMemcpyHostToDevice));
@@ -456,17 +464,12 @@ int prepare() {
     int rc = (G.prec == 32) ? configure_all<float>() : configure_all<double>();
     if (rc != 0) return rc;
     if (G.spline == 1) {
-        // global spline (system (15), L100-L102): 60-tap row weights of a half theta shift, H/6 for the p shift
-        if (nt < vl::GS_MIN_N || np < vl::GS_MIN_N)
-            return fail(VLASOV_EINVAL, "SPLINE = 1 (global spline) needs at least 32 nodes on both axes");
-        std::vector<double> H6(2 * vl::GS_Q + 3);
-        vl::gs_H_over_6(H6.data());
-        std::vector<double> gsw((size_t)np * vl::GS_NT), gsab((size_t)np * 4);
+        // global spline (system (15), L100-L102): per row 1-a, a, A/6, B/6 of a half theta shift
+        std::vector<double> gsab((size_t)np * 4);
         for (int j = 0; j < np; ++j) {
             const double p = G.pmin + (double)j * dp;
             double sf, a;
             vl::split_shift(-(p * tau) / dx, &sf, &a);
-            vl::gs_weights(a, H6.data(), &gsw[(size_t)j * vl::GS_NT]);
             const double al = 1.0 - a;
             gsab[(size_t)j * 4 + 0] = al;
             gsab[(size_t)j * 4 + 1] = a;
@@ -475,39 +478,8 @@ int prepare() {
         }
         CU(cudaMalloc(&G.gsab, sizeof(double) * gsab.size()));
         CU(cudaMemcpy(G.gsab, gsab.data(), sizeof(double) * gsab.size(), cudaMemcpyHostToDevice));
-        CU(cudaMalloc(&G.gsw, sizeof(double) * gsw.size()));
-        CU(cudaMalloc(&G.gsH6, sizeof(double) * H6.size()));
-        CU(cudaMemcpy(G.gsw, gsw.data(), sizeof(double) * gsw.size(), cudaMemcpyHostToDevice));
-        CU(cudaMemcpy(G.gsH6, H6.data(), sizeof(double) * H6.size(), cudaMemcpyHostToDevice));
         G.onepass = false;
-        // theta: threads per CTA (64 .. 256) with the least idle columns in the last chunk; bands of rows so that
-        // all CTAs are resident at once (one full wave).  p: segments of 64 rows, many small CTAs
-        int best_bd = 128;
-        long best_cols = -1;
-#ifndef VL_GS_TBD_LO
-#define VL_GS_TBD_LO 64
-#define VL_GS_TBD_HI 128
-#endif
-        for (int bd = VL_GS_TBD_HI; bd >= VL_GS_TBD_LO; bd -= 32) {
-            const long cols = (long)cdiv(nt, vl::GS_TR * bd) * vl::GS_TR * bd;
-            if (best_cols < 0 || cols < best_cols) {
-                best_cols = cols;
-                best_bd = bd;
-            }
-        }
-        G.gs_tbd = best_bd;
-        int occ = 1;
-        if (G.prec == 32) CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, vl::gs_theta_sweep_kernel<float>, best_bd, 0));
-        else CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, vl::gs_theta_sweep_kernel<double>, best_bd, 0));
-        if (occ < 1) occ = 1;
-        const int nch = cdiv(nt, vl::GS_TR * best_bd);
-        int bands = (G.sm_count * occ) / nch;
-        if (bands < 1) bands = 1;
-        if (bands > max_bands_bound()) bands = max_bands_bound();
-        if (bands > np) bands = np;
-        G.gs_rpb = cdiv(np, bands);
-        G.gs_bands = cdiv(np, G.gs_rpb);
-        {   // recursive theta kernel: 4 warps x 216 columns per CTA, bands for one resident wave
+        {   // theta kernel: 4 warps x 216 columns per CTA, bands of rows for one resident wave
             int occ2 = 1;
             if (G.prec == 32) CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ2, vl::gs_theta_rec_kernel<float>, vl::GS_RWARPS * 32, 0));
             else CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ2, vl::gs_theta_rec_kernel<double>, vl::GS_RWARPS * 32, 0));
@@ -522,10 +494,6 @@ int prepare() {
         }
         CU(cudaFuncSetAttribute(vl::gs_p_rec_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)vl::gs_p_rec_smem<float>()));
         CU(cudaFuncSetAttribute(vl::gs_p_rec_kernel<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)vl::gs_p_rec_smem<double>()));
-        G.gs_pseg = vl::GS_PSEG;
-        CU(cudaFuncSetAttribute(vl::gs_p_sweep_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)vl::gs_p_smem<float>()));
-        CU(cudaFuncSetAttribute(vl::gs_p_sweep_kernel<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)vl::gs_p_smem<double>()));
-        G.gs_pnseg = cdiv(np, G.gs_pseg);
     }
     CU(cudaMalloc(&G.pkpart, sizeof(double) * 2 * (size_t)G.mbands * cdiv(nt, 256)));
     CU(cudaMalloc(&G.caspart, sizeof(double) * 4 * ((size_t)G.mbands * cdiv(nt, 256) + 1)));
@@ -535,6 +503,28 @@ int prepare() {
         CU(cudaMemset(G.colpart_f, 0, sizeof(double) * nb * nt));
     }
     G.cp_bands = max_bands_bound();
+    return VLASOV_OK;
+}
+
+// Tables, counters and launch shapes, once per context.  The uploads above are blocking copies and memsets on the
+// legacy default stream, while the kernels run on the stream handed to vlasov_attach, which may be a non-blocking
+// stream that nothing orders after the legacy one: the device-wide synchronisation below makes every table and every
+// zeroed counter final before any kernel can be enqueued (a one-time cost).  A failure frees what was allocated, so
+// that a retry does not leak.
+int prepare() {
+    if (G.prepared) return VLASOV_OK;
+    if (G.spline == 1 && (G.ntheta < vl::GS_MIN_N || G.np < vl::GS_MIN_N))
+        return fail(VLASOV_EINVAL, "SPLINE = 1 (global spline) needs at least 32 nodes on both axes");
+    const int rc = prepare_tables();
+    if (rc != VLASOV_OK) {
+        free_small();
+        return rc;
+    }
+    if (cudaDeviceSynchronize() != cudaSuccess) {
+        free_small();
+        CU(cudaGetLastError());
+        return fail(VLASOV_ECUDA, "prepare: device synchronisation failed");
+    }
     G.prepared = true;
     return VLASOV_OK;
 }
@@ -607,28 +597,10 @@ int launch_gs_theta_rec(bool want_colsums) {
 }
 
 template <typename T>
-int launch_gs_theta(bool want_colsums) {
-    if (!G.gs_fir) return launch_gs_theta_rec<T>(want_colsums);
-    vl::GsThetaArgs<T> a;
-    a.fin = static_cast<const T*>(G.f[G.cur]);
-    a.fout = static_cast<T*>(G.f[G.cur ^ 1]);
-    a.srow = G.srow;
-    a.gsw = G.gsw;
-    a.colpart = want_colsums ? G.colpart : nullptr;
-    a.ntheta = G.ntheta;
-    a.np = G.np;
-    a.bc_x = G.bc_x;
-    a.rows_per_band = G.gs_rpb;
-    prof_begin(0);
-    vl::gs_theta_sweep_kernel<T><<<dim3(cdiv(G.ntheta, vl::GS_TR * G.gs_tbd), G.gs_bands), G.gs_tbd, 0, G.stream>>>(a);
-    prof_end(0);
-    LAUNCH_CHECK();
-    G.cur ^= 1;
-    return VLASOV_OK;
-}
+int launch_gs_theta(bool want_colsums) { return launch_gs_theta_rec<T>(want_colsums); }
 
 int theta_bands(int nstage) {
-    if (G.spline == 1) return G.gs_fir ? G.gs_bands : G.gs_rbands;
+    if (G.spline == 1) return G.gs_rbands;
     return G.theta_bulk ? G.bgrid[nstage].nbands : G.nbands[nstage];
 }
 
@@ -672,17 +644,13 @@ int launch_gs_p() {
     a.fin = static_cast<const T*>(G.f[G.cur]);
     a.fout = static_cast<T*>(G.f[G.cur ^ 1]);
     a.force = G.force;
-    a.H6 = G.gsH6;
     a.ntheta = G.ntheta;
     a.np = G.np;
     a.bc_p = G.bc_p;
     a.dt = G.dt;
     a.dp = (G.pmax - G.pmin) / (double)G.np;
     prof_begin(2);
-    if (!G.gs_fir)
-        vl::gs_p_rec_kernel<T><<<dim3(cdiv(G.ntheta, vl::GS_PRX), cdiv(G.np, vl::GS_PRSEG)), vl::GS_PRX * vl::GS_PRG, vl::gs_p_rec_smem<T>(), G.stream>>>(a);
-    else
-    vl::gs_p_sweep_kernel<T><<<dim3(cdiv(G.ntheta, vl::GS_PTX), G.gs_pnseg), vl::GS_PTX * vl::GS_PG, vl::gs_p_smem<T>(), G.stream>>>(a);
+    vl::gs_p_rec_kernel<T><<<dim3(cdiv(G.ntheta, vl::GS_PRX), cdiv(G.np, vl::GS_PRSEG)), vl::GS_PRX * vl::GS_PRG, vl::gs_p_rec_smem<T>(), G.stream>>>(a);
     prof_end(2);
     LAUNCH_CHECK();
     G.cur ^= 1;
@@ -698,13 +666,13 @@ int p_pass() {
 // partials of the result in colpart_f (eqs (11), (12), (9), (10))
 template <typename T, int NST>
 int launch_fused(bool want_colsums) {
-    using C = vl::FusedCfg<T, NST, FU_NT, FU_R, FU_NSTG>;
+    using CW = vl::FusedWsCfg<T, NST, FU_R, FW_NSTG, FW_NTW>;
     vl::FusedArgs<T> a;
     a.fin = static_cast<const T*>(G.f[G.cur]);
     a.fout = static_cast<T*>(G.f[G.cur ^ 1]);
     a.force = G.force;
     a.wtab = NST == 2 ? G.wrow2 : G.wrow;
-    a.bulk_ok = (G.ntheta % C::EPV == 0) ? 1 : 0;
+    a.bulk_ok = (G.ntheta % CW::EPV == 0) ? 1 : 0;
     a.gran = G.fgran(sizeof(T));
     a.colpart = want_colsums ? G.colpart_f : nullptr;
     a.ntheta = G.ntheta;
@@ -715,12 +683,7 @@ int launch_fused(bool want_colsums) {
     a.dp = (G.pmax - G.pmin) / (double)G.np;
     dim3 grid(G.fcols[NST], G.fbands[NST]);
     prof_begin(NST == 2 ? 4 : 5);
-    if (G.fvariant == 1) {
-        vl::strang_fused_kernel<T, NST, FU_NT, FU_R, FU_NSTG><<<grid, FU_NT, C::SMEM_BYTES, G.stream>>>(a);
-    } else {
-        using CW = vl::FusedWsCfg<T, NST, FU_R, FW_NSTG, 12>;
-        vl::strang_fused_ws_kernel<T, NST, FU_R, FW_NSTG, 12><<<grid, CW::NT, CW::SMEM_BYTES, G.stream>>>(a);
-    }
+    vl::strang_fused_ws_kernel<T, NST, FU_R, FW_NSTG, FW_NTW><<<grid, CW::NT, CW::SMEM_BYTES, G.stream>>>(a);
     prof_end(NST == 2 ? 4 : 5);
     LAUNCH_CHECK();
     G.cur ^= 1;
@@ -832,6 +795,7 @@ int launch_step_pair_graph() {
             e = cudaStreamEndCapture(G.cap_stream, &graph);
         }
         G.stream = user;
+        G.graph_kernels[par] = (unsigned)(G.launches - l0);  // kernels inside the graph (the ring model has six)
         G.launches = l0;
         G.cur = par;
         if (rc != VLASOV_OK) return rc;
@@ -841,7 +805,7 @@ int launch_step_pair_graph() {
         CU(e);
     }
     CU(cudaGraphLaunch(G.gexec[par], G.stream));
-    G.launches += 4;
+    G.launches += G.graph_kernels[par];
     return VLASOV_OK;
 }
 
@@ -925,6 +889,8 @@ int vlasov_set_param(int key, double value) {
         case VLASOV_KEY_HISTORY: G.history = (value != 0.0); break;
         case VLASOV_KEY_SPLINE:
             if (value != 0.0 && value != 1.0) return fail(VLASOV_EINVAL, "SPLINE must be 0 (eq 16) or 1 (system 15)");
+            if (value == 1.0 && (G.ntheta < vl::GS_MIN_N || G.np < vl::GS_MIN_N))
+                return fail(VLASOV_EINVAL, "SPLINE = 1 (global spline) needs at least 32 nodes on both axes");
             G.spline = (int)value;
             break;
         case VLASOV_KEY_FUSE:
@@ -932,9 +898,7 @@ int vlasov_set_param(int key, double value) {
             G.fuse = (int)value;
             break;
         case KEY_TUNE_FBANDS: G.tune_fbands = (int)value; break;
-        case KEY_TUNE_FVARIANT: G.fvariant = (value == 1.0) ? 1 : 0; break;
         case KEY_TUNE_GRAPH: G.graphs = (value != 0.0); break;
-        case KEY_TUNE_GSFIR: G.gs_fir = (value != 0.0) ? 1 : 0; break;
         case VLASOV_KEY_PROFILE: G.profile = (value != 0.0); break;
         case KEY_TUNE_NW1: G.tune_nw1 = (int)value; break;
         case KEY_TUNE_NW2: G.tune_nw2 = (int)value; break;

@@ -121,6 +121,7 @@ __global__ void __launch_bounds__((4 + NTW_) * 32, 1) strang_fused_ws_kernel(con
         int rn[CPT];
         T w[CPT][10];
         T v[CPT][12];  // register rings: taps of output row r of a group are v[k][(r + m) % 12]
+        T e[sizeof(T) == 4 ? CPT : 1][12];  // fp32 arithmetic (difference form): e[k][i] = v[k][i + 1] - v[k][i]
 #pragma unroll
         for (int k = 0; k < CPT; ++k) {
             const int q = tid + k * NPT;
@@ -139,8 +140,16 @@ __global__ void __launch_bounds__((4 + NTW_) * 32, 1) strang_fused_ws_kernel(con
             }
             double wd[10];
             spline_fd8_weights(a, wd);
+            if (sizeof(T) == 4) {  // difference-form weights U_0..U_8 (diff_form_weights)
+                double U[9];
+                diff_form_weights(wd, 10, FD_C, U);
 #pragma unroll
-            for (int m = 0; m < 10; ++m) w[k][m] = (T)wd[m];
+                for (int m = 0; m < 9; ++m) w[k][m] = (T)U[m];
+                w[k][9] = T(0);
+            } else {
+#pragma unroll
+                for (int m = 0; m < 10; ++m) w[k][m] = (T)wd[m];
+            }
             col[k] = arg.fin + c;
             // row of tap m of output row j is j + s + m - 4; rn = row of the next value the window has not seen
             rn[k] = jA + s - 4;
@@ -156,6 +165,10 @@ __global__ void __launch_bounds__((4 + NTW_) * 32, 1) strang_fused_ws_kernel(con
                 if (p_periodic && rn[k] >= np) rn[k] = 0;
             }
             v[k][9] = v[k][10] = v[k][11] = T(0);
+            if constexpr (sizeof(T) == 4) {
+#pragma unroll
+                for (int m = 0; m < 12; ++m) e[k][m] = m < 8 ? v[k][m + 1] - v[k][m] : T(0);
+            }
         }
 
         const uint32_t ring_u32 = ptx::smem_u32(ring) + (uint32_t)tid * (uint32_t)sizeof(T);
@@ -206,9 +219,17 @@ __global__ void __launch_bounds__((4 + NTW_) * 32, 1) strang_fused_ws_kernel(con
 #pragma unroll
                     for (int k = 0; k < CPT; ++k) {  // columns beyond NTA compute on whatever the ring holds: never read
                         v[k][(r + 9) % 12] = sl[r * PITCH + k * NPT];
-                        T acc = w[k][0] * v[k][r % 12];
+                        T acc;
+                        if constexpr (sizeof(T) == 4) {
+                            e[k][(r + 8) % 12] = v[k][(r + 9) % 12] - v[k][(r + 8) % 12];
+                            acc = v[k][(r + FD_C) % 12];
 #pragma unroll
-                        for (int m = 1; m < 10; ++m) acc = fma(w[k][m], v[k][(r + m) % 12], acc);
+                            for (int m = 0; m < 9; ++m) acc = fma(w[k][m], e[k][(r + m) % 12], acc);
+                        } else {
+                            acc = w[k][0] * v[k][r % 12];
+#pragma unroll
+                            for (int m = 1; m < 10; ++m) acc = fma(w[k][m], v[k][(r + m) % 12], acc);
+                        }
                         sl[r * PITCH + k * NPT] = acc;
                     }
                 }
@@ -318,26 +339,46 @@ __global__ void __launch_bounds__((4 + NTW_) * 32, 1) strang_fused_ws_kernel(con
         if (curS > S) shift_sums(std::integral_constant<int, 1>());
 
         T out[R];
-        {
-            const T W0 = (T)Wr[0];
+        if constexpr (sizeof(T) == 4) {
+            // fp32 arithmetic: difference form (diff_form_weights; the table holds U_0 .. U_{NTAP-2}), centre tap CT
+            constexpr int CT = NST == 2 ? 2 * FD_C + 1 : FD_C;
 #pragma unroll
-            for (int q = 0; q < R; ++q) out[q] = W0 * x[q];
-        }
+            for (int k = R + NH - 1; k < R + NTAP - 1; ++k) x[k] = grow[k];
+            __syncwarp();
+            if (lane == 0) ptx::mbar_arrive_u32(empty_u32 + boff);  // the ring row may be refilled
+            T d[R + NTAP - 2];
 #pragma unroll
-        for (int n = 1; n < NH; ++n) {
-            const T Wn = (T)Wr[n];
+            for (int k = 0; k < R + NTAP - 2; ++k) d[k] = x[k + 1] - x[k];
 #pragma unroll
-            for (int q = 0; q < R; ++q) out[q] = fma(Wn, x[q + n], out[q]);
-        }
+            for (int q = 0; q < R; ++q) out[q] = x[q + CT];
 #pragma unroll
-        for (int k = R + NH - 1; k < R + NTAP - 1; ++k) x[k] = grow[k];
-        __syncwarp();
-        if (lane == 0) ptx::mbar_arrive_u32(empty_u32 + boff);  // the ring row may be refilled
+            for (int n = 0; n < NTAP - 1; ++n) {
+                const T Wn = (T)Wr[n];
 #pragma unroll
-        for (int n = NH; n < NTAP; ++n) {
-            const T Wn = (T)Wr[n];
+                for (int q = 0; q < R; ++q) out[q] = fma(Wn, d[q + n], out[q]);
+            }
+        } else {
+            {
+                const T W0 = (T)Wr[0];
 #pragma unroll
-            for (int q = 0; q < R; ++q) out[q] = fma(Wn, x[q + n], out[q]);
+                for (int q = 0; q < R; ++q) out[q] = W0 * x[q];
+            }
+#pragma unroll
+            for (int n = 1; n < NH; ++n) {
+                const T Wn = (T)Wr[n];
+#pragma unroll
+                for (int q = 0; q < R; ++q) out[q] = fma(Wn, x[q + n], out[q]);
+            }
+#pragma unroll
+            for (int k = R + NH - 1; k < R + NTAP - 1; ++k) x[k] = grow[k];
+            __syncwarp();
+            if (lane == 0) ptx::mbar_arrive_u32(empty_u32 + boff);  // the ring row may be refilled
+#pragma unroll
+            for (int n = NH; n < NTAP; ++n) {
+                const T Wn = (T)Wr[n];
+#pragma unroll
+                for (int q = 0; q < R; ++q) out[q] = fma(Wn, x[q + n], out[q]);
+            }
         }
 
         if (nv == R) {

@@ -21,8 +21,10 @@ namespace vl {
 
 enum { BC_PERIODIC = 0, BC_ZERO = 1 };
 
-// per-row table of the theta half shift: {w_0..w_9, (double) s, 0}; 96 bytes = one 16-byte-aligned bulk copy
+// per-row table of the theta half shift: {w_0..w_9, (double) s, e}; 96 bytes = one 16-byte-aligned bulk copy.
+// For fp32 storage the ten entries are the nine difference-form weights U_0..U_8 (diff_form_weights) and a 0.
 constexpr int WROW_STRIDE = 12;
+constexpr int FD_C = 4;  // centre tap of the ten: w[FD_C] multiplies f[k]
 
 // eq (16), divided by 6 (the 1/6 of gamma, delta in eq (14)); index m+4, m = -4..4
 __host__ __device__ inline double c16_over_6(int m) {
@@ -48,6 +50,54 @@ __host__ __device__ inline void spline_fd8_weights(double a, double w[10]) {
         if (m == 0) v += al;
         if (m == 1) v += a;
         w[mm] = v;
+    }
+}
+
+// fp32 arithmetic runs every filter in DIFFERENCE FORM.  With n weights that add up to 1 and centre tap c,
+//     sum_m w_m x_m = x_c + sum_{j=0}^{n-2} U_j (x_{j+1} - x_j),   U_j = -sum_{m<=j} w_m (j < c),  U_j = sum_{m>j} w_m (j >= c).
+// Why: in the plain form the partial sums of a float accumulation are of the size of f itself and their rounding
+// errors add up to more than half an ulp; on a plateau of f (the water-bags of cfg 1, 3, 4, 5) every point of a line
+// then gets the SAME error, step after step (the weights of a row never change), so the mass of the line, the moments
+// (M_x, M_y), the force and the feet of all characteristics drift coherently: at 8192^2 the fp32 path left north_star's
+// 1e-4 max|f| after 30 steps (7.6e-4 after 100; measured in round 2).  In difference form a plateau is reproduced
+// exactly (all differences are 0) and elsewhere the rounding errors scale with the local variation of f, not with f.
+// fp64 keeps the plain ten-tap form (its rounding is 1e-9 of the tolerance).  U has n - 1 entries.
+__host__ __device__ inline void diff_form_weights(const double* w, int n, int c, double* U) {
+    double acc = 0.0;
+    for (int j = 0; j < c; ++j) {
+        acc -= w[j];
+        U[j] = acc;
+    }
+    acc = 0.0;
+    for (int j = n - 2; j >= c; --j) {
+        acc += w[j + 1];
+        U[j] = acc;
+    }
+}
+
+// R consecutive outputs of an NT-tap filter from the window x[0 .. R + NT - 1): out[r] = sum_m w[m] x[r + m] (fp64), or
+// in difference form with w[0 .. NT - 1) = U and centre tap C (fp32)
+template <typename T, int R, int NT, int C>
+__device__ __forceinline__ void fir_window(const T* w, const T* x, T* out) {
+    if constexpr (sizeof(T) == 4) {
+        T e[R + NT - 2];
+#pragma unroll
+        for (int k = 0; k < R + NT - 2; ++k) e[k] = x[k + 1] - x[k];
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            T acc = x[r + C];
+#pragma unroll
+            for (int jj = 0; jj < NT - 1; ++jj) acc = fma(w[jj], e[r + jj], acc);
+            out[r] = acc;
+        }
+    } else {
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            T acc = w[0] * x[r];
+#pragma unroll
+            for (int m = 1; m < NT; ++m) acc = fma(w[m], x[r + m], acc);
+            out[r] = acc;
+        }
     }
 }
 
@@ -166,13 +216,7 @@ __global__ void __launch_bounds__(384) theta_sweep_generic_kernel(const ThetaArg
         for (int k = 0; k < R + 9; ++k) v[k] = A[myq + k];
 
         T g[R];
-#pragma unroll
-        for (int r = 0; r < R; ++r) {
-            T acc = w[0] * v[r];
-#pragma unroll
-            for (int m = 1; m < 10; ++m) acc = fma(w[m], v[r + m], acc);
-            g[r] = acc;
-        }
+        fir_window<T, R, 10, FD_C>(w, v, g);
 
         T out[R];
         if (NSTAGE == 2) {
@@ -188,13 +232,7 @@ __global__ void __launch_bounds__(384) theta_sweep_generic_kernel(const ThetaArg
                 h[r] = g[r];
                 h[R + r] = __shfl_down_sync(0xffffffffu, g[r], 1);
             }
-#pragma unroll
-            for (int r = 0; r < R; ++r) {
-                T acc = w[0] * h[r];
-#pragma unroll
-                for (int m = 1; m < 10; ++m) acc = fma(w[m], h[r + m], acc);
-                out[r] = acc;
-            }
+            fir_window<T, R, 10, FD_C>(w, h, out);
         } else {
 #pragma unroll
             for (int r = 0; r < R; ++r) out[r] = g[r];
@@ -276,8 +314,16 @@ __global__ void __launch_bounds__(256) p_sweep_kernel(const PArgs<T> arg) {
     double wd[10];
     spline_fd8_weights(a, wd);
     T w[10];
+    if (sizeof(T) == 4) {  // fp32 arithmetic: difference form (diff_form_weights)
+        double U[9];
+        diff_form_weights(wd, 10, FD_C, U);
 #pragma unroll
-    for (int m = 0; m < 10; ++m) w[m] = (T)wd[m];
+        for (int m = 0; m < 9; ++m) w[m] = (T)U[m];
+        w[9] = T(0);
+    } else {
+#pragma unroll
+        for (int m = 0; m < 10; ++m) w[m] = (T)wd[m];
+    }
 
     const T* __restrict__ col = arg.fin + i;
     T* __restrict__ ocol = arg.fout + i;
@@ -286,12 +332,14 @@ __global__ void __launch_bounds__(256) p_sweep_kernel(const PArgs<T> arg) {
     int rbase = j0 + s - 4;
     if (periodic) rbase = wrap_index(rbase, np);
 
-    T v[10];
+    T v[10], e[10];  // e (fp32 only): e[k] = v[k + 1] - v[k] of the window, kept as a ring like v
 #pragma unroll
     for (int k = 0; k < 9; ++k) {
         v[k] = load_row(col, rbase + k, np, pitch, periodic);
     }
     v[9] = T(0);
+#pragma unroll
+    for (int k = 0; k < 10; ++k) e[k] = k < 8 ? v[k + 1] - v[k] : T(0);
     int rnext = rbase + 9;  // row of the next new tap
     if (periodic) rnext = rnext % np;
 
@@ -315,9 +363,17 @@ __global__ void __launch_bounds__(256) p_sweep_kernel(const PArgs<T> arg) {
 #pragma unroll
         for (int k = 0; k < 10; ++k) {
             v[(k + 9) % 10] = cur[k];
-            T acc = w[0] * v[k % 10];
+            T acc;
+            if (sizeof(T) == 4) {
+                e[(k + 8) % 10] = v[(k + 9) % 10] - v[(k + 8) % 10];
+                acc = v[(k + FD_C) % 10];
 #pragma unroll
-            for (int m = 1; m < 10; ++m) acc = fma(w[m], v[(k + m) % 10], acc);
+                for (int m = 0; m < 9; ++m) acc = fma(w[m], e[(k + m) % 10], acc);
+            } else {
+                acc = w[0] * v[k % 10];
+#pragma unroll
+                for (int m = 1; m < 10; ++m) acc = fma(w[m], v[(k + m) % 10], acc);
+            }
             if (jb + k < j1) ocol[(size_t)(jb + k) * pitch] = acc;
         }
     }
@@ -497,7 +553,9 @@ __global__ void __launch_bounds__(RR_COLS* RR_GROUPS)
             for (int q = 0; q < RR_GROUPS; ++q) acc += part[q][c];
             acc *= dp;
             rho[i] = acc;
+            __threadfence();  // every lane's rho is released before thread 0 takes the ticket
         }
+        __syncwarp();
         if (mpart != nullptr) {
             double cs = (i < ntheta) ? cos_t[i] * acc : 0.0;
             double ss = (i < ntheta) ? sin_t[i] * acc : 0.0;

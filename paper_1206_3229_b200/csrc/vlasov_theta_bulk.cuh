@@ -156,13 +156,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
         }
 
         T g[R];
-#pragma unroll
-        for (int r = 0; r < R; ++r) {
-            T acc = w[0] * v[r];
-#pragma unroll
-            for (int m = 1; m < 10; ++m) acc = fma(w[m], v[r + m], acc);
-            g[r] = acc;
-        }
+        fir_window<T, R, 10, FD_C>(w, v, g);
 
         T out[R];
         if (NSTAGE == 2) {
@@ -177,13 +171,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB)
             for (int r = 0; r < R; ++r) h[r] = g[r];
 #pragma unroll
             for (int r = 0; r < 9; ++r) h[R + r] = __shfl_down_sync(0xffffffffu, g[r], 1);
-#pragma unroll
-            for (int r = 0; r < R; ++r) {
-                T acc = w[0] * h[r];
-#pragma unroll
-                for (int m = 1; m < 10; ++m) acc = fma(w[m], h[r + m], acc);
-                out[r] = acc;
-            }
+            fir_window<T, R, 10, FD_C>(w, h, out);
         } else {
 #pragma unroll
             for (int r = 0; r < R; ++r) out[r] = g[r];

@@ -2,7 +2,7 @@
 of the CUDA path against the CPU oracle, element by element, through the C ABI.
 
 The two sides share nothing: the oracle solves the cyclic tridiagonal system of every line (Thomas + Sherman-
-Morrison) and evaluates eq (13); the CUDA kernels apply the 60-tap filter of the truncated closed-form inverse.
+Morrison) and evaluates eq (13); the CUDA kernels run the closed-form inverse as two first-order recursions.
 Tolerances as for the FD path (north_star): fp64 max|df| <= 1e-10 max|f| after 100 steps, moments to 1e-10.
 """
 from __future__ import annotations
@@ -34,21 +34,10 @@ def rough_state(nt, npp, dom, seed=1):
     return f + 0.1 * rng.random((npp, nt))
 
 
-GSFIR = 0  # which GPU kernels: 0 = the recursive ones (default), 1 = the 60-tap filter kernels (tune_gsfir)
-
-
-@pytest.fixture(autouse=True, params=[0, 1], ids=["recursive", "fir"])
-def gs_kernel_variant(request):
-    global GSFIR
-    GSFIR = request.param
-    yield
-    GSFIR = 0
-
-
 def pair(model, grid, dom, dt, f0, threads=8, precision=64, **params):
     o = Oracle(model, grid, dom, dt, threads=threads, spline=SPLINE_GS, **params)
     o.upload(f0)
-    g = vb.Vlasov(model, grid, dom, dt, precision=precision, spline=vb.SPLINE_GS, tune_gsfir=GSFIR, **params)
+    g = vb.Vlasov(model, grid, dom, dt, precision=precision, spline=vb.SPLINE_GS, **params)
     g.upload(f0)
     return o, g
 
@@ -109,7 +98,7 @@ def test_gs_integer_cell_shifts_are_exact_copies():
     nt, npp = 128, 64
     dom = (0.0, float(nt), -4.0, 4.0)          # dx = 1; p_j tau integer for tau = 8: p_j = -4 + j/8
     f0 = rough_state(nt, npp, dom, seed=7)
-    g = vb.Vlasov(MODEL_FREE, (nt, npp), dom, 16.0, spline=vb.SPLINE_GS, tune_gsfir=GSFIR)
+    g = vb.Vlasov(MODEL_FREE, (nt, npp), dom, 16.0, spline=vb.SPLINE_GS)
     g.upload(f0)
     g.substep(vb.SUB_THETA_HALF)
     out = g.download()
@@ -151,7 +140,7 @@ def test_gs_differs_from_fd_and_history_matches():
     gf.step(10)
     f_fd = gf.download()
     gf.close()
-    g2 = vb.Vlasov(c["model"], c["grid"], c["domain"], c["dt"], spline=vb.SPLINE_GS, history=1, tune_gsfir=GSFIR)
+    g2 = vb.Vlasov(c["model"], c["grid"], c["domain"], c["dt"], spline=vb.SPLINE_GS, history=1)
     g2.upload(c["f0"])
     g2.step(10)
     hist = g2.history(10)
@@ -174,10 +163,15 @@ def test_gs_fp32_storage():
 
 
 def test_gs_refuses_short_axes():
-    g = vb.Vlasov(MODEL_HMF, (31, 64), (-PI, PI, -4.0, 4.0), 0.1, spline=vb.SPLINE_GS, attach=False)
-    with pytest.raises(vb.VlasovError):
-        g.step(1)
-    g.close()
+    """vlasov_set_param itself refuses SPLINE = 1 on an axis shorter than 32 nodes (before anything is allocated), the
+    context stays usable with the default spline, and a retry does not leak"""
+    for grid in ((31, 64), (64, 8)):
+        for _ in range(3):
+            with pytest.raises(vb.VlasovError) as e:
+                vb.Vlasov(MODEL_HMF, grid, (-PI, PI, -4.0, 4.0), 0.1, spline=vb.SPLINE_GS, attach=False)
+            assert e.value.code == vb.EINVAL
+        vb.vlasov_step(1)  # the context of the failed constructor is initialised and runs with the eq (16) spline
+        vb.vlasov_free()
 
 
 def test_gs_at_2048_first_steps_then_22_steps():
@@ -204,7 +198,7 @@ def run_both_gs(c, steps):
     o.step(steps)
     fo, mo = o.download(), o.moments()
     o.close()
-    g = vb.Vlasov(c["model"], c["grid"], c["domain"], c["dt"], spline=vb.SPLINE_GS, tune_gsfir=GSFIR, **c["params"])
+    g = vb.Vlasov(c["model"], c["grid"], c["domain"], c["dt"], spline=vb.SPLINE_GS, **c["params"])
     g.upload(c["f0"])
     g.step(steps)
     fg, mg = g.download(), g.moments()
@@ -223,9 +217,9 @@ def test_gs_full_size_steps_match_oracle(name, kw, steps):
     assert np.max(np.abs(mg - mo)) <= 1e-10 * max(1.0, np.max(np.abs(mo)))
 
 
-def test_gs_bench_size_first_steps_match_oracle():
-    """8192^2 in the configuration bench.py --spline gs times: two steps element by element"""
+def test_gs_bench_size_20_steps_match_oracle():
+    """8192^2 in the configuration bench.py --spline gs times: 20 steps element by element"""
     c = inputs.config("cfg5", n=8192)
-    fo, mo, fg, mg = run_both_gs(c, 2)
-    assert rel_err(fg, fo) <= 1e-12
-    assert np.max(np.abs(mg - mo)) <= 1e-11
+    fo, mo, fg, mg = run_both_gs(c, 20)
+    assert rel_err(fg, fo) <= 1e-10
+    assert np.max(np.abs(mg - mo)) <= 1e-10 * max(1.0, np.max(np.abs(mo)))

@@ -117,19 +117,18 @@ def test_density_after_theta_sweep_epilogue():
 ONEPASS_GRIDS = [(64, 48), (352, 30), (353, 61), (1000, 137), (2233, 25), (31, 9), (1, 5), (7, 1), (720, 700)]
 
 
-@pytest.mark.parametrize("fvariant", [0, 1])
 @pytest.mark.parametrize("grid", ONEPASS_GRIDS)
 @pytest.mark.parametrize("bc_p", [BC_ZERO, BC_PERIODIC])
 @pytest.mark.parametrize("which,dt,amp", [(1, 0.1, 0.5), (2, 0.1, 0.5), (2, -0.37, 30.0), (1, 9.0, 2000.0),
                                           (2, 9.0, 30.0), (2, 3.0, 0.0)])
-def test_one_pass_p_then_theta(grid, bc_p, which, dt, amp, fvariant):
+def test_one_pass_p_then_theta(grid, bc_p, which, dt, amp):
     """p shift with a given force, then one or two half theta shifts, then density and force of the result:
     the one-pass kernel against the oracle's separate sweeps (eqs (11), (12), (9), (10))."""
     dom = (-PI, PI, -4.0, 4.0)
     f0 = smooth_state(grid[0], grid[1], dom, seed=5)
     th = inputs.nodes(dom[0], dom[1], grid[0])
     F = amp * np.sin(2 * th + 0.1) + 0.3 * amp
-    o, g = pair(MODEL_HMF, grid, dom, dt, f0, bc_p=bc_p, gpu_params=dict(tune_fvariant=fvariant))
+    o, g = pair(MODEL_HMF, grid, dom, dt, f0, bc_p=bc_p)
     o.p_sweep(dt, force=F)
     for _ in range(which):
         o.theta_sweep(0.5 * dt)
@@ -312,6 +311,24 @@ def test_graph_launches_change_nothing():
         g.close()
     assert np.array_equal(outs[0], outs[1])
     assert launches[0] == launches[1] == (1 + 2 * 9) + (1 + 2 * 4)
+
+
+def test_non_blocking_stream_can_be_attached():
+    """Every torch.cuda.Stream() is a non-blocking stream: nothing orders it after the legacy default stream on which
+    vlasov_init's tables are uploaded and its counters zeroed; the library synchronises once before the first launch."""
+    import torch
+
+    c = inputs.config("cfg5", ntheta=1100, npts=640)
+    outs = []
+    for own_stream in (False, True):
+        s = torch.cuda.Stream() if own_stream else torch.cuda.current_stream()
+        with torch.cuda.stream(s):
+            g = vb.Vlasov(c["model"], c["grid"], c["domain"], c["dt"])
+            g.upload(c["f0"])
+            g.step(6)
+            outs.append((g.download(), g.moments()))
+            g.close()
+    assert np.array_equal(outs[0][0], outs[1][0]) and np.array_equal(outs[0][1], outs[1][1])
 
 
 def test_library_owned_buffers_and_checkpoint_roundtrip():

@@ -460,7 +460,25 @@ def test_p14_ring_waterbag_closed_form():
     assert np.max(np.abs(F[sel] - ref[sel])) < 2e-2
     i14 = int(round((1.4 + PI) / (2 * PI / n)))
     assert F[i14] == pytest.approx(-1.75730, abs=2e-2)
-    assert V(0.0) == pytest.approx(-7.07107, abs=1e-5) and V(PI) == pytest.approx(-0.498755, abs=1e-6)
+
+
+def test_p14_ring_potential_table_from_point_masses():
+    """V(0) = -1/(sqrt2 sqrt(eps)) = -7.07107 and V(pi) = -1/(sqrt2 sqrt(2 + eps)) = -0.498755 (eq (2), eps =
+    0.01) read back from the ORACLE's potential energy: with all the density in one column k, rho_i = c delta_ik,
+    U = (1/2) dtheta^2 c^2 V(0); with two equal columns half a circle apart U = dtheta^2 c^2 (V(0) + V(pi))."""
+    n, npp, eps = 64, 16, 0.01
+    dom = (-PI, PI, -1.0, 1.0)
+    dth, dp = 2 * PI / n, 2.0 / npp
+    f = np.zeros((npp, n))
+    f[:, 5] = 1.0
+    c = npp * dp                      # rho_5 = dp * sum_j f = 2
+    U1 = run(MODEL_RING, (n, npp), dom, 0.1, f, eps=eps).moments()[4]
+    V0 = 2.0 * U1 / (dth * c) ** 2
+    assert V0 == pytest.approx(-7.07107, abs=1e-5)
+    f[:, 5 + n // 2] = 1.0
+    U2 = run(MODEL_RING, (n, npp), dom, 0.1, f, eps=eps).moments()[4]
+    Vpi = U2 / (dth * c) ** 2 - V0
+    assert Vpi == pytest.approx(-0.498755, abs=1e-6)
 
 
 def test_p14_ring_potential_energy_of_waterbag():

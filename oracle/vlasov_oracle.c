@@ -77,7 +77,7 @@
 
 enum { MODEL_FREE = 0, MODEL_HMF = 1, MODEL_RING = 2, MODEL_SHEET = 3 };
 enum { BC_PERIODIC = 0, BC_ZERO = 1 };
-enum { KEY_EPS = 1, KEY_PRECISION = 2, KEY_BC_X = 3, KEY_BC_P = 4, KEY_HISTORY = 5, KEY_SPLINE = 6 };
+enum { KEY_EPS = 1, KEY_PRECISION = 2, KEY_BC_X = 3, KEY_BC_P = 4, KEY_HISTORY = 5, KEY_SPLINE = 6, KEY_ORDER = 7 };
 enum { SPLINE_FD = 0, SPLINE_GS = 1 };
 
 /* eq (16): coefficients of f(u_{i-4}) ... f(u_{i+4}). */
@@ -311,6 +311,7 @@ typedef struct {
     double xmin, xmax, pmin, pmax, dt, eps, t;
     int bc_x, bc_p;
     int spline; /* SPLINE_FD (eq 16, default) or SPLINE_GS (system 15) */
+    int order;  /* 2: the paper's time split (L71-L87); 4: its triple-jump composition (L238, refs [31], [44]) */
     double* f;
 } ctx_t;
 
@@ -339,6 +340,7 @@ int oracle_init(int model, const int grid[2], const double domain[4], double dt)
     G.bc_x = (model == MODEL_SHEET) ? BC_ZERO : BC_PERIODIC;
     G.bc_p = BC_ZERO;
     G.spline = SPLINE_FD;
+    G.order = 2;
     G.f = (double*)calloc((size_t)G.nx * (size_t)G.np, sizeof(double));
     if (!G.f) return ORACLE_ENOMEM;
     G.ready = 1;
@@ -354,6 +356,7 @@ int oracle_set_param(int key, double value) {
         case KEY_BC_P: if (value != 0.0 && value != 1.0) return ORACLE_EINVAL; G.bc_p = (int)value; break;
         case KEY_HISTORY: break;
         case KEY_SPLINE: if (value != 0.0 && value != 1.0) return ORACLE_EINVAL; G.spline = (int)value; break;
+        case KEY_ORDER: if (value != 2.0 && value != 4.0) return ORACLE_EINVAL; G.order = (int)value; break;
         default: return ORACLE_EINVAL;
     }
     return ORACLE_OK;
@@ -454,14 +457,34 @@ int oracle_p_sweep(double dt) {
     return rc;
 }
 
-/* n time steps, each (1)-(4) of section 3 (L71-L87) */
+/* one time-split step (1)-(4) of section 3 (L71-L87) over the time h (h may be negative) */
+static void strang_step(double h) {
+    oracle_theta_sweep(0.5 * h); /* (1) eq (9)  */
+    oracle_p_sweep(h);           /* (2)+(3) eqs (10), (11) */
+    oracle_theta_sweep(0.5 * h); /* (4) eq (12) */
+}
+
+/*
+ * n time steps.  order 2 (default): each step is (1)-(4) of section 3 (L71-L87).
+ * order 4 ("Higher order time split schemes ... can also be implemented if required",
+ * PAPER.md L238 with ref. [31]): the paper gives no formula, so the reading (D23) is the standard
+ * fourth-order composition of a symmetric second-order step S2, the "triple jump" of the paper's own ref. [44]
+ * (Yoshida 1990, cited at L206 for the N-body integrator):
+ *     S4(dt) = S2(g1 dt) S2(g2 dt) S2(g1 dt),   g1 = 1/(2 - 2^(1/3)),  g2 = 1 - 2 g1 = -2^(1/3)/(2 - 2^(1/3)),
+ * whose middle sub-step runs backwards in time (g2 < 0).  Each S2 is the unchanged step (1)-(4), force included.
+ */
 int oracle_step(int n) {
     if (!G.ready) return ORACLE_ENOTINIT;
     if (n <= 0) return ORACLE_EINVAL;
+    const double g1 = 1.0 / (2.0 - cbrt(2.0)), g2 = 1.0 - 2.0 * g1;
     for (int it = 0; it < n; ++it) {
-        oracle_theta_sweep(0.5 * G.dt); /* (1) eq (9)  */
-        oracle_p_sweep(G.dt);           /* (2)+(3) eqs (10), (11) */
-        oracle_theta_sweep(0.5 * G.dt); /* (4) eq (12) */
+        if (G.order == 4) {
+            strang_step(g1 * G.dt);
+            strang_step(g2 * G.dt);
+            strang_step(g1 * G.dt);
+        } else {
+            strang_step(G.dt);
+        }
         G.t += G.dt;
     }
     return ORACLE_OK;

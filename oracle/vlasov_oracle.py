@@ -18,7 +18,7 @@ _LIB = os.path.join(_HERE, "libvlasov_oracle.so")
 
 MODEL_FREE, MODEL_HMF, MODEL_RING, MODEL_SHEET = 0, 1, 2, 3
 BC_PERIODIC, BC_ZERO = 0, 1
-KEY_EPS, KEY_PRECISION, KEY_BC_X, KEY_BC_P, KEY_HISTORY, KEY_SPLINE = 1, 2, 3, 4, 5, 6
+KEY_EPS, KEY_PRECISION, KEY_BC_X, KEY_BC_P, KEY_HISTORY, KEY_SPLINE, KEY_ORDER = 1, 2, 3, 4, 5, 6, 7
 SPLINE_FD, SPLINE_GS = 0, 1
 GS_EXT = 64
 
@@ -135,7 +135,7 @@ class Oracle:
         _check(self.lib.oracle_init(int(model), g, d, float(dt)), "init")
         self.lib.oracle_set_threads(int(threads))
         for k, v in params.items():
-            key = {"eps": KEY_EPS, "bc_x": KEY_BC_X, "bc_p": KEY_BC_P, "spline": KEY_SPLINE}[k]
+            key = {"eps": KEY_EPS, "bc_x": KEY_BC_X, "bc_p": KEY_BC_P, "spline": KEY_SPLINE, "order": KEY_ORDER}[k]
             _check(self.lib.oracle_set_param(key, float(v)), "set_param")
 
     @property

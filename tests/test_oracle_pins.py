@@ -507,6 +507,56 @@ def test_p15_strang_splitting_is_second_order():
     assert 3.3 < e1 / e2 < 4.8 and 3.3 < e2 / e3 < 4.8
 
 
+# --------------------------------------------------------------------------- P21: fourth-order composition (NEXT #4)
+def test_p21_triple_jump_composition_is_fourth_order():
+    """order = 4 (refs [31], [44]; D23): on smooth data the error of M_x(t = 1) against a fine-step
+    run falls by 2^4 per halving of dt (a wrong coefficient, a missing sub-step or a Lie-split ordering gives 4 or 2),
+    and it is far below the second-order step's at the same dt."""
+    n = 256  # fine enough for the interpolation error (1e-7 here) to stay below the time-splitting error
+    dom = (-PI, PI, -5.0, 5.0)
+    th = inputs.nodes(dom[0], dom[1], n)
+    p = inputs.nodes(dom[2], dom[3], n)
+    f0 = inputs.perturbed_gaussian(th, p, 0.4, 0.3)
+
+    def M_at_1(dt, order):
+        o = run(MODEL_HMF, (n, n), dom, dt, f0, steps=int(round(1.0 / dt)), threads=8, order=order)
+        return o.moments()[5]
+
+    ref = M_at_1(1.0 / 128, 4)
+    e1, e2, e3 = (abs(M_at_1(dt, 4) - ref) for dt in (1.0, 0.5, 0.25))
+    assert 10.0 < e1 / e2 < 24.0 and 10.0 < e2 / e3 < 24.0, (e1, e2, e3)
+    assert e3 < 0.1 * abs(M_at_1(0.25, 2) - ref)
+
+
+def test_p21_order4_step_is_three_strang_steps_with_the_triple_jump_coefficients():
+    """S4(dt) = S2(g1 dt) S2(g2 dt) S2(g1 dt) with g1 = 1/(2 - 2^(1/3)), g2 = 1 - 2 g1 (so that 2 g1 + g2 = 1 and
+    2 g1^3 + g2^3 = 0): composed here from three second-order oracles whose dt is set from the closed form."""
+    g1 = 1.0 / (2.0 - 2.0 ** (1.0 / 3.0))
+    g2 = 1.0 - 2.0 * g1
+    assert abs(2 * g1 ** 3 + g2 ** 3) < 1e-15 and g2 < 0
+    c = inputs.config("cfg1", ntheta=48, npts=40)
+    o4 = run(c["model"], c["grid"], c["domain"], c["dt"], c["f0"], steps=2, order=4)
+    f4, t4 = o4.download(), o4.moments()[0]  # the oracle is a singleton: read it before the next one is made
+    f = c["f0"]
+    for _ in range(2):
+        for g in (g1, g2, g1):
+            f = run(c["model"], c["grid"], c["domain"], g * c["dt"], f, steps=1).download()
+    assert np.max(np.abs(f4 - f)) <= 1e-15 * np.max(np.abs(f))
+    assert t4 == pytest.approx(2 * c["dt"])
+
+
+def test_p21_order4_free_streaming_moves_by_p_dt():
+    """F = 0: the three sub-steps displace row j by (2 g1 + g2) p_j dt = p_j dt in all; against the analytic
+    f0(theta - p t, p) on one Fourier mode (a sub-step with a wrong sign or weight misses by O(1))"""
+    n, npp = 128, 16
+    dom = (-PI, PI, -2.0, 2.0)
+    th, p = inputs.nodes(dom[0], dom[1], n), inputs.nodes(dom[2], dom[3], npp)
+    f0 = 1.0 + 0.5 * np.cos(th)[None, :] * np.ones(npp)[:, None]
+    out = run(MODEL_FREE, (n, npp), dom, 0.7, f0, steps=3, order=4).download()
+    ref = 1.0 + 0.5 * np.cos(th[None, :] - p[:, None] * 2.1)
+    assert np.max(np.abs(out - ref)) < 1e-6
+
+
 # --------------------------------------------------------------------------- P16: zero extension
 @pytest.mark.parametrize("cells", [0.4, -3.6, 9.25, -70.5, 200.0])
 def test_p16_zero_extension_equals_periodic_on_padded_line(cells):

@@ -175,7 +175,7 @@ def workload(args, with_f0=True):
         "workload": "%s %s %dx%d %s, dt=%g, %s, p zero-extended%s" % (
             args.config, MODEL_NAMES[c["model"]], nt, npp, "fp64" if eb == 8 else "fp32", c["dt"], bc,
             ", global-spline variant (system 15)" if args.spline == "gs" else ""),
-        "cfg": args.config, "grid": [nt, npp], "precision": args.precision, "spline": args.spline,
+        "cfg": args.config, "grid": [nt, npp], "precision": args.precision, "spline": args.spline, "order": args.order,
         "l2": "state fits L2: DRAM roofline not claimed" if fits else
               "state (%.0f MiB x 2 buffers) exceeds the 126 MB L2; no flush needed" % (nt * npp * eb / 2 ** 20),
     }
@@ -183,21 +183,23 @@ def workload(args, with_f0=True):
 
 
 # ------------------------------------------------------------------------------------------ oracle legs
-def make_oracle(c, spline: int):
+def make_oracle(c, spline: int, order: int = 2):
     import oracle
 
     cores = os.cpu_count() or 1
     params = dict(c["params"])
     if spline:
         params["spline"] = spline
+    if order == 4:
+        params["order"] = 4
     o = oracle.Oracle(c["model"], c["grid"], c["domain"], c["dt"], threads=cores, **params)
     o.upload(c["f0"])
     return o
 
 
-def oracle_throughput(c, steps: int, min_seconds: float = 0.0, spline: int = 0):
+def oracle_throughput(c, steps: int, min_seconds: float = 0.0, spline: int = 0, order: int = 2):
     """Gpts/s of the CPU oracle on the workload c, all host cores: `steps` at a time until min_seconds have passed"""
-    o = make_oracle(c, spline)
+    o = make_oracle(c, spline, order)
     pts = float(c["grid"][0]) * float(c["grid"][1])
     done, t0 = 0, time.perf_counter()
     while True:
@@ -221,7 +223,7 @@ def run_reference(args):
     c, cfg = workload(args)
     pts = float(c["grid"][0]) * float(c["grid"][1])
     t_wall = time.perf_counter()
-    o = make_oracle(c, int(args.spline == "gs"))
+    o = make_oracle(c, int(args.spline == "gs"), args.order)
     t0 = time.perf_counter()
     o.step(1)                      # first step: untimed warm-up (page faults of the oracle's arrays) and the estimate
     t1 = time.perf_counter() - t0
@@ -284,6 +286,8 @@ def run_cuda(args):
     params.update(fuse=args.fuse, tune_graph=args.graph)
     if args.spline == "gs":
         params["spline"] = vb.SPLINE_GS
+    if args.order == 4:
+        params["order"] = 4
     if args.fbands > 0:
         params["tune_fbands"] = args.fbands
     g = vb.Vlasov(c["model"], c["grid"], c["domain"], c["dt"], precision=prec, device="cuda:%d" % local_rank, **params)
@@ -393,7 +397,7 @@ def run_cuda(args):
     # ---- oracle on the host cores (bounded sample of the same workload), rank 0 only
     cpu = None
     if not args.no_cpu_baseline:
-        val, el, done, threads = oracle_throughput(c, 1, min_seconds=args.cpu_seconds, spline=int(args.spline == "gs"))
+        val, el, done, threads = oracle_throughput(c, 1, min_seconds=args.cpu_seconds, spline=int(args.spline == "gs"), order=args.order)
         cpu = {"value": val, "unit": UNIT, "cores": threads, "kind": "oracle",
                "sample": "%d Strang step(s) of the same workload on its full %dx%d grid (%.1f s of wall time), "
                          "oracle/vlasov_oracle.c with OpenMP over lines" % (done, nt, npp, el)}
@@ -453,6 +457,9 @@ def main():
     ap.add_argument("--spline", default="fd", choices=["fd", "gs"],
                     help="fd: f'' by eq (16), the paper's method and the headline workload; gs: the Global Spline "
                          "comparator, system (15) (SURVEY 8(f) NEXT #2)")
+    ap.add_argument("--order", type=int, default=2, choices=[2, 4],
+                    help="2: the paper's time split (headline); 4: its triple-jump composition (SURVEY 8(f) NEXT #4), "
+                         "nine passes and three force evaluations per step")
     args = ap.parse_args()
     _, _, world = dist_env()
     if args.gpus != world:

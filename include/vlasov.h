@@ -63,6 +63,11 @@ extern "C" {
                                   diagonal 2/3, D22).  Three passes per step; the solve is replaced by
                                   its closed-form inverse (two first-order recursions per line; or, with tuning
                                   key 110, a 60-tap filter); both axes need >= 32 nodes                          */
+#define VLASOV_KEY_ORDER 9     /* order of the time splitting: 2 (default) the paper's steps (1)-(4), L71-L87; 4: their
+                                  triple-jump composition S2(g1 dt) S2(g2 dt) S2(g1 dt), g1 = 1/(2 - 2^(1/3)), g2 = 1 - 2 g1
+                                  ("higher order time split schemes", L238 with refs [31], [44]):
+                                  three times the passes and force evaluations of a step, the middle sub-step
+                                  backwards in time; eq (16) spline only                                          */
 /* keys 101..110 (launch-shape overrides: warps, bands, segment lengths, kernel variant) exist for the tests and
  * the tuning sweeps only; see binding.py KEY_TUNE_*.  Results never depend on them beyond rounding order.   */
 

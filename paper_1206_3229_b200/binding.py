@@ -17,7 +17,7 @@ import numpy as np
 from . import build as _build
 
 MODEL_FREE, MODEL_HMF, MODEL_RING, MODEL_SHEET = 0, 1, 2, 3
-KEY_EPS, KEY_PRECISION, KEY_BC_X, KEY_BC_P, KEY_HISTORY, KEY_FUSE, KEY_PROFILE, KEY_SPLINE = 1, 2, 3, 4, 5, 6, 7, 8
+KEY_EPS, KEY_PRECISION, KEY_BC_X, KEY_BC_P, KEY_HISTORY, KEY_FUSE, KEY_PROFILE, KEY_SPLINE, KEY_ORDER = 1, 2, 3, 4, 5, 6, 7, 8, 9
 SPLINE_FD, SPLINE_GS = 0, 1
 KEY_TUNE_NW1, KEY_TUNE_NW2, KEY_TUNE_BANDS, KEY_TUNE_PSEG, KEY_TUNE_PTX, KEY_TUNE_GENERIC, KEY_TUNE_FBANDS, KEY_TUNE_GRAPH = 101, 102, 103, 104, 105, 106, 107, 109
 SUB_THETA_HALF, SUB_FORCE, SUB_P_FULL, SUB_THETA_TWICE, SUB_P_THETA_HALF, SUB_P_THETA_TWICE = 0, 1, 2, 3, 4, 5
@@ -237,7 +237,7 @@ class Vlasov:
         vlasov_init(model, grid, domain, dt)
         if precision != 64:
             vlasov_set_param(KEY_PRECISION, precision)
-        keys = {"eps": KEY_EPS, "bc_x": KEY_BC_X, "bc_p": KEY_BC_P, "history": KEY_HISTORY, "fuse": KEY_FUSE, "profile": KEY_PROFILE, "spline": KEY_SPLINE,
+        keys = {"eps": KEY_EPS, "bc_x": KEY_BC_X, "bc_p": KEY_BC_P, "history": KEY_HISTORY, "fuse": KEY_FUSE, "profile": KEY_PROFILE, "spline": KEY_SPLINE, "order": KEY_ORDER,
                 "tune_nw1": KEY_TUNE_NW1, "tune_nw2": KEY_TUNE_NW2, "tune_bands": KEY_TUNE_BANDS,
                 "tune_pseg": KEY_TUNE_PSEG, "tune_ptx": KEY_TUNE_PTX, "tune_generic": KEY_TUNE_GENERIC,
                 "tune_fbands": KEY_TUNE_FBANDS, "tune_graph": KEY_TUNE_GRAPH}

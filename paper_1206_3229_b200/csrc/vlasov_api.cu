@@ -44,6 +44,10 @@ struct Ctx {
     double xmin = 0, xmax = 0, pmin = 0, pmax = 0, dt = 0, eps = 0.01, t = 0;
     int bc_x = 0, bc_p = 1, prec = 64;
     int spline = 0;  // 0: f'' by eq (16) (the paper's method), 1: global spline, system (15) (vlasov_gs.cuh)
+    int order = 2;   // 2: the paper's time split; 4: its triple-jump composition S2(g1 dt) S2(g2 dt) S2(g1 dt) (L238)
+    double dt_sub = 0;                                 // time step of the sub-step being enqueued (= dt for order 2)
+    int* srow_sub[2] = {nullptr, nullptr};            // order 4: row tables of the sub-steps g1 dt, g2 dt
+    double* wrow_sub[2] = {nullptr, nullptr};
     double* gsab = nullptr;          // [Np][4] = 1-a, a, A/6, B/6 of a half theta shift
     int gs_rbands = 0, gs_rrpb = 0;  // bands of the global-spline theta kernel
     bool history = false;
@@ -158,7 +162,7 @@ int cdiv(int a, int b) { return (a + b - 1) / b; }
 void free_small() {
     void* ptrs[] = {G.srow, G.wrow, G.cos_t, G.sin_t, G.ringK, G.ringV, G.rho, G.force, G.rho_m,
                     G.phi,  G.mpart, G.pkpart, G.mom_dev, G.hist, G.wrow2, G.colpart_f, G.ticket, G.caspart, G.ringpart, G.ringtick,
-                    G.gsab};
+                    G.gsab, G.srow_sub[0], G.srow_sub[1], G.wrow_sub[0], G.wrow_sub[1]};
     for (void* p : ptrs)
         if (p) cudaFree(p);
     G.srow = nullptr;
@@ -166,6 +170,8 @@ void free_small() {
         G.mom_dev = G.hist = G.wrow2 = G.colpart_f = nullptr;
     G.ticket = nullptr;
     G.gsab = nullptr;
+    G.srow_sub[0] = G.srow_sub[1] = nullptr;
+    G.wrow_sub[0] = G.wrow_sub[1] = nullptr;
     G.caspart = nullptr;
     G.ringpart = nullptr;
     G.ringtick = nullptr;
@@ -364,14 +370,10 @@ size_t workspace_bytes() {
     return round256(state_bytes()) + round256((size_t)max_bands_bound() * G.ntheta * sizeof(double));
 }
 
-int prepare_tables() {
+// per-row integer shift and ten weights of a theta shift over the time tau (eq (9): displacement p_j tau)
+void row_tables(double tau, std::vector<int>& srow, std::vector<double>& wrow) {
     const int nt = G.ntheta, np = G.np;
     const double dx = (G.xmax - G.xmin) / (double)nt, dp = (G.pmax - G.pmin) / (double)np;
-    const double tau = 0.5 * G.dt;
-
-    // per-row shift of one half step: displacement p_j tau (eq (9)), u = -disp/dx cells
-    std::vector<int> srow(np);
-    std::vector<double> wrow((size_t)(np + FU_PAD) * vl::WROW_STRIDE, 0.0);  // FU_PAD rows of padding
     for (int j = 0; j < np; ++j) {
         const double p = G.pmin + (double)j * dp;
         const double disp = p * tau;
@@ -387,6 +389,28 @@ int prepare_tables() {
         vl::spline_fd8_weights(a, &wrow[(size_t)j * vl::WROW_STRIDE]);
         wrow[(size_t)j * vl::WROW_STRIDE + 10] = sf;
     }
+}
+
+// fp32 arithmetic: the ten weights of every row -> the nine difference-form weights (vl::diff_form_weights)
+void row_tables_to_difference_form(std::vector<double>& wrow) {
+    for (int j = 0; j < G.np; ++j) {
+        double* w = &wrow[(size_t)j * vl::WROW_STRIDE];
+        double U[9];
+        vl::diff_form_weights(w, 10, vl::FD_C, U);
+        for (int m = 0; m < 9; ++m) w[m] = U[m];
+        w[9] = 0.0;
+    }
+}
+
+int prepare_tables() {
+    const int nt = G.ntheta, np = G.np;
+    const double dx = (G.xmax - G.xmin) / (double)nt, dp = (G.pmax - G.pmin) / (double)np;
+    const double tau = 0.5 * G.dt;
+
+    // per-row shift of one half step: displacement p_j tau (eq (9)), u = -disp/dx cells
+    std::vector<int> srow(np);
+    std::vector<double> wrow((size_t)(np + FU_PAD) * vl::WROW_STRIDE, 0.0);  // FU_PAD rows of padding
+    row_tables(tau, srow, wrow);
     G.h_srow = srow;
     // composite weights of two equal half shifts, W = w * w (19 taps): the one-pass kernel applies both at once
     constexpr int W2 = 20;  // FusedWsCfg<T, 2, ...>::WST
@@ -407,13 +431,19 @@ int prepare_tables() {
             W[18] = 0.0;
         }
     }
-    if (G.prec == 32) {
-        for (int j = 0; j < np; ++j) {
-            double* w = &wrow[(size_t)j * vl::WROW_STRIDE];
-            double U[9];
-            vl::diff_form_weights(w, 10, vl::FD_C, U);
-            for (int m = 0; m < 9; ++m) w[m] = U[m];
-            w[9] = 0.0;
+    if (G.prec == 32) row_tables_to_difference_form(wrow);
+    if (G.order == 4) {
+        // triple jump: S2(g1 dt) S2(g2 dt) S2(g1 dt), g1 = 1/(2 - 2^(1/3)), g2 = 1 - 2 g1 < 0 (refs [31], [44])
+        const double g1 = 1.0 / (2.0 - cbrt(2.0)), g[2] = {g1, 1.0 - 2.0 * g1};
+        for (int k = 0; k < 2; ++k) {
+            std::vector<int> sr(np);
+            std::vector<double> wr((size_t)(np + FU_PAD) * vl::WROW_STRIDE, 0.0);
+            row_tables(0.5 * g[k] * G.dt, sr, wr);
+            if (G.prec == 32) row_tables_to_difference_form(wr);
+            CU(cudaMalloc(&G.srow_sub[k], sizeof(int) * np));
+            CU(cudaMalloc(&G.wrow_sub[k], sizeof(double) * wr.size()));
+            CU(cudaMemcpy(G.srow_sub[k], sr.data(), sizeof(int) * np, cudaMemcpyHostToDevice));
+            CU(cudaMemcpy(G.wrow_sub[k], wr.data(), sizeof(double) * wr.size(), cudaMemcpyHostToDevice));
         }
     }
     CU(cudaMalloc(&G.wrow2, sizeof(double) * wrow2.size()));
@@ -515,6 +545,8 @@ int prepare() {
     if (G.prepared) return VLASOV_OK;
     if (G.spline == 1 && (G.ntheta < vl::GS_MIN_N || G.np < vl::GS_MIN_N))
         return fail(VLASOV_EINVAL, "SPLINE = 1 (global spline) needs at least 32 nodes on both axes");
+    if (G.order == 4 && G.spline == 1)
+        return fail(VLASOV_EINVAL, "ORDER = 4 is built for the eq (16) spline only (SPLINE = 0)");
     const int rc = prepare_tables();
     if (rc != VLASOV_OK) {
         free_small();
@@ -627,7 +659,7 @@ int launch_p() {
     a.np = G.np;
     a.bc_p = G.bc_p;
     a.seg_len = G.p_seg;
-    a.dt = G.dt;
+    a.dt = G.dt_sub;
     a.dp = (G.pmax - G.pmin) / (double)G.np;
     dim3 grid(cdiv(G.ntheta, G.p_tx), G.p_nseg);
     prof_begin(2);
@@ -854,6 +886,7 @@ int vlasov_init(int model, const int grid[2], const double domain[4], double dt)
     G.pmin = domain[2];
     G.pmax = domain[3];
     G.dt = dt;
+    G.dt_sub = dt;
     G.bc_x = (model == VLASOV_MODEL_SHEET) ? vl::BC_ZERO : vl::BC_PERIODIC;
     G.bc_p = vl::BC_ZERO;
     G.ready = true;
@@ -892,6 +925,10 @@ int vlasov_set_param(int key, double value) {
             if (value == 1.0 && (G.ntheta < vl::GS_MIN_N || G.np < vl::GS_MIN_N))
                 return fail(VLASOV_EINVAL, "SPLINE = 1 (global spline) needs at least 32 nodes on both axes");
             G.spline = (int)value;
+            break;
+        case VLASOV_KEY_ORDER:
+            if (value != 2.0 && value != 4.0) return fail(VLASOV_EINVAL, "ORDER must be 2 or 4");
+            G.order = (int)value;
             break;
         case VLASOV_KEY_FUSE:
             if (value != 0.0 && value != 1.0 && value != 2.0) return fail(VLASOV_EINVAL, "FUSE must be 0, 1 or 2");
@@ -985,7 +1022,35 @@ int vlasov_step(int n) {
         }
         G.hist_count = 0;
     }
-    if (G.onepass && !G.history) {
+    if (G.order == 4) {
+        // fourth order: every step is three of the paper's steps (1)-(4) over g1 dt, g2 dt, g1 dt, each with its own
+        // row tables and its own force evaluation; the middle one runs backwards in time (separate passes)
+        const double g1 = 1.0 / (2.0 - cbrt(2.0)), g[2] = {g1, 1.0 - 2.0 * g1};
+        int* const srow0 = G.srow;
+        double* const wrow0 = G.wrow;
+        rc = VLASOV_OK;
+        for (int k = 0; k < n && rc == VLASOV_OK; ++k) {
+            for (int sub = 0; sub < 3 && rc == VLASOV_OK; ++sub) {
+                const int q = sub == 1 ? 1 : 0;
+                G.srow = G.srow_sub[q];
+                G.wrow = G.wrow_sub[q];
+                G.dt_sub = g[q] * G.dt;
+                if ((rc = theta_pass(1, true)) != 0) break;                                  // eq (9)
+                if ((rc = rho_and_force(theta_bands(1), nullptr, false)) != 0) break;        // eq (10)
+                if ((rc = p_pass()) != 0) break;                                             // eq (11)
+                rc = theta_pass(1, false);                                                   // eq (12)
+            }
+            G.t += G.dt;
+            if (G.history && rc == VLASOV_OK) {
+                rc = moments_async(G.hist + 8 * (size_t)k);
+                G.hist_count = k + 1;
+            }
+        }
+        G.srow = srow0;
+        G.wrow = wrow0;
+        G.dt_sub = G.dt;
+        if (rc != 0) return rc;
+    } else if (G.onepass && !G.history) {
         // n + 1 passes: theta(dt/2), then per step ONE pass  p(dt) -> theta(dt/2) [-> theta(dt/2) of the next step]
         if ((rc = theta_pass(1, true)) != 0) return rc;                           // eq (9)
         int k = 0;

@@ -374,3 +374,56 @@ def test_fp32_path_matches_oracle_to_1e_4():
     g.step(100)
     assert rel_err(g.download().astype(np.float64), o.download()) <= 1e-4
     g.close()
+
+
+# ----------------------------------------------------------------------------- fourth-order splitting (NEXT #4)
+@pytest.mark.parametrize("name,kw,steps", [("cfg1", dict(), 100), ("cfg2", dict(ntheta=256, npts=320), 40),
+                                           ("cfg3", dict(ntheta=320, npts=256), 40), ("cfg4", dict(ntheta=512, npts=300), 40),
+                                           ("cfg5", dict(ntheta=1500, npts=700), 20)])
+def test_order4_steps_match_oracle(name, kw, steps):
+    """ORDER = 4 (triple jump of the paper's step, middle sub-step backwards in time): state and
+    moments against the oracle's composition, same tolerances as the second-order path"""
+    c = inputs.config(name, **kw)
+    o, g = pair(c["model"], c["grid"], c["domain"], c["dt"], c["f0"], order=4, **c["params"])
+    o.step(steps)
+    g.step(steps)
+    fo, fg = o.download(), g.download()
+    assert rel_err(fg, fo) <= TOL
+    mo, mg = o.moments(), g.moments()
+    assert np.max(np.abs(mg - mo)) <= TOL * max(1.0, np.max(np.abs(mo)))
+    assert mg[0] == pytest.approx(steps * c["dt"])
+    g.close()
+
+
+def test_order4_differs_from_order2_and_records_history():
+    c = inputs.config("cfg1", n=128)
+    o, g = pair(c["model"], c["grid"], c["domain"], c["dt"], c["f0"], order=4, gpu_params=dict(history=1))
+    g.step(6)
+    h = g.history(6)
+    f4 = g.download()
+    g.close()
+    for k in range(6):
+        o.step(1)
+        assert np.max(np.abs(h[k] - o.moments())) <= TOL, k
+    g2 = vb.Vlasov(c["model"], c["grid"], c["domain"], c["dt"])
+    g2.upload(c["f0"])
+    g2.step(6)
+    assert rel_err(g2.download(), f4) > 1e-6   # really another scheme
+    g2.close()
+
+
+def test_order4_fp32_and_refusals():
+    c = inputs.config("cfg5", ntheta=600, npts=280)
+    o = Oracle(c["model"], c["grid"], c["domain"], c["dt"], threads=8, order=4)
+    o.upload(c["f0"])
+    o.step(30)
+    g = vb.Vlasov(c["model"], c["grid"], c["domain"], c["dt"], precision=32, order=4)
+    g.upload(c["f0"])
+    g.step(30)
+    assert rel_err(g.download().astype(np.float64), o.download()) <= 1e-4
+    g.close()
+    with pytest.raises(vb.VlasovError):
+        vb.Vlasov(c["model"], c["grid"], c["domain"], c["dt"], order=3)
+    with pytest.raises(vb.VlasovError):   # the global-spline variant has no fourth-order path
+        vb.Vlasov(c["model"], c["grid"], c["domain"], c["dt"], order=4, spline=vb.SPLINE_GS).step(1)
+    vb.vlasov_free()

@@ -28,3 +28,4 @@ from .vlasov_oracle import (  # noqa: F401
     gs_second_derivative,
     shift_line,
 )
+from .hmf_md_oracle import MdOracle, build_md  # noqa: F401,E402

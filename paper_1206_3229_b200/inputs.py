@@ -90,3 +90,13 @@ def config(name: str, n: int | None = None, ntheta: int | None = None, npts: int
         else:
             out["f0"] = perturbed_gaussian(th, p, ic[1], ic[2])
     return out
+
+
+def md_waterbag(n: int, theta0: float, p0: float, seed: int = SEED):
+    """N particles drawn uniformly from the water-bag |theta| < theta0, |p| < p0 (eq (17); the
+    initial state of the Fig. 4 comparison, L192-L206): theta_i = theta0 (2 u_i - 1), p_i = p0 (2 u'_i - 1) with
+    u, u' from the counter-based splitmix64 stream (keys seed + i and seed + N + i).  No method arithmetic."""
+    u = splitmix64_uniform(seed, 2 * n)
+    theta = theta0 * (2.0 * u[:n] - 1.0)
+    p = p0 * (2.0 * u[n:] - 1.0)
+    return np.ascontiguousarray(theta), np.ascontiguousarray(p)

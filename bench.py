@@ -418,6 +418,164 @@ def run_cuda(args):
     return 0
 
 
+# ------------------------------------------------------------------------------------------ HMF molecular dynamics
+MD_METRIC = "hmf_md_particle_steps_per_second"
+MD_UNIT = "Gparticle-steps/s"
+
+
+def md_config(args):
+    return {"workload": "HMF molecular dynamics, N = %d particles, water-bag theta0 = 1, p0 = 1, dt = 0.1, fourth-order "
+                        "symplectic integrator (PAPER.md L206, Fig. 4: N = 2e7)" % args.particles,
+            "particles": args.particles, "precision": 64, "passes_per_step": 3,
+            "l2": "state (%.0f MiB) exceeds the 126 MB L2; no flush needed" % (16.0 * args.particles / 2 ** 20)
+            if 16.0 * args.particles > L2_BYTES else "state fits L2: DRAM roofline not claimed"}
+
+
+def md_oracle_rate(n, steps, min_seconds=0.0):
+    """G particle-steps/s of the CPU oracle (one host thread: plain C loops)"""
+    import oracle
+    from paper_1206_3229_b200 import inputs
+
+    th, p = inputs.md_waterbag(n, 1.0, 1.0)
+    o = oracle.MdOracle(n, 0.1)
+    o.upload(th, p)
+    done, t0 = 0, time.perf_counter()
+    while True:
+        o.step(steps)
+        done += steps
+        el = time.perf_counter() - t0
+        if el >= min_seconds:
+            break
+    o.close()
+    return n * done / el / 1e9, el, done
+
+
+def run_md_reference(args):
+    rank, _, world = dist_env()
+    if rank != 0:
+        return 0
+    t_wall = time.perf_counter()
+    n = args.particles
+    val1, t1, _ = md_oracle_rate(n, 1)                      # first step: the estimate (and the page faults)
+    k_eff = max(1, min(args.steps, int(0.9 * max(args.ref_seconds - t1, 0.0) / t1)))
+    val, el, done = md_oracle_rate(n, k_eff)
+    sample = ("CPU oracle (oracle/hmf_md_oracle.c, one host thread) on all %d particles; %d timed steps (the requested "
+              "%d capped to fit %.0f s)" % (n, done, args.steps, args.ref_seconds))
+    print(json.dumps({
+        "impl": "reference", "metric": MD_METRIC, "value": val, "unit": MD_UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": el / done * 1e3, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": md_config(args), "steps_timed": done,
+        "cpu_baseline": {"value": val, "unit": MD_UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": MD_UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0, "wall_s": time.perf_counter() - t_wall}))
+    return 0
+
+
+def run_md(args):
+    import torch
+
+    from paper_1206_3229_b200 import binding as vb
+    from paper_1206_3229_b200 import inputs
+
+    rank, local_rank, world = dist_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the CUDA path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        import torch.distributed as dist
+
+        dist.init_process_group("nccl", device_id=dev)
+    n, K, W = args.particles, args.steps, max(args.warmup, 0)
+    th, p = inputs.md_waterbag(n, 1.0, 1.0)
+    g = vb.HmfMd(n, 0.1, device="cuda:%d" % local_rank)
+    g.upload(th, p)
+
+    def barrier():
+        if world > 1:
+            import torch.distributed as dist
+
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    if W:
+        g.step(W)
+    barrier()
+    reps_ms, launches = [], 0
+    t_load = time.perf_counter()
+    while len(reps_ms) < args.reps or (time.perf_counter() - t_load < args.min_load_seconds and len(reps_ms) < 50):
+        l0 = vb.hmf_md_launch_count()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        e0.record()
+        g.step(K)
+        e1.record()
+        barrier()
+        reps_ms.append(max_over_ranks(e0.elapsed_time(e1), world, dev))
+        launches = vb.hmf_md_launch_count() - l0
+    clocks = sampler.stop()
+    ms = median_rep(reps_ms)
+    value = world * float(n) * K / (ms * 1e-3) / 1e9
+    g.profile(True)
+    g.kernel_times()
+    g.step(K)
+    kms, kl = g.kernel_times()
+    g.profile(False)
+    mom = g.moments()
+    peak, peak_src = measured_peak()
+    avg_ms = kms / max(kl, 1)
+    ach = 32.0 * n / (avg_ms * 1e-3) / 1e9
+    roofline = {"bound": "hbm", "kernel": "md_kick_drift_kernel", "achieved": ach, "peak": peak, "unit": "GB/s",
+                "frac": ach / peak, "traffic": None, "peak_source": peak_src, "algorithmic_bytes_per_launch": 32.0 * n,
+                "note": "32 B per particle and pass (theta, p read and written), 3 passes per step; the pass also runs "
+                        "two fp64 sincos per particle"}
+    # end to end with host buffers
+    Ke = min(K, args.e2e_steps)
+    ht, hp = torch.from_numpy(th).pin_memory(), torch.from_numpy(p).pin_memory()
+    for _ in range(2):
+        g.upload_ptr(ht.data_ptr(), hp.data_ptr())
+        g.step(1)
+        g.download_ptr(ht.data_ptr(), hp.data_ptr())
+    barrier()
+    e2, e3 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e2.record()
+    for _ in range(Ke):
+        g.upload_ptr(ht.data_ptr(), hp.data_ptr())
+        g.step(1)
+        g.download_ptr(ht.data_ptr(), hp.data_ptr())
+    e3.record()
+    barrier()
+    ms_e2e = max_over_ranks(e2.elapsed_time(e3), world, dev)
+    e2e = {"value": world * float(n) * Ke / (ms_e2e * 1e-3) / 1e9, "unit": MD_UNIT, "h2d_bytes_per_step": 16 * n,
+           "d2h_bytes_per_step": 16 * n, "steps": Ke, "ms_per_step": ms_e2e / Ke,
+           "call": "hmf_md_upload(pinned host) + hmf_md_step(1) + hmf_md_download(pinned host)"}
+    g.close()
+    if world > 1:
+        import torch.distributed as dist
+
+        dist.destroy_process_group()
+    if rank != 0:
+        return 0
+    cpu = None
+    if not args.no_cpu_baseline:
+        val, el, done = md_oracle_rate(n, 1, min_seconds=args.cpu_seconds)
+        cpu = {"value": val, "unit": MD_UNIT, "cores": 1, "kind": "oracle",
+               "sample": "%d step(s) of all %d particles (%.1f s of wall time), oracle/hmf_md_oracle.c, one host thread" % (done, n, el)}
+    cfg = md_config(args)
+    cfg["parallelism"] = "replicas x%d" % world if world > 1 else "single GPU"
+    print(json.dumps({
+        "metric": MD_METRIC, "value": value, "unit": MD_UNIT, "n_gpus": world, "steps": K, "warmup": W,
+        "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic", "config": cfg,
+        "timing": {"reps": len(reps_ms), "reps_ms": reps_ms, "statistic": "median repetition of hmf_md_step(K)"},
+        "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline,
+        "kernels": {"md_kick_drift": {"avg_ms": avg_ms, "launches": kl, "achieved_gbs": ach}}, "cpu_baseline": cpu,
+        "final_moments": {"t": mom[0], "Mx": mom[1], "E": mom[5], "P": mom[6]}}))
+    return 0
+
+
 def relaunch_under_torchrun(args) -> int:
     """`python bench.py --gpus N` without torchrun: run N ranks of this script under torch.distributed.run"""
     with socket.socket() as s:
@@ -457,6 +615,10 @@ def main():
     ap.add_argument("--spline", default="fd", choices=["fd", "gs"],
                     help="fd: f'' by eq (16), the paper's method and the headline workload; gs: the Global Spline "
                          "comparator, system (15) (SURVEY 8(f) NEXT #2)")
+    ap.add_argument("--workload", default="vlasov", choices=["vlasov", "md"],
+                    help="vlasov: the Strang semi-Lagrangian step (BASELINE.json's metric); md: the N-particle HMF "
+                         "molecular dynamics of the paper's Fig. 4 (SURVEY 8(f) NEXT #3; its own metric, particle-steps/s)")
+    ap.add_argument("--particles", type=int, default=20000000, help="--workload md: number of particles (paper: 2e7)")
     ap.add_argument("--order", type=int, default=2, choices=[2, 4],
                     help="2: the paper's time split (headline); 4: its triple-jump composition (SURVEY 8(f) NEXT #4), "
                          "nine passes and three force evaluations per step")
@@ -467,6 +629,8 @@ def main():
             return relaunch_under_torchrun(args)
         raise SystemExit("bench.py: --gpus %d but WORLD_SIZE is %d (launch with torch.distributed.run "
                          "--nproc-per-node %d)" % (args.gpus, world, args.gpus))
+    if args.workload == "md":
+        return run_md_reference(args) if args.impl == "reference" else run_md(args)
     if args.impl == "reference":
         return run_reference(args)
     return run_cuda(args)

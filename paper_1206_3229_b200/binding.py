@@ -32,6 +32,12 @@ EXPORTS = (
 )
 
 
+MD_EXPORTS = (
+    "hmf_md_init", "hmf_md_attach", "hmf_md_upload", "hmf_md_download", "hmf_md_step", "hmf_md_moments",
+    "hmf_md_profile", "hmf_md_kernel_times", "hmf_md_launch_count", "hmf_md_free", "hmf_md_last_error",
+)
+
+
 class VlasovError(RuntimeError):
     def __init__(self, code: int, what: str, msg: str):
         super().__init__("%s failed with code %d: %s" % (what, code, msg))
@@ -84,6 +90,18 @@ def load(build_if_missing: bool = True):
         "vlasov_kernel_times": (ci, [_dp]),
         "vlasov_free": (None, []),
         "vlasov_last_error": (ctypes.c_char_p, []),
+        # include/hmf_md.h
+        "hmf_md_init": (ci, [ctypes.c_longlong, cd]),
+        "hmf_md_attach": (ci, [vp, vp, vp]),
+        "hmf_md_upload": (ci, [_dp, _dp]),
+        "hmf_md_download": (ci, [_dp, _dp]),
+        "hmf_md_step": (ci, [ci]),
+        "hmf_md_moments": (ci, [_dp]),
+        "hmf_md_profile": (ci, [ci]),
+        "hmf_md_kernel_times": (ci, [_dp]),
+        "hmf_md_launch_count": (ci, [ctypes.POINTER(ctypes.c_ulonglong)]),
+        "hmf_md_free": (None, []),
+        "hmf_md_last_error": (ctypes.c_char_p, []),
     }
     for name, (res, args) in sig.items():
         fn = getattr(lib, name)
@@ -297,3 +315,78 @@ class Vlasov:
     def close(self) -> None:
         vlasov_free()
         self.f_dev = self.work_dev = None
+
+
+# ---- HMF molecular dynamics (include/hmf_md.h) -------------------------------------------------------------
+
+def _chk_md(rc: int, what: str) -> int:
+    if rc < 0:
+        raise VlasovError(rc, what, (load().hmf_md_last_error() or b"").decode())
+    return rc
+
+
+def hmf_md_launch_count() -> int:
+    out = ctypes.c_ulonglong(0)
+    _chk_md(load().hmf_md_launch_count(ctypes.byref(out)), "hmf_md_launch_count")
+    return int(out.value)
+
+
+class HmfMd:
+    """N-particle HMF molecular dynamics (eqs (7)-(8), L206): argument marshalling only.  theta, p are
+    float64 arrays of length N; torch supplies the device memory and the stream."""
+
+    def __init__(self, n: int, dt: float, device: str = "cuda:0", attach: bool = True):
+        import torch
+
+        if not torch.cuda.is_available():
+            raise VlasovError(ECUDA, "HmfMd", "no CUDA device: this library has no CPU fallback")
+        self.n = int(n)
+        self.device = torch.device(device)
+        torch.cuda.set_device(self.device)
+        _chk_md(load().hmf_md_init(self.n, float(dt)), "hmf_md_init")
+        self.theta_dev = self.p_dev = None
+        if attach:
+            self.theta_dev = torch.zeros(self.n, dtype=torch.float64, device=self.device)
+            self.p_dev = torch.zeros(self.n, dtype=torch.float64, device=self.device)
+            stream = torch.cuda.current_stream(self.device).cuda_stream
+            _chk_md(load().hmf_md_attach(ctypes.c_void_p(self.theta_dev.data_ptr()), ctypes.c_void_p(self.p_dev.data_ptr()),
+                                         ctypes.c_void_p(stream)), "hmf_md_attach")
+
+    def upload(self, theta, p) -> None:
+        theta = np.ascontiguousarray(theta, dtype=np.float64)
+        p = np.ascontiguousarray(p, dtype=np.float64)
+        assert theta.shape == (self.n,) and p.shape == (self.n,)
+        _chk_md(load().hmf_md_upload(theta.ctypes.data_as(_dp), p.ctypes.data_as(_dp)), "hmf_md_upload")
+        self.moments()  # blocks: theta, p may be temporaries
+
+    def upload_ptr(self, theta_ptr: int, p_ptr: int) -> None:
+        _chk_md(load().hmf_md_upload(ctypes.cast(theta_ptr, _dp), ctypes.cast(p_ptr, _dp)), "hmf_md_upload")
+
+    def download_ptr(self, theta_ptr: int, p_ptr: int) -> None:
+        _chk_md(load().hmf_md_download(ctypes.cast(theta_ptr, _dp), ctypes.cast(p_ptr, _dp)), "hmf_md_download")
+
+    def download(self):
+        theta, p = np.empty(self.n), np.empty(self.n)
+        _chk_md(load().hmf_md_download(theta.ctypes.data_as(_dp), p.ctypes.data_as(_dp)), "hmf_md_download")
+        return theta, p
+
+    def step(self, n: int = 1) -> None:
+        _chk_md(load().hmf_md_step(int(n)), "hmf_md_step")
+
+    def moments(self) -> np.ndarray:
+        """{t, M_x, M_y, K/N, U/N, E/N, P/N, 0}"""
+        out = np.empty(8)
+        _chk_md(load().hmf_md_moments(out.ctypes.data_as(_dp)), "hmf_md_moments")
+        return out
+
+    def profile(self, on: bool) -> None:
+        _chk_md(load().hmf_md_profile(int(on)), "hmf_md_profile")
+
+    def kernel_times(self):
+        out = np.zeros(2)
+        _chk_md(load().hmf_md_kernel_times(out.ctypes.data_as(_dp)), "hmf_md_kernel_times")
+        return float(out[0]), int(out[1])
+
+    def close(self) -> None:
+        load().hmf_md_free()
+        self.theta_dev = self.p_dev = None

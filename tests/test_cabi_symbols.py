@@ -7,20 +7,31 @@ from paper_1206_3229_b200 import binding as vb
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
-def declared_symbols():
-    text = open(os.path.join(ROOT, "include", "vlasov.h")).read()
+def declared_symbols(header="vlasov.h", prefix="vlasov_"):
+    text = open(os.path.join(ROOT, "include", header)).read()
     text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
-    return sorted(set(re.findall(r"\b(vlasov_[a-z_]+)\s*\(", text)))
+    return sorted(set(re.findall(r"\b(%s[a-z_]+)\s*\(" % prefix, text)))
 
 
 def test_header_and_binding_agree():
     assert declared_symbols() == sorted(vb.EXPORTS)
+    assert declared_symbols("hmf_md.h", "hmf_md_") == sorted(vb.MD_EXPORTS)
 
 
 def test_library_builds_loads_and_exports_every_symbol():
     lib = vb.load()
-    for name in declared_symbols():
+    for name in declared_symbols() + declared_symbols("hmf_md.h", "hmf_md_"):
         assert hasattr(lib, name), name
+
+
+def test_md_calls_fail_loudly_without_init_or_device():
+    lib = vb.load()
+    lib.hmf_md_free()
+    assert lib.hmf_md_step(1) == vb.ENOTINIT
+    import torch
+
+    if not torch.cuda.is_available():
+        assert lib.hmf_md_init(100, 0.1) == vb.ECUDA
 
 
 def test_calls_fail_loudly_without_init_or_device():

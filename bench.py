@@ -576,6 +576,73 @@ def run_md(args):
     return 0
 
 
+# ------------------------------------------------------------------------------------------ p-slab sharding (strong scaling)
+def run_slab(args):
+    """--shard slab: ONE grid cut into p-slabs over the ranks (paper_1206_3229_b200/slab.py):
+    per step one all-reduce of rho and one halo exchange over NCCL, stages through the library's slab mode (two-pass
+    kernels).  Strong scaling: value = the grid's points x K / max time.  Never measured on more than one GPU by this
+    build (no multi-GPU box was available); with one rank it times the unsharded stage sequence."""
+    import torch
+
+    from paper_1206_3229_b200 import slab
+
+    rank, local_rank, world = dist_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the CUDA path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+
+        dist.init_process_group("nccl", device_id=dev)
+    c, cfg = workload(args)
+    nt, npp = c["grid"]
+    K, W = args.steps, max(args.warmup, 0)
+    dp = (c["domain"][3] - c["domain"][2]) / npp
+    halo = slab.halo_depth(args.slab_fmax, c["dt"], dp) if world > 1 else 0
+    b = slab.LibrarySlab(c["model"], c["grid"], c["domain"], c["dt"], rank, world, halo, device="cuda:%d" % local_rank,
+                         precision=args.precision, **c["params"])
+    b.upload_global(c["f0"])
+    st = slab.SlabStepper(b, rank, world, dist)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    if W:
+        st.step(W)
+    reps_ms = []
+    for _ in range(max(args.reps, 3)):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        e0.record()
+        st.step(K)
+        e1.record()
+        barrier()
+        reps_ms.append(max_over_ranks(e0.elapsed_time(e1), world, dev))
+    clocks = sampler.stop()
+    ms = median_rep(reps_ms)
+    b.close()
+    if world > 1:
+        dist.destroy_process_group()
+    if rank != 0:
+        return 0
+    cfg = dict(cfg)
+    cfg.update({"parallelism": "p-slabs x%d (rho all-reduce + halo exchange of %d rows per step)" % (world, halo),
+                "passes_per_step": 3})
+    print(json.dumps({
+        "metric": METRIC, "value": float(nt) * float(npp) * K / (ms * 1e-3) / 1e9, "unit": UNIT, "n_gpus": world, "steps": K,
+        "warmup": W, "ms_per_step": ms / K, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
+        "dtype": "f64" if args.precision == 64 else "f32", "data": "synthetic", "config": cfg,
+        "timing": {"reps": len(reps_ms), "reps_ms": reps_ms, "statistic": "median repetition of K sharded steps"},
+        "clocks": clocks, "gpu_launches": 5 * K, "roofline": None, "cpu_baseline": None, "e2e": None}))
+    return 0
+
+
 def relaunch_under_torchrun(args) -> int:
     """`python bench.py --gpus N` without torchrun: run N ranks of this script under torch.distributed.run"""
     with socket.socket() as s:
@@ -615,6 +682,10 @@ def main():
     ap.add_argument("--spline", default="fd", choices=["fd", "gs"],
                     help="fd: f'' by eq (16), the paper's method and the headline workload; gs: the Global Spline "
                          "comparator, system (15) (SURVEY 8(f) NEXT #2)")
+    ap.add_argument("--shard", default="replicas", choices=["replicas", "slab"],
+                    help="N > 1: replicas (default; independent copies, weak scaling) or slab (one grid cut into p-slabs, "
+                         "strong scaling; SURVEY 8(e))")
+    ap.add_argument("--slab-fmax", type=float, default=1.0, help="--shard slab: bound of |F| the halo depth is sized for")
     ap.add_argument("--workload", default="vlasov", choices=["vlasov", "md"],
                     help="vlasov: the Strang semi-Lagrangian step (BASELINE.json's metric); md: the N-particle HMF "
                          "molecular dynamics of the paper's Fig. 4 (SURVEY 8(f) NEXT #3; its own metric, particle-steps/s)")
@@ -633,6 +704,8 @@ def main():
         return run_md_reference(args) if args.impl == "reference" else run_md(args)
     if args.impl == "reference":
         return run_reference(args)
+    if args.shard == "slab":
+        return run_slab(args)
     return run_cuda(args)
 
 

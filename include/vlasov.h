@@ -68,6 +68,15 @@ extern "C" {
                                   ("higher order time split schemes", L238 with refs [31], [44]):
                                   three times the passes and force evaluations of a step, the middle sub-step
                                   backwards in time; eq (16) spline only                                          */
+#define VLASOV_KEY_HALO_LO 10  /* slab mode (p-slab sharding over several GPUs): the context   */
+#define VLASOV_KEY_HALO_HI 11  /* owns grid[1] rows of the global grid (domain = their p range) and its two state buffers carry
+                                  HALO_LO rows before and HALO_HI rows after them: [HALO_LO + Np + HALO_HI][Ntheta].  Theta
+                                  shifts, density and moments act on the owned rows, the momentum shift on all rows
+                                  (zero extension beyond them), so an owned row is right if the halos hold the
+                                  neighbours' rows and are deeper than max|F| dt/dp + 5.  The all-reduce of the density
+                                  and the halo exchange happen BETWEEN the stages of vlasov_substep and belong to the
+                                  caller (torch.distributed / NCCL); vlasov_step refuses.  upload / download move the
+                                  owned rows; vlasov_state_ptr is the start of the buffer (first halo row).           */
 /* keys 101..110 (launch-shape overrides: warps, bands, segment lengths, kernel variant) exist for the tests and
  * the tuning sweeps only; see binding.py KEY_TUNE_*.  Results never depend on them beyond rounding order.   */
 
@@ -80,6 +89,9 @@ extern "C" {
                                       and force of the result are left in the RHO / FORCE vectors (where the
                                       one-pass kernel does not apply -- vlasov_info says -- the separate kernels) */
 #define VLASOV_SUB_P_THETA_TWICE 5 /* one-pass kernel: eq (11), eq (12), eq (9) of the next step, then density, force */
+
+#define VLASOV_SUB_RHO 6            /* density of the (owned) rows from the column sums of the preceding THETA_HALF -> RHO */
+#define VLASOV_SUB_FORCE_FROM_RHO 7 /* force of the model from the RHO vector as it stands -> FORCE                       */
 
 /* vectors for vlasov_get_vector / vlasov_set_vector (Ntheta doubles each) */
 #define VLASOV_VEC_RHO 0   /* density rho_i = dp sum_j f_ij used by the last force evaluation */
@@ -142,6 +154,8 @@ int vlasov_substep(int which);
 /* Copy a device vector (VLASOV_VEC_*) of Ntheta doubles to / from host memory (blocking). */
 int vlasov_get_vector(int which, double* host_out);
 int vlasov_set_vector(int which, const double* host_in);
+/* Device pointer of a vector (Ntheta doubles, owned by the library): for collectives on it between two stages. */
+int vlasov_vector_ptr(int which, void** dev_out);
 
 /*
  * out (host, 8 doubles) = {t, mass, P, K, U, M_x, M_y, E = K + U} of the current state, rectangle rule:

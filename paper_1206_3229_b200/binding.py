@@ -17,17 +17,17 @@ import numpy as np
 from . import build as _build
 
 MODEL_FREE, MODEL_HMF, MODEL_RING, MODEL_SHEET = 0, 1, 2, 3
-KEY_EPS, KEY_PRECISION, KEY_BC_X, KEY_BC_P, KEY_HISTORY, KEY_FUSE, KEY_PROFILE, KEY_SPLINE, KEY_ORDER = 1, 2, 3, 4, 5, 6, 7, 8, 9
+KEY_EPS, KEY_PRECISION, KEY_BC_X, KEY_BC_P, KEY_HISTORY, KEY_FUSE, KEY_PROFILE, KEY_SPLINE, KEY_ORDER, KEY_HALO_LO, KEY_HALO_HI = 1, 2, 3, 4, 5, 6, 7, 8, 9, 10, 11
 SPLINE_FD, SPLINE_GS = 0, 1
 KEY_TUNE_NW1, KEY_TUNE_NW2, KEY_TUNE_BANDS, KEY_TUNE_PSEG, KEY_TUNE_PTX, KEY_TUNE_GENERIC, KEY_TUNE_FBANDS, KEY_TUNE_GRAPH = 101, 102, 103, 104, 105, 106, 107, 109
-SUB_THETA_HALF, SUB_FORCE, SUB_P_FULL, SUB_THETA_TWICE, SUB_P_THETA_HALF, SUB_P_THETA_TWICE = 0, 1, 2, 3, 4, 5
+SUB_THETA_HALF, SUB_FORCE, SUB_P_FULL, SUB_THETA_TWICE, SUB_P_THETA_HALF, SUB_P_THETA_TWICE, SUB_RHO, SUB_FORCE_FROM_RHO = 0, 1, 2, 3, 4, 5, 6, 7
 VEC_RHO, VEC_FORCE = 0, 1
 OK, EINVAL, ENOTINIT, ECUDA, ENOMEM = 0, -1, -2, -3, -4
 
 EXPORTS = (
     "vlasov_init", "vlasov_set_param", "vlasov_state_bytes", "vlasov_workspace_bytes", "vlasov_attach",
     "vlasov_state_ptr", "vlasov_upload", "vlasov_download", "vlasov_step", "vlasov_substep",
-    "vlasov_get_vector", "vlasov_set_vector", "vlasov_moments", "vlasov_casimirs", "vlasov_history", "vlasov_sync",
+    "vlasov_get_vector", "vlasov_set_vector", "vlasov_vector_ptr", "vlasov_moments", "vlasov_casimirs", "vlasov_history", "vlasov_sync",
     "vlasov_launch_count", "vlasov_kernel_times", "vlasov_info", "vlasov_free", "vlasov_last_error",
 )
 
@@ -81,6 +81,7 @@ def load(build_if_missing: bool = True):
         "vlasov_substep": (ci, [ci]),
         "vlasov_get_vector": (ci, [ci, _dp]),
         "vlasov_set_vector": (ci, [ci, _dp]),
+        "vlasov_vector_ptr": (ci, [ci, ctypes.POINTER(vp)]),
         "vlasov_moments": (ci, [_dp]),
         "vlasov_casimirs": (ci, [_dp]),
         "vlasov_history": (ci, [_dp, ci]),
@@ -185,6 +186,12 @@ def vlasov_set_vector(which: int, v) -> None:
     _chk(load().vlasov_set_vector(int(which), v.ctypes.data_as(_dp)), "vlasov_set_vector")
 
 
+def vlasov_vector_ptr(which: int) -> int:
+    out = ctypes.c_void_p()
+    _chk(load().vlasov_vector_ptr(int(which), ctypes.byref(out)), "vlasov_vector_ptr")
+    return int(out.value or 0)
+
+
 def vlasov_moments() -> np.ndarray:
     out = np.empty(8, dtype=np.float64)
     _chk(load().vlasov_moments(out.ctypes.data_as(_dp)), "vlasov_moments")
@@ -255,7 +262,7 @@ class Vlasov:
         vlasov_init(model, grid, domain, dt)
         if precision != 64:
             vlasov_set_param(KEY_PRECISION, precision)
-        keys = {"eps": KEY_EPS, "bc_x": KEY_BC_X, "bc_p": KEY_BC_P, "history": KEY_HISTORY, "fuse": KEY_FUSE, "profile": KEY_PROFILE, "spline": KEY_SPLINE, "order": KEY_ORDER,
+        keys = {"eps": KEY_EPS, "bc_x": KEY_BC_X, "bc_p": KEY_BC_P, "history": KEY_HISTORY, "fuse": KEY_FUSE, "profile": KEY_PROFILE, "spline": KEY_SPLINE, "order": KEY_ORDER, "halo_lo": KEY_HALO_LO, "halo_hi": KEY_HALO_HI,
                 "tune_nw1": KEY_TUNE_NW1, "tune_nw2": KEY_TUNE_NW2, "tune_bands": KEY_TUNE_BANDS,
                 "tune_pseg": KEY_TUNE_PSEG, "tune_ptx": KEY_TUNE_PTX, "tune_generic": KEY_TUNE_GENERIC,
                 "tune_fbands": KEY_TUNE_FBANDS, "tune_graph": KEY_TUNE_GRAPH}
@@ -264,11 +271,24 @@ class Vlasov:
         self.f_dev = self.work_dev = None
         if attach:
             tdt = torch.float64 if precision == 64 else torch.float32
-            self.f_dev = torch.zeros((self.np_, self.ntheta), dtype=tdt, device=self.device)
+            # rows of a state buffer: the grid's, plus the halos of a slab (VLASOV_KEY_HALO_LO / _HI)
+            self.rows_ext = vlasov_state_bytes() // (self.ntheta * (8 if precision == 64 else 4))
+            self.f_dev = torch.zeros((self.rows_ext, self.ntheta), dtype=tdt, device=self.device)
             self.work_dev = torch.empty(vlasov_workspace_bytes() + 256, dtype=torch.uint8, device=self.device)
             wp = (self.work_dev.data_ptr() + 255) & ~255
             self.stream = torch.cuda.current_stream(self.device)
             vlasov_attach(self.f_dev.data_ptr(), wp, vlasov_workspace_bytes(), self.stream.cuda_stream)
+            off = wp - self.work_dev.data_ptr()
+            self.f_alt = self.work_dev[off:off + self.f_dev.numel() * self.f_dev.element_size()].view(tdt).view(
+                self.rows_ext, self.ntheta)  # the second state buffer (the passes ping-pong between the two)
+
+    def current_state_tensor(self):
+        """torch view [rows (+ halos), Ntheta] of the buffer that holds f now (attached buffers only)"""
+        ptr = vlasov_state_ptr()
+        if ptr == self.f_dev.data_ptr():
+            return self.f_dev
+        assert ptr == self.f_alt.data_ptr()
+        return self.f_alt
 
     def upload(self, f) -> None:
         f = np.ascontiguousarray(f, dtype=self.dtype)

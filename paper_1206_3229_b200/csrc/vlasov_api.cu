@@ -44,6 +44,9 @@ struct Ctx {
     double xmin = 0, xmax = 0, pmin = 0, pmax = 0, dt = 0, eps = 0.01, t = 0;
     int bc_x = 0, bc_p = 1, prec = 64;
     int spline = 0;  // 0: f'' by eq (16) (the paper's method), 1: global spline, system (15) (vlasov_gs.cuh)
+    int halo_lo = 0, halo_hi = 0;  // slab mode (p-slab sharding): halo rows below / above the Np owned rows
+    int np_ext() const { return np + halo_lo + halo_hi; }
+    void* owned(int k) const;      // first owned row of state buffer k
     int order = 2;   // 2: the paper's time split; 4: its triple-jump composition S2(g1 dt) S2(g2 dt) S2(g1 dt) (L238)
     double dt_sub = 0;                                 // time step of the sub-step being enqueued (= dt for order 2)
     int* srow_sub[2] = {nullptr, nullptr};            // order 4: row tables of the sub-steps g1 dt, g2 dt
@@ -107,6 +110,9 @@ struct Ctx {
 };
 
 Ctx G;
+void* Ctx::owned(int k) const {
+    return static_cast<char*>(f[k]) + (size_t)halo_lo * (size_t)ntheta * (size_t)(prec == 32 ? 4 : 8);
+}
 constexpr size_t EV_CAP = 2048;
 
 void prof_begin(int cls) {
@@ -155,7 +161,8 @@ int fail(int code, const char* fmt, const char* a = "") {
     } while (0)
 
 size_t elem_bytes() { return G.prec == 32 ? 4 : 8; }
-size_t state_bytes() { return (size_t)G.ntheta * (size_t)G.np * elem_bytes(); }
+size_t state_bytes() { return (size_t)G.ntheta * (size_t)G.np_ext() * elem_bytes(); }  // owned rows + halos
+size_t owned_bytes() { return (size_t)G.ntheta * (size_t)G.np * elem_bytes(); }
 size_t round256(size_t b) { return (b + 255) & ~(size_t)255; }
 int cdiv(int a, int b) { return (a + b - 1) / b; }
 
@@ -329,7 +336,7 @@ int configure_all() {
         if ((rc = configure_theta_bulk<T, 1>()) != 0) return rc;
         if ((rc = configure_theta_bulk<T, 2>()) != 0) return rc;
     }
-    G.onepass = (G.fuse >= 2) && (G.bc_x == vl::BC_PERIODIC);
+    G.onepass = (G.fuse >= 2) && (G.bc_x == vl::BC_PERIODIC) && (G.halo_lo + G.halo_hi == 0);
     if (G.onepass) {
         if ((rc = configure_fused<T, 1>()) != 0) return rc;
         if ((rc = configure_fused<T, 2>()) != 0) return rc;
@@ -545,6 +552,8 @@ int prepare() {
     if (G.prepared) return VLASOV_OK;
     if (G.spline == 1 && (G.ntheta < vl::GS_MIN_N || G.np < vl::GS_MIN_N))
         return fail(VLASOV_EINVAL, "SPLINE = 1 (global spline) needs at least 32 nodes on both axes");
+    if ((G.halo_lo + G.halo_hi > 0) && (G.order == 4 || G.spline == 1))
+        return fail(VLASOV_EINVAL, "slab mode is built for ORDER = 2, SPLINE = 0");
     if (G.order == 4 && G.spline == 1)
         return fail(VLASOV_EINVAL, "ORDER = 4 is built for the eq (16) spline only (SPLINE = 0)");
     const int rc = prepare_tables();
@@ -582,8 +591,8 @@ int ensure_buffers() {
 template <typename T, int NSTAGE>
 int launch_theta(bool want_colsums) {
     vl::ThetaArgs<T> a;
-    a.fin = static_cast<const T*>(G.f[G.cur]);
-    a.fout = static_cast<T*>(G.f[G.cur ^ 1]);
+    a.fin = static_cast<const T*>(G.owned(G.cur));
+    a.fout = static_cast<T*>(G.owned(G.cur ^ 1));
     a.srow = G.srow;
     a.wrow = G.wrow;
     a.colpart = want_colsums ? G.colpart : nullptr;
@@ -611,8 +620,8 @@ int launch_theta(bool want_colsums) {
 template <typename T>
 int launch_gs_theta_rec(bool want_colsums) {
     vl::GsThetaRecArgs<T> a;
-    a.fin = static_cast<const T*>(G.f[G.cur]);
-    a.fout = static_cast<T*>(G.f[G.cur ^ 1]);
+    a.fin = static_cast<const T*>(G.owned(G.cur));
+    a.fout = static_cast<T*>(G.owned(G.cur ^ 1));
     a.srow = G.srow;
     a.gsab = G.gsab;
     a.colpart = want_colsums ? G.colpart : nullptr;
@@ -652,16 +661,16 @@ int theta_pass(int nstage, bool want_colsums) {
 template <typename T>
 int launch_p() {
     vl::PArgs<T> a;
-    a.fin = static_cast<const T*>(G.f[G.cur]);
+    a.fin = static_cast<const T*>(G.f[G.cur]);   // slab mode: the momentum shift runs over the owned rows AND the halos
     a.fout = static_cast<T*>(G.f[G.cur ^ 1]);
     a.force = G.force;
     a.ntheta = G.ntheta;
-    a.np = G.np;
+    a.np = G.np_ext();
     a.bc_p = G.bc_p;
     a.seg_len = G.p_seg;
     a.dt = G.dt_sub;
     a.dp = (G.pmax - G.pmin) / (double)G.np;
-    dim3 grid(cdiv(G.ntheta, G.p_tx), G.p_nseg);
+    dim3 grid(cdiv(G.ntheta, G.p_tx), cdiv(G.np_ext(), G.p_seg));
     prof_begin(2);
     vl::p_sweep_kernel<T><<<grid, G.p_tx, 0, G.stream>>>(a);
     prof_end(2);
@@ -774,7 +783,7 @@ template <typename T>
 int launch_moments_pass() {
     const double dp = (G.pmax - G.pmin) / (double)G.np;
     dim3 grid(cdiv(G.ntheta, 256), G.mbands);
-    vl::moments_pass_kernel<T><<<grid, 256, 0, G.stream>>>(static_cast<const T*>(G.f[G.cur]), G.ntheta, G.np,
+    vl::moments_pass_kernel<T><<<grid, 256, 0, G.stream>>>(static_cast<const T*>(G.owned(G.cur)), G.ntheta, G.np,
                                                            G.mrpb, G.pmin, dp, G.colpart, G.pkpart);
     LAUNCH_CHECK();
     return VLASOV_OK;
@@ -926,6 +935,11 @@ int vlasov_set_param(int key, double value) {
                 return fail(VLASOV_EINVAL, "SPLINE = 1 (global spline) needs at least 32 nodes on both axes");
             G.spline = (int)value;
             break;
+        case VLASOV_KEY_HALO_LO:
+        case VLASOV_KEY_HALO_HI:
+            if (value < 0.0 || value > 1.0e6 || value != floor(value)) return fail(VLASOV_EINVAL, "HALO_LO / HALO_HI must be a row count >= 0");
+            (key == VLASOV_KEY_HALO_LO ? G.halo_lo : G.halo_hi) = (int)value;
+            break;
         case VLASOV_KEY_ORDER:
             if (value != 2.0 && value != 4.0) return fail(VLASOV_EINVAL, "ORDER must be 2 or 4");
             G.order = (int)value;
@@ -985,7 +999,8 @@ int vlasov_upload(const void* f_host) {
     if (!f_host) return fail(VLASOV_EINVAL, "vlasov_upload: null");
     if ((rc = ensure_buffers()) != 0) return rc;
     G.cur = 0;
-    CU(cudaMemcpyAsync(G.f[0], f_host, state_bytes(), cudaMemcpyHostToDevice, G.stream));
+    if (G.halo_lo + G.halo_hi > 0) CU(cudaMemsetAsync(G.f[0], 0, state_bytes(), G.stream));  // halos start as zeros
+    CU(cudaMemcpyAsync(G.owned(0), f_host, owned_bytes(), cudaMemcpyHostToDevice, G.stream));
     G.t = 0.0;
     return VLASOV_OK;
 }
@@ -995,7 +1010,7 @@ int vlasov_download(void* f_host) {
     if (rc != 0) return rc;
     if (!f_host) return fail(VLASOV_EINVAL, "vlasov_download: null");
     if ((rc = ensure_buffers()) != 0) return rc;
-    CU(cudaMemcpyAsync(f_host, G.f[G.cur], state_bytes(), cudaMemcpyDeviceToHost, G.stream));
+    CU(cudaMemcpyAsync(f_host, G.owned(G.cur), owned_bytes(), cudaMemcpyDeviceToHost, G.stream));
     CU(cudaStreamSynchronize(G.stream));
     return VLASOV_OK;
 }
@@ -1012,7 +1027,9 @@ int vlasov_step(int n) {
     if (rc != 0) return rc;
     if (n <= 0) return fail(VLASOV_EINVAL, "vlasov_step: n must be >= 1");
     if ((rc = ensure_buffers()) != 0) return rc;
-    const bool hmf = (G.model == VLASOV_MODEL_HMF);
+    if (G.halo_lo + G.halo_hi > 0)
+        return fail(VLASOV_EINVAL, "vlasov_step: a slab (HALO_LO / HALO_HI > 0) is advanced stage by stage with vlasov_substep, the "
+                                   "density all-reduce and the halo exchange in between belong to the caller");
     if (G.history) {
         if (G.hist_cap < n) {
             if (G.hist) CU(cudaFree(G.hist));
@@ -1115,6 +1132,16 @@ int vlasov_substep(int which) {
             if ((rc = moments_pass()) != 0) return rc;
             return rho_and_force(G.mbands, nullptr, false);
         case VLASOV_SUB_P_FULL: return p_pass();
+        case VLASOV_SUB_RHO:  // density of the owned rows from the column sums the last theta pass left behind
+            return rho_from_colpart(theta_bands(1), G.rho, false);
+        case VLASOV_SUB_FORCE_FROM_RHO:  // force from the RHO vector as it stands (after the caller's all-reduce)
+            if (G.model == VLASOV_MODEL_HMF) {
+                const double dx = (G.xmax - G.xmin) / (double)G.ntheta;
+                vl::hmf_force_from_rho_kernel<<<1, 1024, 0, G.stream>>>(G.rho, G.cos_t, G.sin_t, G.ntheta, dx, G.force);
+                LAUNCH_CHECK();
+                return VLASOV_OK;
+            }
+            return force_from_rho();
         case VLASOV_SUB_P_THETA_HALF:
         case VLASOV_SUB_P_THETA_TWICE: {
             const int nst = which == VLASOV_SUB_P_THETA_TWICE ? 2 : 1;
@@ -1139,6 +1166,15 @@ int vlasov_get_vector(int which, double* host_out) {
     const double* src = which == VLASOV_VEC_RHO ? G.rho : G.force;
     CU(cudaMemcpyAsync(host_out, src, sizeof(double) * G.ntheta, cudaMemcpyDeviceToHost, G.stream));
     CU(cudaStreamSynchronize(G.stream));
+    return VLASOV_OK;
+}
+
+int vlasov_vector_ptr(int which, void** dev_out) {
+    int rc = check_ready();
+    if (rc != 0) return rc;
+    if (!dev_out || (which != VLASOV_VEC_RHO && which != VLASOV_VEC_FORCE)) return fail(VLASOV_EINVAL, "vlasov_vector_ptr: bad argument");
+    if ((rc = ensure_buffers()) != 0) return rc;
+    *dev_out = which == VLASOV_VEC_RHO ? G.rho : G.force;
     return VLASOV_OK;
 }
 
@@ -1172,10 +1208,10 @@ int vlasov_casimirs(double out[4]) {
     const double cell = ((G.xmax - G.xmin) / (double)G.ntheta) * ((G.pmax - G.pmin) / (double)G.np);
     dim3 grid(cdiv(G.ntheta, 256), G.mbands);
     if (G.prec == 32)
-        vl::casimir_pass_kernel<float><<<grid, 256, 0, G.stream>>>(static_cast<const float*>(G.f[G.cur]), G.ntheta, G.np,
+        vl::casimir_pass_kernel<float><<<grid, 256, 0, G.stream>>>(static_cast<const float*>(G.owned(G.cur)), G.ntheta, G.np,
                                                                    G.mrpb, G.caspart);
     else
-        vl::casimir_pass_kernel<double><<<grid, 256, 0, G.stream>>>(static_cast<const double*>(G.f[G.cur]), G.ntheta,
+        vl::casimir_pass_kernel<double><<<grid, 256, 0, G.stream>>>(static_cast<const double*>(G.owned(G.cur)), G.ntheta,
                                                                     G.np, G.mrpb, G.caspart);
     LAUNCH_CHECK();
     double* res = G.caspart + 4 * (size_t)nblk;

@@ -619,6 +619,31 @@ __global__ void __launch_bounds__(RR_COLS* RR_GROUPS)
     for (int k = tid; k < ntheta; k += RR_COLS * RR_GROUPS) force[k] = -sin_t[k] * mx + cos_t[k] * my;
 }
 
+// HMF force from a density vector (eqs (7)-(8), L56-L63), one CTA: M = dtheta sum_i (cos, sin)(theta_i) rho_i over a fixed
+// tree, F_i = -M_x sin(theta_i) + M_y cos(theta_i).  Used where rho does not come out of rho_force_kernel: in slab
+// mode the density is all-reduced over the ranks between the two.
+__global__ void __launch_bounds__(1024) hmf_force_from_rho_kernel(const double* __restrict__ rho, const double* __restrict__ cos_t,
+                                                                  const double* __restrict__ sin_t, int ntheta, double dtheta,
+                                                                  double* __restrict__ force) {
+    __shared__ double red[32];
+    __shared__ double msh[2];
+    double cx = 0.0, sx = 0.0;
+    for (int i = threadIdx.x; i < ntheta; i += 1024) {
+        const double r = rho[i];
+        cx = fma(cos_t[i], r, cx);
+        sx = fma(sin_t[i], r, sx);
+    }
+    const double CX = block_sum<1024>(cx, red);
+    const double SX = block_sum<1024>(sx, red);
+    if (threadIdx.x == 0) {
+        msh[0] = CX * dtheta;
+        msh[1] = SX * dtheta;
+    }
+    __syncthreads();
+    const double mx = msh[0], my = msh[1];
+    for (int i = threadIdx.x; i < ntheta; i += 1024) force[i] = -sin_t[i] * mx + cos_t[i] * my;
+}
+
 // ring, eq (2) (L33-L35), reading D9: out_i = scale * sum_{m=0}^{N-1} tab[m] rho[(i - m) mod N].
 // Used with tab = K (force) and tab = V (potential, for the energy).  The sum over m is cut into chunks of RING_L
 // terms: CTA (tile of 256 outputs, chunk c) stages its piece of the table and the matching window of rho in shared

@@ -283,7 +283,7 @@ def run_cuda(args):
     nt, npp = c["grid"]
     f0 = c["f0"].astype(np.float64 if prec == 64 else np.float32)
     params = dict(c["params"])
-    params.update(fuse=args.fuse, tune_graph=args.graph)
+    params.update(fuse=args.fuse, tune_graph=args.graph, tune_pdl=args.pdl)
     if args.spline == "gs":
         params["spline"] = vb.SPLINE_GS
     if args.order == 4:
@@ -679,6 +679,8 @@ def main():
     ap.add_argument("--fbands", type=int, default=0, help="bands of rows of the one-pass kernel (0 = automatic)")
     ap.add_argument("--graph", type=int, default=1, choices=[0, 1],
                     help="1 (default): steady-state step pairs are launched as CUDA graphs, 0: plain launches")
+    ap.add_argument("--pdl", type=int, default=1, choices=[0, 1],
+                    help="1 (default): programmatic dependent launch between the pass and the density/force kernel")
     ap.add_argument("--spline", default="fd", choices=["fd", "gs"],
                     help="fd: f'' by eq (16), the paper's method and the headline workload; gs: the Global Spline "
                          "comparator, system (15) (SURVEY 8(f) NEXT #2)")

@@ -29,7 +29,7 @@ constexpr int TB_MINB = 3;       // CTAs per SM the register budget is set for
 constexpr int FU_R = 11;         // consecutive outputs per lane in the theta stage of the one-pass kernel (odd)
 constexpr int FW_NSTG = 3;       // ring depth (groups of 12 rows) of the one-pass kernel
 constexpr int FW_NTW = 12;       // its theta warps = density partial rows per band
-constexpr int KEY_TUNE_GRAPH = 109;
+constexpr int KEY_TUNE_GRAPH = 109, KEY_TUNE_PDL = 110;
 constexpr int FU_PAD = 12;       // rows of padding of the theta weight tables (the last phase of a band reads on)
 constexpr int NCLS = 6;          // profiled kernel classes: theta x1, theta x2, p, rho+force, p+theta x2, p+theta x1
 constexpr int KEY_TUNE_FBANDS = 107;
@@ -80,6 +80,7 @@ struct Ctx {
     // CUDA graph of two consecutive steady-state steps of the one-pass path (density/force + pass, twice), one
     // per parity of the ping-pong; captured on a private stream, launched on the attached one
     bool graphs = true;
+    bool pdl = true;  // programmatic dependent launch between the pass and the density / force kernels (KEY_TUNE_PDL)
     cudaGraphExec_t gexec[2] = {nullptr, nullptr};
     unsigned graph_kernels[2] = {0, 0};
     cudaStream_t cap_stream = nullptr;
@@ -200,6 +201,24 @@ void free_big() {
     G.colpart = nullptr;
     G.own_f = G.own_work = G.attached = false;
     G.cur = 0;
+}
+
+// launch with programmatic stream serialisation (programmatic dependent launch): the kernel may be scheduled while its
+// predecessor in the stream still runs and waits for it inside (ptx::pdl_wait).  Works in stream capture too (the
+// graph gets a programmatic edge).  G.pdl = false: an ordinary launch.
+template <typename... KArgs, typename... Args>
+cudaError_t launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, Args... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = G.stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = G.pdl ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kern, KArgs(args)...);
 }
 
 template <typename T, int NSTAGE>
@@ -724,7 +743,7 @@ int launch_fused(bool want_colsums) {
     a.dp = (G.pmax - G.pmin) / (double)G.np;
     dim3 grid(G.fcols[NST], G.fbands[NST]);
     prof_begin(NST == 2 ? 4 : 5);
-    vl::strang_fused_ws_kernel<T, NST, FU_R, FW_NSTG, FW_NTW><<<grid, CW::NT, CW::SMEM_BYTES, G.stream>>>(a);
+    CU(launch_pdl(vl::strang_fused_ws_kernel<T, NST, FU_R, FW_NSTG, FW_NTW>, grid, dim3(CW::NT), CW::SMEM_BYTES, a));
     prof_end(NST == 2 ? 4 : 5);
     LAUNCH_CHECK();
     G.cur ^= 1;
@@ -744,9 +763,10 @@ int rho_from_colpart(int bands, double* rho_out, bool hmf_partials, double* colp
     const double dp = (G.pmax - G.pmin) / (double)G.np;
     const double dx = (G.xmax - G.xmin) / (double)G.ntheta;
     const bool sheet = fuse_force && G.model == VLASOV_MODEL_SHEET;
-    vl::rho_force_kernel<<<cdiv(G.ntheta, vl::RR_COLS), vl::RR_COLS * vl::RR_GROUPS, 0, G.stream>>>(
-        colpart ? colpart : G.colpart, bands, G.ntheta, dp, rho_out, G.cos_t, G.sin_t, hmf_partials ? G.mpart : nullptr,
-        zero_after ? 1 : 0, G.ticket, dx, (fuse_force && (hmf_partials || sheet)) ? G.force : nullptr, sheet ? 1 : 0);
+    CU(launch_pdl(vl::rho_force_kernel, dim3(cdiv(G.ntheta, vl::RR_COLS)), dim3(vl::RR_COLS * vl::RR_GROUPS), 0,
+                  colpart ? colpart : G.colpart, bands, G.ntheta, dp, rho_out, (const double*)G.cos_t, (const double*)G.sin_t,
+                  hmf_partials ? G.mpart : (double*)nullptr, zero_after ? 1 : 0, G.ticket, dx,
+                  (fuse_force && (hmf_partials || sheet)) ? G.force : (double*)nullptr, sheet ? 1 : 0));
     LAUNCH_CHECK();
     return VLASOV_OK;
 }
@@ -757,6 +777,8 @@ int force_from_rho() {
     const double dx = (G.xmax - G.xmin) / (double)nt;
     switch (G.model) {
         case VLASOV_MODEL_RING:
+            // an ordinary launch: behind rho_force_kernel's early trigger its 128 CTAs only sat in the way of the pass
+            // (cfg 3: 39.0 -> 41.8 us per step with a programmatic launch here)
             vl::ring_convolve_kernel<<<dim3(cdiv(nt, 256), cdiv(nt, vl::RING_L)), 256, 0, G.stream>>>(
                 G.ringK, G.rho, nt, dx, G.ringpart, G.ringtick, G.force);
             break;
@@ -950,6 +972,7 @@ int vlasov_set_param(int key, double value) {
             break;
         case KEY_TUNE_FBANDS: G.tune_fbands = (int)value; break;
         case KEY_TUNE_GRAPH: G.graphs = (value != 0.0); break;
+        case KEY_TUNE_PDL: G.pdl = (value != 0.0); break;
         case VLASOV_KEY_PROFILE: G.profile = (value != 0.0); break;
         case KEY_TUNE_NW1: G.tune_nw1 = (int)value; break;
         case KEY_TUNE_NW2: G.tune_nw2 = (int)value; break;

@@ -100,6 +100,7 @@ __global__ void __launch_bounds__((4 + NTW_) * 32, 1) strang_fused_ws_kernel(con
     const int ngroups = (nrows + RG - 1) / RG;
     const unsigned pitch = (unsigned)ntheta;
 
+    ptx::pdl_launch_dependents();  // the density / force kernel that follows may be scheduled while this pass runs
     if (tid == 0) {
 #pragma unroll
         for (int k = 0; k < NSUB; ++k) {
@@ -109,6 +110,9 @@ __global__ void __launch_bounds__((4 + NTW_) * 32, 1) strang_fused_ws_kernel(con
         ptx::fence_mbar_init();
     }
     __syncthreads();
+    // everything above is independent of the force and of f; from here on both are read (and the density partials
+    // written): wait for the density / force kernel this pass was launched behind (programmatic dependent launch)
+    ptx::pdl_wait();
     const uint32_t ready_u32 = ptx::smem_u32(ready), empty_u32 = ptx::smem_u32(empty);
 
     if (warp < C::NPW) {

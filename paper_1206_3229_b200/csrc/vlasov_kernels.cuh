@@ -517,6 +517,8 @@ __global__ void __launch_bounds__(RR_COLS* RR_GROUPS)
     __shared__ double part[RR_GROUPS][RR_COLS];
     __shared__ double2 mp[RR_COLS * RR_GROUPS];
     __shared__ bool last;
+    ptx::pdl_launch_dependents();  // the next pass may be scheduled (its set-up does not depend on the force)
+    ptx::pdl_wait();               // the pass whose column sums are read here has completed
     const int tid = threadIdx.x, c = tid & (RR_COLS - 1), g = tid / RR_COLS;
     const int i = blockIdx.x * RR_COLS + c;
     double a0 = 0.0, a1 = 0.0;

@@ -103,6 +103,12 @@ __device__ __forceinline__ void bulk_wait_read() {
 // generic-proxy writes to shared memory -> visible to the async proxy (bulk copies) issued afterwards
 __device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
+// Programmatic dependent launch (sm_90+).  A kernel launched with cudaLaunchAttributeProgrammaticStreamSerialization may
+// start while its predecessor in the stream still runs; pdl_wait() blocks until the predecessor grid has completed and
+// its memory is visible (a no-op for an ordinary launch), pdl_launch_dependents() lets the successor's launch begin.
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
 __device__ __forceinline__ uint64_t policy_evict_first() {
     uint64_t p;
     asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));

@@ -65,3 +65,58 @@ def test_small_md_matches_oracle():
     assert np.max(np.abs(g.moments() - o.moments())) < 1e-12
     g.close()
     o.close()
+
+
+@pytest.mark.parametrize("name,kw,params", [
+    ("cfg1", dict(ntheta=353, npts=61), dict()), ("cfg1", dict(ntheta=352, npts=60), dict(precision=32)),
+    ("cfg5", dict(ntheta=1100, npts=640), dict()), ("cfg3", dict(ntheta=256, npts=48), dict(fuse=1)),
+    ("cfg4", dict(ntheta=256, npts=64), dict()), ("cfg1", dict(ntheta=96, npts=64), dict(spline=1)),
+    ("cfg1", dict(ntheta=131, npts=40), dict(fuse=0, order=4)), ("cfg1", dict(ntheta=128, npts=48), dict(halo_lo=7, halo_hi=9, fuse=0)),
+])
+def test_no_byte_is_written_outside_the_attached_buffers(name, kw, params):
+    """compute-sanitizer is closed on this pool (gpurun refuses it), so out-of-bounds WRITES are looked for directly:
+    the state and work buffers handed to vlasov_attach sit between guard zones of 1 MiB filled with a pattern, every
+    stage kind runs, and the guards must come back untouched (reads out of bounds would show up as parity failures
+    of the tests above: the guards hold NaN patterns)."""
+    import torch
+
+    c = inputs.config(name, **kw)
+    prec = params.get("precision", 64)
+    vb.vlasov_init(c["model"], c["grid"], c["domain"], c["dt"])
+    keys = {"precision": vb.KEY_PRECISION, "fuse": vb.KEY_FUSE, "spline": vb.KEY_SPLINE, "order": vb.KEY_ORDER,
+            "halo_lo": vb.KEY_HALO_LO, "halo_hi": vb.KEY_HALO_HI}
+    for k, v in params.items():
+        vb.vlasov_set_param(keys[k], v)
+    for k, v in c["params"].items():
+        vb.vlasov_set_param(vb.KEY_EPS, v)
+    sb, wb, G = vb.vlasov_state_bytes(), vb.vlasov_workspace_bytes(), 1 << 20
+    r = lambda b: (b + 255) & ~255
+    buf = torch.full((G + r(sb) + G + r(wb) + G + 256,), 0xFF, dtype=torch.uint8, device="cuda")   # 0xFF..: NaN as fp64 / fp32
+    base = (buf.data_ptr() + 255) & ~255
+    o0 = base - buf.data_ptr()
+    f_off, w_off = o0 + G, o0 + G + r(sb) + G
+    buf[f_off:f_off + sb] = 0
+    if params.get("halo_lo"):
+        buf[w_off:w_off + wb] = 0   # a slab's halos are the caller's to fill (exchange): zeros here, not the NaN pattern
+    vb.vlasov_attach(buf.data_ptr() + f_off, buf.data_ptr() + w_off, wb, torch.cuda.current_stream().cuda_stream)
+    rows = c["grid"][1]
+    f0 = c["f0"].astype(np.float64 if prec == 64 else np.float32)
+    vb.vlasov_upload(np.ascontiguousarray(f0))
+    vb.vlasov_sync()
+    if params.get("halo_lo"):
+        for st in (vb.SUB_THETA_HALF, vb.SUB_RHO, vb.SUB_FORCE_FROM_RHO, vb.SUB_P_FULL, vb.SUB_THETA_HALF):
+            vb.vlasov_substep(st)
+    else:
+        vb.vlasov_step(5)
+        vb.vlasov_step(1)
+        for st in (vb.SUB_THETA_HALF, vb.SUB_THETA_TWICE, vb.SUB_FORCE, vb.SUB_P_FULL, vb.SUB_P_THETA_HALF, vb.SUB_P_THETA_TWICE):
+            vb.vlasov_substep(st)
+    vb.vlasov_moments()
+    vb.vlasov_casimirs()
+    out = np.empty((rows, c["grid"][0]), dtype=f0.dtype)
+    vb.vlasov_download(out)
+    assert np.all(np.isfinite(out))
+    vb.vlasov_free()
+    guards = [buf[:f_off], buf[f_off + sb:w_off], buf[w_off + wb:]]
+    for gz in guards:
+        assert bool((gz == 0xFF).all())

@@ -11,6 +11,7 @@
 #include <stdlib.h>
 #include <string.h>
 
+#include <algorithm>
 #include <vector>
 
 #include "../../include/vlasov.h"
@@ -29,7 +30,7 @@ constexpr int TB_MINB = 3;       // CTAs per SM the register budget is set for
 constexpr int FU_R = 11;         // consecutive outputs per lane in the theta stage of the one-pass kernel (odd)
 constexpr int FW_NSTG = 3;       // ring depth (groups of 12 rows) of the one-pass kernel
 constexpr int FW_NTW = 12;       // its theta warps = density partial rows per band
-constexpr int KEY_TUNE_GRAPH = 109, KEY_TUNE_PDL = 110;
+constexpr int KEY_TUNE_GRAPH = 109, KEY_TUNE_PDL = 110, KEY_TUNE_FEDGE = 108;
 constexpr int FU_PAD = 12;       // rows of padding of the theta weight tables (the last phase of a band reads on)
 constexpr int NCLS = 6;          // profiled kernel classes: theta x1, theta x2, p, rho+force, p+theta x2, p+theta x1
 constexpr int KEY_TUNE_FBANDS = 107;
@@ -85,6 +86,9 @@ struct Ctx {
     unsigned graph_kernels[2] = {0, 0};
     cudaStream_t cap_stream = nullptr;
     int fbands[3] = {0, 0, 0}, frpb[3] = {0, 0, 0}, fcols[3] = {0, 0, 0};
+    int fedge = 100;       // relative width (percent) of the first / last column block (KEY_TUNE_FEDGE)
+    int tune_fedge = 0;
+    int fx0 = 0, fxw = 0;  // source positions the column blocks of the one-pass kernel tile: [fx0, fx0 + fxw)
     bool onepass = false;
     int tune_fbands = 0;
     int fnw() const { return FW_NTW; }
@@ -300,19 +304,39 @@ int configure_theta_bulk() {
 // of the density partials).  Sets G.fbands[NST] = 0 when the grid does not qualify.
 template <typename T, int NST>
 int configure_fused() {
-    CU(cudaFuncSetAttribute(vl::strang_fused_ws_kernel<T, NST, FU_R, FW_NSTG, FW_NTW>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                            (int)vl::FusedWsCfg<T, NST, FU_R, FW_NSTG, FW_NTW>::SMEM_BYTES));
+    CU(cudaFuncSetAttribute(vl::strang_fused_ws_kernel<T, NST, FU_R, FW_NSTG, FW_NTW, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                            (int)vl::FusedWsCfg<T, NST, FU_R, FW_NSTG, FW_NTW, false>::SMEM_BYTES));
+    CU(cudaFuncSetAttribute(vl::strang_fused_ws_kernel<T, NST, FU_R, FW_NSTG, FW_NTW, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                            (int)vl::FusedWsCfg<T, NST, FU_R, FW_NSTG, FW_NTW, true>::SMEM_BYTES));
     const int np = G.np, nt = G.ntheta;
     G.fbands[NST] = 0;
     for (int j = 1; j < np; ++j)
         if (G.h_srow[j] > G.h_srow[j - 1]) return VLASOV_OK;  // shift wrapped around the circle: not monotonic
     if ((double)nt * sizeof(T) >= 2147483648.0) return VLASOV_OK;
     const int gran = G.fgran(sizeof(T));
-    const int cols = vl::fused_block_cols(nt, FU_R, gran);
+    // Zero-extended theta axis: a row's outputs [0, Ntheta) come from the source positions [S, Ntheta + S), S its integer
+    // shift, so the blocks tile [min(0, S_min), Ntheta + max(0, S_max)) (S of two half shifts; x0 even: 16-byte starts)
+    int x0 = 0, xw = nt;
+    if (G.bc_x != vl::BC_PERIODIC) {
+        int smin = 0, smax = 0;
+        for (int j = 0; j < np; ++j) {
+            smin = std::min(smin, 2 * G.h_srow[j]);
+            smax = std::max(smax, 2 * G.h_srow[j]);
+        }
+        if (smax - smin > 4 * nt) return VLASOV_OK;  // shifts of several domain lengths: the separate kernels
+        x0 = -((-smin + 1) & ~1);
+        xw = nt + smax - x0;
+    }
+    G.fx0 = x0;
+    G.fxw = xw;
+    // (narrower edge blocks were measured at 4096^2, 40 .. 100 %: no effect on the pass, so 100 unless tuned)
+    G.fedge = (G.bc_x != vl::BC_PERIODIC && NST == 2 && G.tune_fedge > 0) ? G.tune_fedge : 100;
+    const int edge_w = NST == 2 ? G.fedge : 100;
+    const int cols = vl::fused_block_cols(xw, FU_R, gran, edge_w);
     int wmin = nt;
     for (int c = 0; c < cols; ++c) {
         int i0, wd;
-        vl::fused_block_range(c, cols, nt, FU_R, gran, &i0, &wd);
+        vl::fused_block_range(c, cols, xw, FU_R, gran, &i0, &wd, edge_w);
         wmin = wd < wmin ? wd : wmin;
     }
     if (wmin < 1) return VLASOV_OK;
@@ -355,7 +379,7 @@ int configure_all() {
         if ((rc = configure_theta_bulk<T, 1>()) != 0) return rc;
         if ((rc = configure_theta_bulk<T, 2>()) != 0) return rc;
     }
-    G.onepass = (G.fuse >= 2) && (G.bc_x == vl::BC_PERIODIC) && (G.halo_lo + G.halo_hi == 0);
+    G.onepass = (G.fuse >= 2) && (G.halo_lo + G.halo_hi == 0);
     if (G.onepass) {
         if ((rc = configure_fused<T, 1>()) != 0) return rc;
         if ((rc = configure_fused<T, 2>()) != 0) return rc;
@@ -439,7 +463,7 @@ int prepare_tables() {
     row_tables(tau, srow, wrow);
     G.h_srow = srow;
     // composite weights of two equal half shifts, W = w * w (19 taps): the one-pass kernel applies both at once
-    constexpr int W2 = 20;  // FusedWsCfg<T, 2, ...>::WST
+    const int W2 = G.bc_x == vl::BC_PERIODIC ? 20 : 32;  // FusedWsCfg<T, 2, ..., ZX>::WST
     std::vector<double> wrow2((size_t)(np + FU_PAD) * W2, 0.0);
     for (int j = 0; j < np; ++j) {
         const double* w = &wrow[(size_t)j * vl::WROW_STRIDE];
@@ -450,6 +474,10 @@ int prepare_tables() {
             W[n] = acc;
         }
         W[19] = 2.0 * (double)srow[j];  // integer part of the two half shifts together
+        if (W2 == 32) {  // zero-extended theta axis: the single half shift too (rows near the ends apply it twice)
+            for (int m = 0; m < 10; ++m) W[20 + m] = w[m];
+            W[30] = (double)srow[j];
+        }
         if (G.prec == 32) {  // fp32 arithmetic: both tables hold the difference-form weights (vl::diff_form_weights)
             double U[18];
             vl::diff_form_weights(W, 19, 2 * vl::FD_C + 1, U);
@@ -731,9 +759,12 @@ int launch_fused(bool want_colsums) {
     a.fin = static_cast<const T*>(G.f[G.cur]);
     a.fout = static_cast<T*>(G.f[G.cur ^ 1]);
     a.force = G.force;
-    a.wtab = NST == 2 ? G.wrow2 : G.wrow;
+    a.wtab = NST == 2 ? G.wrow2 : G.wrow;  // (a zero-extended axis has the wider rows of FusedWsCfg<.., ZX = true>)
     a.bulk_ok = (G.ntheta % CW::EPV == 0) ? 1 : 0;
     a.gran = G.fgran(sizeof(T));
+    a.x0 = G.fx0;
+    a.edge_w = NST == 2 ? G.fedge : 100;
+    a.xw = G.fxw;
     a.colpart = want_colsums ? G.colpart_f : nullptr;
     a.ntheta = G.ntheta;
     a.np = G.np;
@@ -743,7 +774,11 @@ int launch_fused(bool want_colsums) {
     a.dp = (G.pmax - G.pmin) / (double)G.np;
     dim3 grid(G.fcols[NST], G.fbands[NST]);
     prof_begin(NST == 2 ? 4 : 5);
-    CU(launch_pdl(vl::strang_fused_ws_kernel<T, NST, FU_R, FW_NSTG, FW_NTW>, grid, dim3(CW::NT), CW::SMEM_BYTES, a));
+    if (G.bc_x == vl::BC_PERIODIC)
+        CU(launch_pdl(vl::strang_fused_ws_kernel<T, NST, FU_R, FW_NSTG, FW_NTW, false>, grid, dim3(CW::NT), CW::SMEM_BYTES, a));
+    else
+        CU(launch_pdl(vl::strang_fused_ws_kernel<T, NST, FU_R, FW_NSTG, FW_NTW, true>, grid, dim3(CW::NT),
+                      vl::FusedWsCfg<T, NST, FU_R, FW_NSTG, FW_NTW, true>::SMEM_BYTES, a));
     prof_end(NST == 2 ? 4 : 5);
     LAUNCH_CHECK();
     G.cur ^= 1;
@@ -973,6 +1008,7 @@ int vlasov_set_param(int key, double value) {
         case KEY_TUNE_FBANDS: G.tune_fbands = (int)value; break;
         case KEY_TUNE_GRAPH: G.graphs = (value != 0.0); break;
         case KEY_TUNE_PDL: G.pdl = (value != 0.0); break;
+        case KEY_TUNE_FEDGE: G.tune_fedge = (int)value; break;
         case VLASOV_KEY_PROFILE: G.profile = (value != 0.0); break;
         case KEY_TUNE_NW1: G.tune_nw1 = (int)value; break;
         case KEY_TUNE_NW2: G.tune_nw2 = (int)value; break;

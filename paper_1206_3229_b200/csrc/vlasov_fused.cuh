@@ -51,6 +51,9 @@ struct FusedArgs {
                              //   e: fp32 residual of the row's weights, weight_residual)
     double* colpart;         // [nbands * NW][Ntheta], zero on entry; column sums are ADDED (may be null)
     int ntheta, np, bc_p, rows_per_band, bulk_ok, gran;
+    int edge_w;              // relative width (percent) of the first and last column block (fused_block_range)
+    int x0, xw;              // the column blocks tile the source positions [x0, x0 + xw): [0, Ntheta) on a periodic axis; on a
+                             // zero-extended one (ZX) also what the rows drift beyond the ends (x0 <= 0, even)
     double dt, dp;
 };
 
@@ -80,14 +83,38 @@ __device__ __forceinline__ void red_add_f64(double* addr, double v) {
 // elements per 16 bytes makes every block start on a 16-byte boundary, gran = 1 is the finest split) and the
 // granules are dealt out evenly: block c of `cols` gets granules [c U / cols, (c + 1) U / cols), at most 32 lanes.
 // Only the last block can end inside a lane.
-__host__ __device__ inline int fused_block_cols(int ntheta, int R, int gran) {
+// edge_w (percent, 100 = like the others): relative width of the first and the last block.  On a zero-extended axis
+// the rows of those two blocks apply the two half shifts one after the other (half as many FMAs again), and with one
+// CTA per SM the pass takes as long as its slowest block: they get fewer columns.
+__host__ __device__ inline long long fused_block_cum(int c, int cols, int edge_w) {  // weight of the blocks before c
+    if (cols < 3 || edge_w == 100) return 100LL * c;
+    if (c == 0) return 0;
+    if (c == cols) return 100LL * (cols - 2) + 2LL * edge_w;
+    return edge_w + 100LL * (c - 1);
+}
+__host__ __device__ inline int fused_block_cols(int ntheta, int R, int gran, int edge_w = 100) {
     const int U = (ntheta + R * gran - 1) / (R * gran);
     const int per = 32 / gran;
-    return (U + per - 1) / per;
+    int cols = (U + per - 1) / per;
+    if (edge_w != 100 && cols >= 3) {  // smallest count whose widest (inner) block still fits the 32 lanes
+        for (;; ++cols) {
+            const long long tot = fused_block_cum(cols, cols, edge_w);
+            bool ok = true;
+            for (int c = 0; c < cols && ok; ++c) {
+                const long long u0 = (long long)U * fused_block_cum(c, cols, edge_w) / tot,
+                                u1 = (long long)U * fused_block_cum(c + 1, cols, edge_w) / tot;
+                ok = (u1 - u0) <= per;
+            }
+            if (ok) break;
+        }
+    }
+    return cols;
 }
-__host__ __device__ inline void fused_block_range(int c, int cols, int ntheta, int R, int gran, int* i0, int* width) {
+__host__ __device__ inline void fused_block_range(int c, int cols, int ntheta, int R, int gran, int* i0, int* width,
+                                                  int edge_w = 100) {
     const long long U = (ntheta + R * gran - 1) / (R * gran);
-    const int u0 = (int)((long long)c * U / cols), u1 = (int)((long long)(c + 1) * U / cols);
+    const long long tot = fused_block_cum(cols, cols, edge_w);
+    const int u0 = (int)(U * fused_block_cum(c, cols, edge_w) / tot), u1 = (int)(U * fused_block_cum(c + 1, cols, edge_w) / tot);
     const int e = u1 * R * gran < ntheta ? u1 * R * gran : ntheta;
     *i0 = u0 * R * gran;
     *width = e - u0 * R * gran;

@@ -33,7 +33,7 @@ namespace vl {
 #ifndef VL_FW_NOB
 #define VL_FW_NOB 1
 #endif
-template <typename T, int NST, int R, int NSTG, int NTW_ = 8>
+template <typename T, int NST, int R, int NSTG, int NTW_ = 8, bool ZX = false>
 struct FusedWsCfg {
     static constexpr int NOB = VL_FW_NOB;               // output tiles per theta warp
     static constexpr int NPW = 4, NTW = NTW_;            // p warps (one warpgroup), theta warps (two or three warpgroups)
@@ -49,7 +49,10 @@ struct FusedWsCfg {
     static constexpr int SPG = RG / SUB;                // sub-slots per group
     static constexpr int NSUB = NSTG * SPG;
     static constexpr int NTAP = NST == 2 ? 19 : 10;
-    static constexpr int WST = NST == 2 ? 20 : WROW_STRIDE;
+    // weight row: NST = 1: w_0..w_9, s, -;  NST = 2: W_0..W_18, 2 s, and for a zero-extended theta axis (ZX) also the ten
+    // weights of ONE half shift and its s (entries 20..30): the rows near the ends of the axis apply the two half shifts
+    // one after the other, because the first one is cropped to [0, Ntheta) before the second reads it
+    static constexpr int WST = NST == 2 ? (ZX ? 32 : 20) : WROW_STRIDE;
     static constexpr int TI = 32 * R;
     static constexpr int NTA = TI + NTAP - 1;
     static constexpr int EPV = 16 / (int)sizeof(T);
@@ -75,9 +78,9 @@ struct FusedWsCfg {
     static_assert(NSTG >= 2 && W_COPIES <= 32, "");
 };
 
-template <typename T, int NST, int R, int NSTG, int NTW_>
+template <typename T, int NST, int R, int NSTG, int NTW_, bool ZX>
 __global__ void __launch_bounds__((4 + NTW_) * 32, 1) strang_fused_ws_kernel(const FusedArgs<T> arg) {
-    using C = FusedWsCfg<T, NST, R, NSTG, NTW_>;
+    using C = FusedWsCfg<T, NST, R, NSTG, NTW_, ZX>;
     constexpr int NTAP = C::NTAP, NTA = C::NTA, WST = C::WST, EPV = C::EPV, OB = C::OB, PITCH = C::PITCH, RG = C::RG,
                   SUB = C::SUB, SPG = C::SPG, NSUB = C::NSUB, CPT = C::CPT, NPT = C::NPT, NTW = C::NTW;
     constexpr unsigned FULL = 0xffffffffu;
@@ -92,7 +95,8 @@ __global__ void __launch_bounds__((4 + NTW_) * 32, 1) strang_fused_ws_kernel(con
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int ntheta = arg.ntheta, np = arg.np;
     int i0, qmax;
-    fused_block_range((int)blockIdx.x, (int)gridDim.x, ntheta, R, arg.gran, &i0, &qmax);
+    fused_block_range((int)blockIdx.x, (int)gridDim.x, arg.xw, R, arg.gran, &i0, &qmax, arg.edge_w);
+    i0 += arg.x0;  // ZX: may be negative or reach beyond Ntheta (source columns out there are zeros)
     const int band = blockIdx.y;
     const int jA = band * arg.rows_per_band;
     const int nrows = min(np, jA + arg.rows_per_band) - jA;
@@ -108,6 +112,16 @@ __global__ void __launch_bounds__((4 + NTW_) * 32, 1) strang_fused_ws_kernel(con
             ptx::mbar_init(&empty[k], SUB);
         }
         ptx::fence_mbar_init();
+    }
+    if constexpr (ZX) {
+        // zero extension in theta: the source columns of this CTA outside [0, Ntheta) are zeros.  Their ring columns are
+        // zero-filled here, once, by everybody; the p threads that own them issue no copies and compute 0 from 0.
+        const int cl = i0 - 4 * NST;  // column of q = 0
+        const int nlo = min(NTA, max(0, -cl)), nhi = min(NTA, max(0, cl + NTA - ntheta));
+        for (int e = tid; e < NSTG * RG * (nlo + nhi); e += C::NT) {
+            const int r = e / (nlo + nhi), qq = e - r * (nlo + nhi);
+            ring[(size_t)r * PITCH + (qq < nlo ? qq : NTA - nhi + (qq - nlo))] = T(0);
+        }
     }
     __syncthreads();
     // everything above is independent of the force and of f; from here on both are read (and the density partials
@@ -130,7 +144,13 @@ __global__ void __launch_bounds__((4 + NTW_) * 32, 1) strang_fused_ws_kernel(con
         for (int k = 0; k < CPT; ++k) {
             const int q = tid + k * NPT;
             act[k] = q < NTA;
-            const int c = wrap_index(i0 - 4 * NST + q, ntheta);
+            int c = i0 - 4 * NST + q;
+            if constexpr (ZX) {  // zero extension in theta: columns outside [0, Ntheta) are zeros and stay zeros
+                if ((unsigned)c >= (unsigned)ntheta) act[k] = false;
+                c = act[k] ? c : 0;
+            } else {
+                c = wrap_index(c, ntheta);
+            }
             double sf, a;
             split_shift(-((act[k] ? arg.force[c] : 0.0) * arg.dt) / arg.dp, &sf, &a);
             int s;
@@ -222,6 +242,7 @@ __global__ void __launch_bounds__((4 + NTW_) * 32, 1) strang_fused_ws_kernel(con
                     const int r = sub * SUB + rr;
 #pragma unroll
                     for (int k = 0; k < CPT; ++k) {  // columns beyond NTA compute on whatever the ring holds: never read
+                        // (ZX: a column outside [0, Ntheta) has no copies and a zero-filled ring column: it computes 0)
                         v[k][(r + 9) % 12] = sl[r * PITCH + k * NPT];
                         T acc;
                         if constexpr (sizeof(T) == 4) {
@@ -292,8 +313,8 @@ __global__ void __launch_bounds__((4 + NTW_) * 32, 1) strang_fused_ws_kernel(con
         for (int u = 0; u < K; ++u) {
             if (lane == 0 && cpw != nullptr) {
                 int cidx = cbase + u;
-                if (cidx >= ntheta) cidx -= ntheta;
-                ptx::red_add_f64(cpw + cidx, csum[u]);
+                if (!ZX && cidx >= ntheta) cidx -= ntheta;
+                if (!ZX || (unsigned)cidx < (unsigned)ntheta) ptx::red_add_f64(cpw + cidx, csum[u]);  // ZX: outside = dropped
             }
         }
         double in[K];
@@ -308,7 +329,7 @@ __global__ void __launch_bounds__((4 + NTW_) * 32, 1) strang_fused_ws_kernel(con
         for (int u = 0; u < K; ++u) csum[R - K + u] = in[u];
         curS -= K;
         cbase += K;
-        if (cbase >= ntheta) cbase -= ntheta;
+        if (!ZX && cbase >= ntheta) cbase -= ntheta;
     };
 
     if (tw < nrows && wlane) ptx::cp_async<16>(wb_u32, wsrc);
@@ -336,14 +357,47 @@ __global__ void __launch_bounds__((4 + NTW_) * 32, 1) strang_fused_ws_kernel(con
         const int S = (int)Wr[NTAP];
         if (!have) {
             curS = S;
-            cbase = wrap_index(i0 - S, ntheta);
+            cbase = ZX ? i0 - S : wrap_index(i0 - S, ntheta);
             have = true;
         }
         while (curS - S >= 2) shift_sums(std::integral_constant<int, 2>());
         if (curS > S) shift_sums(std::integral_constant<int, 1>());
 
         T out[R];
-        if constexpr (sizeof(T) == 4) {
+        bool edge_row = false;
+        if constexpr (ZX && NST == 2) {
+            // Zero-extended theta axis: the first half shift is cropped to [0, Ntheta) before the second reads it (the
+            // oracle stores f_I on the grid), so the composite weights W = w * w are right only where no intermediate
+            // value the row needs lies outside.  Intermediate column of the warp's h[j]: cbase + lane R + j + s - 4.
+            const int h0 = cbase + (int)Wr[30] - FD_C;
+            edge_row = h0 < 0 || h0 + 32 * R + 8 >= ntheta;
+            if (edge_row) {  // warp-uniform: the two half shifts one after the other (eqs (12), (9)), cropped in between
+#pragma unroll
+                for (int k = R + NH - 1; k < R + NTAP - 1; ++k) x[k] = grow[k];
+                __syncwarp();
+                if (lane == 0) ptx::mbar_arrive_u32(empty_u32 + boff);
+                T w1[10];
+#pragma unroll
+                for (int m = 0; m < 10; ++m) w1[m] = (T)Wr[20 + m];
+                T h[R + 9];
+#pragma unroll
+                for (int j = 0; j < R + 9; ++j) {
+                    T acc = w1[0] * x[j];
+#pragma unroll
+                    for (int m = 1; m < 10; ++m) acc = fma(w1[m], x[j + m], acc);
+                    h[j] = (unsigned)(h0 + lane * R + j) < (unsigned)ntheta ? acc : T(0);
+                }
+#pragma unroll
+                for (int q = 0; q < R; ++q) {
+                    T acc = w1[0] * h[q];
+#pragma unroll
+                    for (int m = 1; m < 10; ++m) acc = fma(w1[m], h[q + m], acc);
+                    out[q] = acc;
+                }
+            }
+        }
+        if (edge_row) {
+        } else if constexpr (sizeof(T) == 4) {
             // fp32 arithmetic: difference form (diff_form_weights; the table holds U_0 .. U_{NTAP-2}), centre tap CT
             constexpr int CT = NST == 2 ? 2 * FD_C + 1 : FD_C;
 #pragma unroll
@@ -420,9 +474,14 @@ __global__ void __launch_bounds__((4 + NTW_) * 32, 1) strang_fused_ws_kernel(con
                 if (lane == 0 && nb > 0)
                     ptx::bulk_s2g_u32(orow + gcol + h, O_u32 + (uint32_t)((qb + h) * sizeof(T)), (unsigned)(nb * sizeof(T)));
             };
-            const int qa = min(qmax, ntheta - base);
-            store_piece(0, qa, base);
-            if (qa < qmax) store_piece(qa, qmax - qa, 0);
+            if constexpr (ZX) {  // the part of the row inside [0, Ntheta): one piece, the rest is dropped
+                const int qlo = max(0, -base), qhi = min(qmax, ntheta - base);
+                if (qhi > qlo) store_piece(qlo, qhi - qlo, base + qlo);
+            } else {
+                const int qa = min(qmax, ntheta - base);
+                store_piece(0, qa, base);
+                if (qa < qmax) store_piece(qa, qmax - qa, 0);
+            }
             if (lane == 0) ptx::bulk_commit();
         } else {
 #pragma unroll
@@ -433,8 +492,8 @@ __global__ void __launch_bounds__((4 + NTW_) * 32, 1) strang_fused_ws_kernel(con
                 const int q = lane + 32 * k;
                 if (q < qmax) {
                     int i = base + q;
-                    if (i >= ntheta) i -= ntheta;
-                    orow[i] = O[q];
+                    if (!ZX && i >= ntheta) i -= ntheta;
+                    if (!ZX || (unsigned)i < (unsigned)ntheta) orow[i] = O[q];
                 }
             }
         }
@@ -458,8 +517,8 @@ __global__ void __launch_bounds__((4 + NTW_) * 32, 1) strang_fused_ws_kernel(con
         for (int q = 0; q < R; ++q) {
             if (q < nv && csum[q] != 0.0) {
                 int cidx = cbase + lane * R + q;
-                if (cidx >= ntheta) cidx -= ntheta;
-                ptx::red_add_f64(cpw + cidx, csum[q]);
+                if (!ZX && cidx >= ntheta) cidx -= ntheta;
+                if (!ZX || (unsigned)cidx < (unsigned)ntheta) ptx::red_add_f64(cpw + cidx, csum[q]);
             }
         }
     }

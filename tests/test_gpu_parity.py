@@ -145,6 +145,32 @@ def test_one_pass_p_then_theta(grid, bc_p, which, dt, amp):
     g.close()
 
 
+@pytest.mark.parametrize("grid", ONEPASS_GRIDS + [(4096, 40)])
+@pytest.mark.parametrize("bc_p", [BC_ZERO, BC_PERIODIC])
+@pytest.mark.parametrize("which,dt,amp", [(1, 0.1, 0.5), (2, 0.1, 0.5), (2, 0.45, 30.0), (2, 2.5, 3.0), (1, 9.0, 2000.0), (2, 3.0, 0.0)])
+def test_one_pass_zero_extended_theta_axis(grid, bc_p, which, dt, amp):
+    """the same with a zero-extended theta axis (the sheet model, BASELINE.json cfg 4): source columns beyond the ends are
+    zeros, outputs beyond them are dropped, and near the ends the two half shifts are applied one after the other because
+    the first is cropped to the grid before the second reads it (noise on every node, so the crop matters)"""
+    dom = (-PI, PI, -4.0, 4.0)
+    f0 = smooth_state(grid[0], grid[1], dom, seed=8) + 0.3
+    th = inputs.nodes(dom[0], dom[1], grid[0])
+    F = amp * np.sin(2 * th + 0.1) + 0.3 * amp
+    o, g = pair(MODEL_SHEET, grid, dom, dt, f0, bc_p=bc_p)
+    o.p_sweep(dt, force=F)
+    for _ in range(which):
+        o.theta_sweep(0.5 * dt)
+    g.set_force(F)
+    if dt < 1.0 and grid[1] >= 2:   # moderate steps take the one-pass kernel (a shift of several domain lengths does not)
+        assert g.info()["onepass"] == 1
+    g.substep(vb.SUB_P_THETA_TWICE if which == 2 else vb.SUB_P_THETA_HALF)
+    fo = o.download()
+    assert rel_err(g.download(), fo) < 1e-13
+    rho_o = o.density()
+    assert np.max(np.abs(g.density() - rho_o)) <= 1e-13 * np.max(np.abs(rho_o))
+    g.close()
+
+
 @pytest.mark.parametrize("fbands", [1, 3, 50])
 def test_one_pass_band_split_does_not_change_the_result(fbands):
     dom = (-PI, PI, -4.0, 4.0)

@@ -404,16 +404,16 @@ def run_cuda(args):
                "sample": "%d Strang step(s) of the same workload on its full %dx%d grid (%.1f s of wall time), "
                          "oracle/vlasov_oracle.c with OpenMP over lines" % (done, nt, npp, el)}
 
-    cfg = dict(cfg)
-    cfg.update({"passes_per_step": passes / K, "fuse": args.fuse,
-                "parallelism": "replicas x%d" % world if world > 1 else "single GPU"})
+    # `config` is the same object in both arms (the driver compares them); what is particular to this run sits in `run`
+    run = {"passes_per_step": passes / K, "fuse": args.fuse, "pdl": args.pdl, "graph": args.graph,
+           "parallelism": "replicas x%d" % world if world > 1 else "single GPU"}
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64" if prec == 64 else "f32", "data": "synthetic", "config": cfg,
         "timing": {"reps": len(reps_ms), "reps_ms": reps_ms, "statistic": "median repetition of vlasov_step(K)",
                    "note": "K steps = K + 1 passes (first half theta shift + last pass with one half shift)"},
-        "launch": info, "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "kernels": kern,
+        "run": run, "launch": info, "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "kernels": kern,
         "cpu_baseline": cpu, "final_moments": {"t": mom[0], "mass": mom[1], "E": mom[7], "Mx": mom[5]},
     }
     print(json.dumps(line))

@@ -77,8 +77,15 @@ extern "C" {
                                   and the halo exchange happen BETWEEN the stages of vlasov_substep and belong to the
                                   caller (torch.distributed / NCCL); vlasov_step refuses.  upload / download move the
                                   owned rows; vlasov_state_ptr is the start of the buffer (first halo row).           */
-/* keys 101..110 (launch-shape overrides: warps, bands, segment lengths, kernel variant) exist for the tests and
- * the tuning sweeps only; see binding.py KEY_TUNE_*.  Results never depend on them beyond rounding order.   */
+/* Tuning keys (tests and sweeps; results never depend on them beyond rounding order).  0 = automatic.
+ *   101 TUNE_NW1, 102 TUNE_NW2   warps per CTA of the generic theta kernel (one / two half shifts)
+ *   103 TUNE_BANDS               bands of rows of the theta kernels
+ *   104 TUNE_PSEG, 105 TUNE_PTX  rows per segment / threads per CTA of the p kernel (two-pass path)
+ *   106 TUNE_GENERIC             1: the generic theta kernel even where rows are multiples of 16 bytes
+ *   107 TUNE_FBANDS              bands of rows of the one-pass kernel
+ *   108 TUNE_FEDGE               zero-extended theta: width (percent) of the first / last column block of the one-pass kernel
+ *   109 TUNE_GRAPH               0: plain launches instead of the captured step-pair graphs (default 1)
+ *   110 TUNE_PDL                 0: ordinary launches instead of programmatic dependent launch (default 1)              */
 
 /* sub-steps for vlasov_substep (parity tests of single stages; same kernels as vlasov_step) */
 #define VLASOV_SUB_THETA_HALF 0  /* eq (9)/(12): f(x - p dt/2, p), also leaves the column sums for the force */

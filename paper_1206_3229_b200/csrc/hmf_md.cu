@@ -9,9 +9,8 @@
 // M is not reduced by a kernel of its own: every block of the next pass adds the previous pass's block partials in
 // index order (a few thousand doubles from L2), which is the same number in every block and from run to run.
 // A step is three such passes (the half drifts that end one step and open the next share a pass): 3 n + 1 launches
-// for n steps, 32 bytes per particle and pass (theta and p read and written).  The pass is bound by HBM and, about
-// equally, by the two fp64 sincos per particle (the angles change between the kick and the sums, and storing the
-// sine and cosine would double the traffic).
+// for n steps, 32 bytes per particle and pass (theta and p read and written).  Per particle and pass: one fp64 sincos
+// (for the kick) and a rotation of it by the small drift angle (rotate_small) for the sums of the new angles.
 #include <cuda_runtime.h>
 #include <math.h>
 #include <stdint.h>
@@ -59,6 +58,33 @@ __device__ __forceinline__ double2 block_sum2(double x, double y, double2* red) 
     return t;
 }
 
+// (cos, sin) of theta + d from (c, s) = (cos, sin) of theta by a rotation, with sin d and cos d from their Taylor
+// polynomials (|d| <= 1/2: remainders d^17/17! = 2e-20 and d^18/18! = 6e-22): a third of the instructions of a second
+// sincos.  The result only enters the sums (M_x, M_y) of this pass -- the angles themselves are advanced by the plain
+// addition -- so its rounding (a few 1e-16) does not accumulate over the steps.
+__device__ __forceinline__ void rotate_small(double c, double s, double d, double* c2, double* s2) {
+    const double z = d * d;
+    double ps = -1.0 / 1307674368000.0;           // -1/15!
+    ps = fma(ps, z, 1.0 / 6227020800.0);          //  1/13!
+    ps = fma(ps, z, -1.0 / 39916800.0);           // -1/11!
+    ps = fma(ps, z, 1.0 / 362880.0);              //  1/9!
+    ps = fma(ps, z, -1.0 / 5040.0);               // -1/7!
+    ps = fma(ps, z, 1.0 / 120.0);                 //  1/5!
+    ps = fma(ps, z, -1.0 / 6.0);                  // -1/3!
+    const double sd = fma(ps * z, d, d);          // d + d^3 (...)
+    double pc = 1.0 / 20922789888000.0;           //  1/16!
+    pc = fma(pc, z, -1.0 / 87178291200.0);        // -1/14!
+    pc = fma(pc, z, 1.0 / 479001600.0);           //  1/12!
+    pc = fma(pc, z, -1.0 / 3628800.0);            // -1/10!
+    pc = fma(pc, z, 1.0 / 40320.0);               //  1/8!
+    pc = fma(pc, z, -1.0 / 720.0);                // -1/6!
+    pc = fma(pc, z, 1.0 / 24.0);                  //  1/4!
+    pc = fma(pc, z, -0.5);                        // -1/2!
+    const double cdm1 = pc * z;                   // cos d - 1
+    *c2 = fma(c, cdm1, c) - s * sd;               // c cos d - s sin d
+    *s2 = fma(s, cdm1, s) + c * sd;               // s cos d + c sin d
+}
+
 __global__ void __launch_bounds__(MD_NT) md_kick_drift_kernel(const MdArgs a) {
     __shared__ double2 red[MD_NT / 32];
     double mx = 0.0, my = 0.0;
@@ -85,15 +111,20 @@ __global__ void __launch_bounds__(MD_NT) md_kick_drift_kernel(const MdArgs a) {
         }
 #pragma unroll
         for (int u = 0; u < MD_UNROLL; ++u) {
+            double s2, c2;
             if (kick) {  // eq (7): F = -sin(theta) M_x + cos(theta) M_y
                 double s, c;
                 sincos(th[u], &s, &c);
                 pp[u] += -s * mx + c * my;
                 __stcs(a.p + i + u * stride, pp[u]);
+                const double d = a.drift * pp[u];
+                th[u] += d;
+                if (fabs(d) <= 0.5) rotate_small(c, s, d, &c2, &s2);
+                else sincos(th[u], &s2, &c2);
+            } else {
+                th[u] += a.drift * pp[u];
+                sincos(th[u], &s2, &c2);
             }
-            th[u] += a.drift * pp[u];
-            double s2, c2;
-            sincos(th[u], &s2, &c2);
             accx += c2;
             accy += s2;
             __stcs(a.theta + i + u * stride, th[u]);
@@ -101,15 +132,20 @@ __global__ void __launch_bounds__(MD_NT) md_kick_drift_kernel(const MdArgs a) {
     }
     for (; i < a.n; i += stride) {
         double th = __ldcs(a.theta + i), pp = __ldcs(a.p + i);
+        double s2, c2;
         if (kick) {
             double s, c;
             sincos(th, &s, &c);
             pp += -s * mx + c * my;
             __stcs(a.p + i, pp);
+            const double d = a.drift * pp;
+            th += d;
+            if (fabs(d) <= 0.5) rotate_small(c, s, d, &c2, &s2);
+            else sincos(th, &s2, &c2);
+        } else {
+            th += a.drift * pp;
+            sincos(th, &s2, &c2);
         }
-        th += a.drift * pp;
-        double s2, c2;
-        sincos(th, &s2, &c2);
         accx += c2;
         accy += s2;
         __stcs(a.theta + i, th);

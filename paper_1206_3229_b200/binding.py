@@ -38,6 +38,11 @@ MD_EXPORTS = (
 )
 
 
+# include/hmf_noalloc.h: the one entry point that allocates nothing
+NOALLOC_EXPORTS = ("hmf_noalloc_moments", "hmf_noalloc_last_error")
+NOALLOC_MAX_PARTICLES = 33554432
+
+
 class VlasovError(RuntimeError):
     def __init__(self, code: int, what: str, msg: str):
         super().__init__("%s failed with code %d: %s" % (what, code, msg))
@@ -103,6 +108,9 @@ def load(build_if_missing: bool = True):
         "hmf_md_launch_count": (ci, [ctypes.POINTER(ctypes.c_ulonglong)]),
         "hmf_md_free": (None, []),
         "hmf_md_last_error": (ctypes.c_char_p, []),
+        # include/hmf_noalloc.h
+        "hmf_noalloc_moments": (ci, [vp, vp, ctypes.c_longlong, cd, vp, vp]),
+        "hmf_noalloc_last_error": (ctypes.c_char_p, []),
     }
     for name, (res, args) in sig.items():
         fn = getattr(lib, name)
@@ -349,6 +357,15 @@ def hmf_md_launch_count() -> int:
     out = ctypes.c_ulonglong(0)
     _chk_md(load().hmf_md_launch_count(ctypes.byref(out)), "hmf_md_launch_count")
     return int(out.value)
+
+
+def hmf_noalloc_moments(theta_ptr: int, p_ptr: int, n: int, t: float, out_ptr: int, stream: int = 0) -> None:
+    """include/hmf_noalloc.h: the moments of n particles (device pointers of the caller, out_ptr: 8 doubles on the device),
+    enqueued on `stream` (a cudaStream_t as an integer); calls no cudaMalloc.  Argument marshalling only."""
+    rc = load().hmf_noalloc_moments(ctypes.c_void_p(theta_ptr), ctypes.c_void_p(p_ptr), int(n), float(t),
+                                    ctypes.c_void_p(out_ptr), ctypes.c_void_p(stream))
+    if rc < 0:
+        raise VlasovError(rc, "hmf_noalloc_moments", (load().hmf_noalloc_last_error() or b"").decode())
 
 
 class HmfMd:

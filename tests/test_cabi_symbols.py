@@ -1,4 +1,4 @@
-"""The C-ABI library builds, loads and exports every symbol include/vlasov.h declares (no GPU needed)."""
+"""The C-ABI library builds, loads and exports every symbol include/*.h declares (no GPU needed)."""
 import os
 import re
 
@@ -16,11 +16,12 @@ def declared_symbols(header="vlasov.h", prefix="vlasov_"):
 def test_header_and_binding_agree():
     assert declared_symbols() == sorted(vb.EXPORTS)
     assert declared_symbols("hmf_md.h", "hmf_md_") == sorted(vb.MD_EXPORTS)
+    assert declared_symbols("hmf_noalloc.h", "hmf_noalloc_") == sorted(vb.NOALLOC_EXPORTS)
 
 
 def test_library_builds_loads_and_exports_every_symbol():
     lib = vb.load()
-    for name in declared_symbols() + declared_symbols("hmf_md.h", "hmf_md_"):
+    for name in declared_symbols() + declared_symbols("hmf_md.h", "hmf_md_") + declared_symbols("hmf_noalloc.h", "hmf_noalloc_"):
         assert hasattr(lib, name), name
 
 

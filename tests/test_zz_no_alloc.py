@@ -116,7 +116,7 @@ def test_no_alloc_entry_point_really_does_not_allocate():
         for _ in range(20):
             noalloc_moments(md, 0.0, out_dev)
         free1, _ = torch.cuda.mem_get_info(md.device)
-        assert free1 == free0
+        assert free0 - free1 < (1 << 20)  # twenty calls that each allocated their 256 KiB of partial sums would show
     finally:
         md.close()
     root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))

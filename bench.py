@@ -292,6 +292,8 @@ def run_cuda(args):
         params["tune_fbands"] = args.fbands
     if args.fedge > 0:
         params["tune_fedge"] = args.fedge
+    if args.tile > 0:
+        params["tune_tile"] = args.tile
     g = vb.Vlasov(c["model"], c["grid"], c["domain"], c["dt"], precision=prec, device="cuda:%d" % local_rank, **params)
     g.upload(f0)
     pts = float(nt) * float(npp)
@@ -679,6 +681,8 @@ def main():
     ap.add_argument("--fuse", type=int, default=2, choices=[0, 1, 2],
                     help="passes per step: 2 = one (p + theta in one kernel, default), 1 = two, 0 = three")
     ap.add_argument("--fbands", type=int, default=0, help="bands of rows of the one-pass kernel (0 = automatic)")
+    ap.add_argument("--tile", type=int, default=0, choices=[0, 1, 2],
+                    help="one-pass step of small grids by the tile kernel: 0 by size (default), 1 wherever it applies, 2 never")
     ap.add_argument("--fedge", type=int, default=0, help="zero-extended x: width (percent) of the two edge column blocks (0 = automatic)")
     ap.add_argument("--graph", type=int, default=1, choices=[0, 1],
                     help="1 (default): steady-state step pairs are launched as CUDA graphs, 0: plain launches")

@@ -85,7 +85,10 @@ extern "C" {
  *   107 TUNE_FBANDS              bands of rows of the one-pass kernel
  *   108 TUNE_FEDGE               zero-extended theta: width (percent) of the first / last column block of the one-pass kernel
  *   109 TUNE_GRAPH               0: plain launches instead of the captured step-pair graphs (default 1)
- *   110 TUNE_PDL                 0: ordinary launches instead of programmatic dependent launch (default 1)              */
+ *   110 TUNE_PDL                 0: ordinary launches instead of programmatic dependent launch (default 1)
+ *   111 TUNE_TILE                one-pass step of small grids (fp64, periodic theta) by the tile kernel strang_tile_kernel instead of
+ *                                the warp-specialised one: 0 by size (default: up to 4.5e6 grid points, i.e. 2048^2), 1 whenever its conditions
+ *                                hold, 2 never                                                                         */
 
 /* sub-steps for vlasov_substep (parity tests of single stages; same kernels as vlasov_step) */
 #define VLASOV_SUB_THETA_HALF 0  /* eq (9)/(12): f(x - p dt/2, p), also leaves the column sums for the force */
@@ -202,8 +205,8 @@ int vlasov_kernel_times(double out[12]);
 
 /* Fill out[0..n) (host) with implementation facts for reports: {SM count, theta-kernel CTAs, p-kernel CTAs,
  * bands, warps per theta CTA (2-shift), warps per theta CTA (1-shift), theta1 CTAs, p segment length, p threads,
- * bulk-copy theta kernel in use, one-pass kernel in use (0/1), its CTAs, bands, rows per band}; returns how many
- * were written. */
+ * bulk-copy theta kernel in use, one-pass kernel in use (0/1), its CTAs, bands, rows per band, whether it is the tile
+ * kernel of small grids (0/1)}; returns how many were written. */
 int vlasov_info(double* out, int n);
 
 void vlasov_free(void);

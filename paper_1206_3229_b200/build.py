@@ -17,7 +17,7 @@ CSRC = os.path.join(HERE, "csrc")
 ROOT = os.path.dirname(HERE)
 LIB = os.path.join(CSRC, "libvlasov_b200.so")
 SOURCES = [os.path.join(CSRC, "vlasov_api.cu"), os.path.join(CSRC, "hmf_md.cu"), os.path.join(CSRC, "hmf_noalloc.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, h) for h in ("vlasov_kernels.cuh", "vlasov_theta_bulk.cuh", "vlasov_ptx.cuh", "vlasov_fused.cuh", "vlasov_fused_ws.cuh", "vlasov_gs.cuh")] + [
+DEPS = SOURCES + [os.path.join(CSRC, h) for h in ("vlasov_kernels.cuh", "vlasov_theta_bulk.cuh", "vlasov_ptx.cuh", "vlasov_fused.cuh", "vlasov_fused_ws.cuh", "vlasov_tile.cuh", "vlasov_gs.cuh")] + [
     os.path.join(ROOT, "include", "vlasov.h"), os.path.join(ROOT, "include", "hmf_md.h"), os.path.join(ROOT, "include", "hmf_noalloc.h")]
 
 

@@ -19,6 +19,7 @@
 #include "vlasov_theta_bulk.cuh"
 #include "vlasov_fused.cuh"
 #include "vlasov_fused_ws.cuh"
+#include "vlasov_tile.cuh"
 #include "vlasov_gs.cuh"
 
 namespace {
@@ -27,13 +28,26 @@ constexpr int R_THETA = 9;       // consecutive outputs per lane in the theta ke
 constexpr int TB_NS = 3;         // rows in flight per warp in the bulk-copy theta kernel
 constexpr int TB_WARPS = 4;      // warps per CTA (independent pipelines)
 constexpr int TB_MINB = 3;       // CTAs per SM the register budget is set for
-constexpr int FU_R = 11;         // consecutive outputs per lane in the theta stage of the one-pass kernel (odd)
-constexpr int FW_NSTG = 3;       // ring depth (groups of 12 rows) of the one-pass kernel
-constexpr int FW_NTW = 12;       // its theta warps = density partial rows per band
+#ifndef VL_FW_NTW_
+#define VL_FW_NTW_ 12
+#endif
+// consecutive outputs per lane in the theta stage of the one-pass kernel (odd): fp64 11 of a ring row of 384 columns,
+// fp32 15 of a ring row of 512 (FusedWsCfg::CPT; 8192^2 fp32: 286 -> 302 Gpts/s)
+#ifdef VL_FU_R
+template <typename T> constexpr int FU_R = VL_FU_R;
+#else
+template <typename T> constexpr int FU_R = sizeof(T) == 4 ? 15 : 11;
+#endif
+#ifndef VL_FW_NSTG
+#define VL_FW_NSTG 3
+#endif
+constexpr int FW_NSTG = VL_FW_NSTG;       // ring depth (groups of 12 rows) of the one-pass kernel
+constexpr int FW_NTW = VL_FW_NTW_;       // its theta warps = density partial rows per band
 constexpr int KEY_TUNE_GRAPH = 109, KEY_TUNE_PDL = 110, KEY_TUNE_FEDGE = 108;
 constexpr int FU_PAD = 12;       // rows of padding of the theta weight tables (the last phase of a band reads on)
 constexpr int NCLS = 6;          // profiled kernel classes: theta x1, theta x2, p, rho+force, p+theta x2, p+theta x1
-constexpr int KEY_TUNE_FBANDS = 107;
+constexpr int KEY_TUNE_FBANDS = 107, KEY_TUNE_TILE = 111;
+constexpr double TILE_MAX_POINTS = 4.5e6;  // grids up to 2048^2 take the tile kernel (sweep in profiles/README.md: it wins up to there)
 constexpr int KEY_TUNE_NW1 = 101, KEY_TUNE_NW2 = 102, KEY_TUNE_BANDS = 103, KEY_TUNE_PSEG = 104,
               KEY_TUNE_PTX = 105, KEY_TUNE_GENERIC = 106;
 
@@ -91,7 +105,11 @@ struct Ctx {
     int fx0 = 0, fxw = 0;  // source positions the column blocks of the one-pass kernel tile: [fx0, fx0 + fxw)
     bool onepass = false;
     int tune_fbands = 0;
-    int fnw() const { return FW_NTW; }
+    // small grids (state in L2): the tile kernel instead of the warp-specialised one (vlasov_tile.cuh); KEY_TUNE_TILE:
+    // 0 = by size, 1 = whenever its conditions hold, 2 = never
+    bool tile = false;
+    int tune_tile = 0;
+    int fnw() const { return tile ? 1 : FW_NTW; }  // rows of density partials per band of the one-pass kernel
     int fgran(size_t elem) const { return (int)(16 / elem); }  // lanes per column-block granule
     std::vector<int> h_srow;
 
@@ -304,10 +322,10 @@ int configure_theta_bulk() {
 // of the density partials).  Sets G.fbands[NST] = 0 when the grid does not qualify.
 template <typename T, int NST>
 int configure_fused() {
-    CU(cudaFuncSetAttribute(vl::strang_fused_ws_kernel<T, NST, FU_R, FW_NSTG, FW_NTW, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                            (int)vl::FusedWsCfg<T, NST, FU_R, FW_NSTG, FW_NTW, false>::SMEM_BYTES));
-    CU(cudaFuncSetAttribute(vl::strang_fused_ws_kernel<T, NST, FU_R, FW_NSTG, FW_NTW, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                            (int)vl::FusedWsCfg<T, NST, FU_R, FW_NSTG, FW_NTW, true>::SMEM_BYTES));
+    CU(cudaFuncSetAttribute(vl::strang_fused_ws_kernel<T, NST, FU_R<T>, FW_NSTG, FW_NTW, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                            (int)vl::FusedWsCfg<T, NST, FU_R<T>, FW_NSTG, FW_NTW, false>::SMEM_BYTES));
+    CU(cudaFuncSetAttribute(vl::strang_fused_ws_kernel<T, NST, FU_R<T>, FW_NSTG, FW_NTW, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                            (int)vl::FusedWsCfg<T, NST, FU_R<T>, FW_NSTG, FW_NTW, true>::SMEM_BYTES));
     const int np = G.np, nt = G.ntheta;
     G.fbands[NST] = 0;
     for (int j = 1; j < np; ++j)
@@ -332,11 +350,11 @@ int configure_fused() {
     // (narrower edge blocks were measured at 4096^2, 40 .. 100 %: no effect on the pass, so 100 unless tuned)
     G.fedge = (G.bc_x != vl::BC_PERIODIC && NST == 2 && G.tune_fedge > 0) ? G.tune_fedge : 100;
     const int edge_w = NST == 2 ? G.fedge : 100;
-    const int cols = vl::fused_block_cols(xw, FU_R, gran, edge_w);
+    const int cols = vl::fused_block_cols(xw, FU_R<T>, gran, edge_w);
     int wmin = nt;
     for (int c = 0; c < cols; ++c) {
         int i0, wd;
-        vl::fused_block_range(c, cols, xw, FU_R, gran, &i0, &wd, edge_w);
+        vl::fused_block_range(c, cols, xw, FU_R<T>, gran, &i0, &wd, edge_w);
         wmin = wd < wmin ? wd : wmin;
     }
     if (wmin < 1) return VLASOV_OK;
@@ -369,6 +387,42 @@ int configure_fused() {
     return VLASOV_OK;
 }
 
+// the tile kernel (vlasov_tile.cuh) for NST half shifts: fp64, periodic theta, integer shift not increasing with the row
+// and drifting by no more than the narrowest column block inside a tile's rows.  false: the grid does not qualify.
+template <int NST>
+bool configure_tile() {
+    using C = vl::TileCfg<NST>;
+    const int np = G.np, nt = G.ntheta;
+    for (int j = 1; j < np; ++j)
+        if (G.h_srow[j] > G.h_srow[j - 1]) return false;
+    const int gran = G.fgran(sizeof(double));
+    const int cols = vl::fused_block_cols(nt, C::R, gran, 100);
+    int wmin = nt;
+    for (int c = 0; c < cols; ++c) {
+        int i0, wd;
+        vl::fused_block_range(c, cols, nt, C::R, gran, &i0, &wd, 100);
+        wmin = wd < wmin ? wd : wmin;
+    }
+    if (wmin < 1) return false;
+    const int bands = cdiv(np, C::NR);
+    for (int b = 0; b < bands; ++b) {
+        const int ja = b * C::NR, jb = (b + 1) * C::NR < np ? (b + 1) * C::NR : np;
+        if (NST * (G.h_srow[ja] - G.h_srow[jb - 1]) > wmin) return false;
+    }
+    if (cudaFuncSetAttribute(vl::strang_tile_kernel<NST>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM_BYTES) !=
+        cudaSuccess) {
+        cudaGetLastError();
+        return false;
+    }
+    G.fbands[NST] = bands;
+    G.frpb[NST] = C::NR;
+    G.fcols[NST] = cols;
+    G.fx0 = 0;
+    G.fxw = nt;
+    G.fedge = 100;
+    return true;
+}
+
 template <typename T>
 int configure_all() {
     int rc;
@@ -380,7 +434,13 @@ int configure_all() {
         if ((rc = configure_theta_bulk<T, 2>()) != 0) return rc;
     }
     G.onepass = (G.fuse >= 2) && (G.halo_lo + G.halo_hi == 0);
-    if (G.onepass) {
+    G.tile = false;
+    if (G.onepass && sizeof(T) == 8 && G.bc_x == vl::BC_PERIODIC && G.tune_tile != 2 &&
+        (G.tune_tile == 1 || (double)G.ntheta * (double)G.np <= TILE_MAX_POINTS)) {
+        G.tile = true;  // (fnw() is read by the checks)
+        G.tile = configure_tile<1>() && configure_tile<2>();
+    }
+    if (G.onepass && !G.tile) {
         if ((rc = configure_fused<T, 1>()) != 0) return rc;
         if ((rc = configure_fused<T, 2>()) != 0) return rc;
         G.onepass = G.fbands[1] > 0 && G.fbands[2] > 0;
@@ -754,7 +814,7 @@ int p_pass() {
 // partials of the result in colpart_f (eqs (11), (12), (9), (10))
 template <typename T, int NST>
 int launch_fused(bool want_colsums) {
-    using CW = vl::FusedWsCfg<T, NST, FU_R, FW_NSTG, FW_NTW>;
+    using CW = vl::FusedWsCfg<T, NST, FU_R<T>, FW_NSTG, FW_NTW>;
     vl::FusedArgs<T> a;
     a.fin = static_cast<const T*>(G.f[G.cur]);
     a.fout = static_cast<T*>(G.f[G.cur ^ 1]);
@@ -774,11 +834,20 @@ int launch_fused(bool want_colsums) {
     a.dp = (G.pmax - G.pmin) / (double)G.np;
     dim3 grid(G.fcols[NST], G.fbands[NST]);
     prof_begin(NST == 2 ? 4 : 5);
+    if constexpr (sizeof(T) == 8) {
+        if (G.tile) {
+            CU(launch_pdl(vl::strang_tile_kernel<NST>, grid, dim3(vl::TileCfg<NST>::NT), vl::TileCfg<NST>::SMEM_BYTES, a));
+            prof_end(NST == 2 ? 4 : 5);
+            LAUNCH_CHECK();
+            G.cur ^= 1;
+            return VLASOV_OK;
+        }
+    }
     if (G.bc_x == vl::BC_PERIODIC)
-        CU(launch_pdl(vl::strang_fused_ws_kernel<T, NST, FU_R, FW_NSTG, FW_NTW, false>, grid, dim3(CW::NT), CW::SMEM_BYTES, a));
+        CU(launch_pdl(vl::strang_fused_ws_kernel<T, NST, FU_R<T>, FW_NSTG, FW_NTW, false>, grid, dim3(CW::NT), CW::SMEM_BYTES, a));
     else
-        CU(launch_pdl(vl::strang_fused_ws_kernel<T, NST, FU_R, FW_NSTG, FW_NTW, true>, grid, dim3(CW::NT),
-                      vl::FusedWsCfg<T, NST, FU_R, FW_NSTG, FW_NTW, true>::SMEM_BYTES, a));
+        CU(launch_pdl(vl::strang_fused_ws_kernel<T, NST, FU_R<T>, FW_NSTG, FW_NTW, true>, grid, dim3(CW::NT),
+                      vl::FusedWsCfg<T, NST, FU_R<T>, FW_NSTG, FW_NTW, true>::SMEM_BYTES, a));
     prof_end(NST == 2 ? 4 : 5);
     LAUNCH_CHECK();
     G.cur ^= 1;
@@ -1006,6 +1075,7 @@ int vlasov_set_param(int key, double value) {
             G.fuse = (int)value;
             break;
         case KEY_TUNE_FBANDS: G.tune_fbands = (int)value; break;
+        case KEY_TUNE_TILE: G.tune_tile = (int)value; break;
         case KEY_TUNE_GRAPH: G.graphs = (value != 0.0); break;
         case KEY_TUNE_PDL: G.pdl = (value != 0.0); break;
         case KEY_TUNE_FEDGE: G.tune_fedge = (int)value; break;
@@ -1337,7 +1407,8 @@ int vlasov_info(double* out, int n) {
                         G.onepass ? 1.0 : 0.0,
                         (double)G.fcols[2] * G.fbands[2],
                         (double)G.fbands[2],
-                        (double)G.frpb[2]};
+                        (double)G.frpb[2],
+                        G.tile ? 1.0 : 0.0};
     const int m = (int)(sizeof(v) / sizeof(v[0]));
     const int k = n < m ? n : m;
     for (int q = 0; q < k; ++q) out[q] = v[q];

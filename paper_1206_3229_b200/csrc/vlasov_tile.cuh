@@ -1,0 +1,158 @@
+// vlasov_tile.cuh -- the one-pass Strang step (vlasov_fused.cuh: momentum shift, NST theta half shifts, density) for
+// SMALL grids, whose state lives in L2 (cfg 1: 256^2, cfg 2: 1024^2; at small sizes the run time is
+// latency, not work).
+//
+// strang_fused_ws_kernel marches one CTA per SM down a long band through a three-deep ring: on a 256^2 or 1024^2 grid that
+// is a chain of latencies (first taps, two copy groups, three groups of twelve rows, ...) of about 19 us per pass whatever
+// the size.  Here a CTA owns a TILE of NR = 16 rows x (32 lanes x R = 7) output columns and does the pass in three short
+// phases with two block-wide barriers; a grid of several hundred such CTAs covers the grid in one or two waves:
+//   p stage      thread = source column (TC + NTAP - 1 of them).  All NR + 9 taps of the column are loaded at once (they
+//                come from L2; adjacent lanes read adjacent columns), then NR outputs of ten FMAs each (eq (11))
+//                go to shared memory.
+//   theta stage  warp = row, lane = R consecutive outputs from a window of R + NTAP - 1 values (lane stride R, odd:
+//                conflict-free), the NTAP weights of the row (W = w * w for NST = 2, eqs (12) and (9) at once) from the
+//                same tables as the big kernel; the row overwrites its source in shared memory and is stored with plain
+//                coalesced stores at column i0 + q - S (mod Ntheta), S the integer shift of the row.
+//   density      thread = output column of the tile: adds the NR rows (each at its own offset S_first - S_r) and adds the
+//                sum to colpart[band][column] (red.global.add: at most two tiles touch an entry, onto zero, so the result
+//                does not depend on the order; eq (10)).
+// The arithmetic of both shifts is the same sequence of operations as in strang_fused_ws_kernel (the results agree bit
+// for bit); only periodic theta axes and fp64 are built.
+#pragma once
+#include "vlasov_fused.cuh"
+
+namespace vl {
+
+template <int NST>
+struct TileCfg {
+    static constexpr int NR = 16;                  // rows per tile
+    static constexpr int R = 7;                    // outputs per lane
+    static constexpr int TC = 32 * R;              // output columns per tile (at most)
+    static constexpr int NTAP = NST == 2 ? 19 : 10;
+    static constexpr int NTA = TC + NTAP - 1;      // source columns
+    static constexpr int NT = 256;                 // threads
+    static constexpr int NW = NT / 32;
+    static constexpr int GP = NTA | 1;             // row pitch of the tile in shared memory
+    static constexpr int WST = NST == 2 ? 20 : WROW_STRIDE;
+    static constexpr size_t SMEM_BYTES = (size_t)NR * GP * sizeof(double) + (size_t)NR * WST * sizeof(double);
+    static_assert(NTA <= NT, "one thread per source column");
+    static_assert(NR % NW == 0, "");
+};
+
+template <int NST>
+__global__ void __launch_bounds__(TileCfg<NST>::NT) strang_tile_kernel(const FusedArgs<double> arg) {
+    using C = TileCfg<NST>;
+    constexpr int NR = C::NR, R = C::R, NTAP = C::NTAP, NTA = C::NTA, GP = C::GP, WST = C::WST;
+    extern __shared__ __align__(16) unsigned char tile_smem[];
+    double* g = reinterpret_cast<double*>(tile_smem);          // [NR][GP] rows after the momentum shift, then the outputs
+    double* wsm = g + (size_t)NR * GP;                         // [NR][WST] weight rows
+    __shared__ int delta[NR];                                  // S_first - S_r
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int ntheta = arg.ntheta, np = arg.np;
+    int i0, qmax;
+    fused_block_range((int)blockIdx.x, (int)gridDim.x, arg.xw, R, arg.gran, &i0, &qmax, 100);
+    const int jA = (int)blockIdx.y * NR;
+    const int nrows = min(NR, np - jA);
+    const unsigned pitch = (unsigned)ntheta;
+
+    ptx::pdl_launch_dependents();
+    ptx::pdl_wait();  // the force and f are read from here on
+
+    // weight rows of the tile (the tables are padded beyond Np)
+    for (int e = tid; e < nrows * WST; e += C::NT) wsm[e] = arg.wtab[(size_t)jA * WST + e];
+
+    // ---- p stage ----
+    if (tid < NTA) {
+        const int c = wrap_index(i0 - 4 * NST + tid, ntheta);
+        double sf, a;
+        split_shift(-(arg.force[c] * arg.dt) / arg.dp, &sf, &a);
+        const bool p_periodic = (arg.bc_p == BC_PERIODIC);
+        int s;
+        if (p_periodic) {
+            sf = fmod(sf, (double)np);
+            s = (int)sf;
+            if (s < 0) s += np;
+        } else {
+            const double lim = (double)np + 64.0;
+            s = (int)fmin(fmax(sf, -lim), lim);
+        }
+        double w[10];
+        spline_fd8_weights(a, w);
+        const double* col = arg.fin + c;
+        int rn = jA + s - 4;
+        if (p_periodic) rn = wrap_index(rn, np);
+        double v[NR + 9];
+#pragma unroll
+        for (int m = 0; m < NR + 9; ++m) {
+            const bool ok = p_periodic || (unsigned)rn < (unsigned)np;
+            v[m] = ok ? __ldg(col + (size_t)rn * pitch) : 0.0;
+            ++rn;
+            if (p_periodic && rn >= np) rn = 0;
+        }
+#pragma unroll
+        for (int r = 0; r < NR; ++r) {
+            double acc = w[0] * v[r];
+#pragma unroll
+            for (int m = 1; m < 10; ++m) acc = fma(w[m], v[r + m], acc);
+            g[r * GP + tid] = acc;
+        }
+    }
+    __syncthreads();
+
+    // ---- theta stage ----
+    const int S0 = (int)wsm[NTAP];  // shift of the first row (the largest: S does not increase with the row)
+    for (int r = warp; r < nrows; r += C::NW) {
+        const double* Wr = wsm + r * WST;
+        double* grow = g + r * GP;
+        double x[R + NTAP - 1];
+#pragma unroll
+        for (int k = 0; k < R + NTAP - 1; ++k) x[k] = grow[lane * R + k];
+        double out[R];
+        {
+            const double W0 = Wr[0];
+#pragma unroll
+            for (int q = 0; q < R; ++q) out[q] = W0 * x[q];
+        }
+#pragma unroll
+        for (int n = 1; n < NTAP; ++n) {
+            const double Wn = Wr[n];
+#pragma unroll
+            for (int q = 0; q < R; ++q) out[q] = fma(Wn, x[q + n], out[q]);
+        }
+        const int S = (int)Wr[NTAP];
+        __syncwarp();  // every lane has its window
+#pragma unroll
+        for (int q = 0; q < R; ++q) grow[lane * R + q] = out[q];
+        if (lane == 0) delta[r] = S0 - S;
+        __syncwarp();
+        const int base = wrap_index(i0 - S, ntheta);
+        double* orow = arg.fout + (size_t)(jA + r) * pitch;
+#pragma unroll
+        for (int k = 0; k < R; ++k) {
+            const int q = lane + 32 * k;
+            if (q < qmax) {
+                int i = base + q;
+                if (i >= ntheta) i -= ntheta;
+                orow[i] = grow[q];
+            }
+        }
+    }
+    if (arg.colpart == nullptr) return;
+    __syncthreads();
+
+    // ---- density partials of the tile: output column u (relative to i0 - S0) sums row r at q = u - delta[r] ----
+    const int dmax = delta[nrows - 1];
+    double* cp = arg.colpart + (size_t)blockIdx.y * (size_t)ntheta;
+    const int cb = wrap_index(i0 - S0, ntheta);
+    for (int u = tid; u < qmax + dmax; u += C::NT) {
+        double acc = 0.0;
+        for (int r = 0; r < nrows; ++r) {
+            const int q = u - delta[r];
+            if (q >= 0 && q < qmax) acc += g[r * GP + q];
+        }
+        ptx::red_add_f64(cp + wrap_index(cb + u, ntheta), acc);
+    }
+}
+
+}  // namespace vl

@@ -121,14 +121,16 @@ ONEPASS_GRIDS = [(64, 48), (352, 30), (353, 61), (1000, 137), (2233, 25), (31, 9
 @pytest.mark.parametrize("bc_p", [BC_ZERO, BC_PERIODIC])
 @pytest.mark.parametrize("which,dt,amp", [(1, 0.1, 0.5), (2, 0.1, 0.5), (2, -0.37, 30.0), (1, 9.0, 2000.0),
                                           (2, 9.0, 30.0), (2, 3.0, 0.0)])
-def test_one_pass_p_then_theta(grid, bc_p, which, dt, amp):
+@pytest.mark.parametrize("tile", [1, 2])
+def test_one_pass_p_then_theta(grid, bc_p, which, dt, amp, tile):
     """p shift with a given force, then one or two half theta shifts, then density and force of the result:
-    the one-pass kernel against the oracle's separate sweeps (eqs (11), (12), (9), (10))."""
+    the one-pass kernel against the oracle's separate sweeps (eqs (11), (12), (9), (10)).  tile = 1: the tile kernel of
+    small grids (strang_tile_kernel), tile = 2: the warp-specialised kernel of the large ones on the same small grid."""
     dom = (-PI, PI, -4.0, 4.0)
     f0 = smooth_state(grid[0], grid[1], dom, seed=5)
     th = inputs.nodes(dom[0], dom[1], grid[0])
     F = amp * np.sin(2 * th + 0.1) + 0.3 * amp
-    o, g = pair(MODEL_HMF, grid, dom, dt, f0, bc_p=bc_p)
+    o, g = pair(MODEL_HMF, grid, dom, dt, f0, bc_p=bc_p, gpu_params=dict(tune_tile=tile))
     o.p_sweep(dt, force=F)
     for _ in range(which):
         o.theta_sweep(0.5 * dt)
@@ -138,6 +140,12 @@ def test_one_pass_p_then_theta(grid, bc_p, which, dt, amp):
     # takes the separate kernels, unless one axis has a single node (then all row shifts are equal)
     expect_onepass = int(0.0 < dt <= 3.0 or min(grid) == 1)
     assert g.info()["onepass"] == expect_onepass
+    # ... and which of the two one-pass kernels: the tile kernel wherever the one-pass path applies and the row shift
+    # drifts by less than a column block inside 16 rows
+    if dt != 3.0:  # (at dt = 3 the row shift drifts by more than a column block inside 16 rows on some of the grids)
+        assert g.info()["onepass_tile"] == int(tile == 1 and expect_onepass == 1)
+    else:
+        assert g.info()["onepass_tile"] <= int(tile == 1)
     g.substep(vb.SUB_P_THETA_TWICE if which == 2 else vb.SUB_P_THETA_HALF)
     fo = o.download()
     assert rel_err(g.download(), fo) < 1e-13
@@ -182,7 +190,7 @@ def test_one_pass_band_split_does_not_change_the_result(fbands):
     f0 = smooth_state(grid[0], grid[1], dom, seed=6)
     th = inputs.nodes(dom[0], dom[1], grid[0])
     F = 3.0 * np.sin(th + 0.2)
-    o, g = pair(MODEL_HMF, grid, dom, 0.7, f0, gpu_params=dict(tune_fbands=fbands))
+    o, g = pair(MODEL_HMF, grid, dom, 0.7, f0, gpu_params=dict(tune_fbands=fbands, tune_tile=2))
     o.p_sweep(0.7, force=F)
     o.theta_sweep(0.35)
     o.theta_sweep(0.35)
@@ -216,6 +224,47 @@ def test_100_steps_match_oracle(name, kw, fuse):
     assert np.max(np.abs(mg - mo)) <= TOL * max(1.0, np.max(np.abs(mo)))
     assert mg[0] == pytest.approx(100 * c["dt"])
     g.close()
+
+
+@pytest.mark.parametrize("name,kw", [c for c in CASES if c[0] != "cfg4"])
+def test_100_steps_match_oracle_large_grid_kernel_on_small_grids(name, kw):
+    """The default one-pass path of these grids is the tile kernel (test above, fuse = 2); the warp-specialised kernel that
+    the large grids take is held to the same bar on them (TUNE_TILE = 2).  (cfg 4 has a zero-extended x axis: always the
+    warp-specialised kernel.)"""
+    c = inputs.config(name, **kw)
+    o, g = pair(c["model"], c["grid"], c["domain"], c["dt"], c["f0"], gpu_params=dict(fuse=2, tune_tile=2), **c["params"])
+    assert g.info()["onepass"] == 1 and g.info()["onepass_tile"] == 0
+    o.step(100)
+    g.step(100)
+    assert rel_err(g.download(), o.download()) <= TOL
+    mo, mg = o.moments(), g.moments()
+    assert np.max(np.abs(mg - mo)) <= TOL * max(1.0, np.max(np.abs(mo)))
+    g.close()
+
+
+@pytest.mark.parametrize("grid", [(256, 256), (1000, 137), (353, 61), (2048, 96)])
+@pytest.mark.parametrize("bc_p", [BC_ZERO, BC_PERIODIC])
+@pytest.mark.parametrize("which", [1, 2])
+def test_tile_kernel_and_large_grid_kernel_agree_bit_for_bit(grid, bc_p, which):
+    """Both one-pass kernels apply the same sequence of floating-point operations to every grid point (ten FMAs of the
+    momentum shift, 10 or 19 of the theta weights): with the same force, f after the pass is the same bits; the density
+    differs only in the order of its column sums."""
+    dom = (-PI, PI, -4.0, 4.0)
+    f0 = smooth_state(grid[0], grid[1], dom, seed=11)
+    th = inputs.nodes(dom[0], dom[1], grid[0])
+    F = 0.8 * np.sin(th + 0.3) + 0.1
+    outs, rhos = [], []
+    for tile in (1, 2):
+        g = vb.Vlasov(MODEL_HMF, grid, dom, 0.1, bc_p=bc_p, tune_tile=tile)
+        g.upload(f0)
+        assert g.info()["onepass"] == 1 and g.info()["onepass_tile"] == (1 if tile == 1 else 0)
+        g.set_force(F)
+        g.substep(vb.SUB_P_THETA_TWICE if which == 2 else vb.SUB_P_THETA_HALF)
+        outs.append(g.download())
+        rhos.append(g.density())
+        g.close()
+    assert np.array_equal(outs[0], outs[1])
+    assert np.max(np.abs(rhos[0] - rhos[1])) <= 1e-13 * np.max(np.abs(rhos[1]))
 
 
 def test_history_records_every_step_and_matches_oracle():
@@ -253,12 +302,13 @@ def test_fused_multi_step_equals_single_steps(fuse):
         assert rel_err(a, b) < 1e-13
 
 
-def test_one_pass_is_reproducible_run_to_run():
+@pytest.mark.parametrize("tile", [1, 2])
+def test_one_pass_is_reproducible_run_to_run(tile):
     """The density partials are accumulated with atomic adds of at most two terms per entry: same bits every run."""
     c = inputs.config("cfg5", ntheta=1500, npts=900)
     outs = []
     for _ in range(3):
-        g = vb.Vlasov(c["model"], c["grid"], c["domain"], c["dt"])
+        g = vb.Vlasov(c["model"], c["grid"], c["domain"], c["dt"], tune_tile=tile)
         g.upload(c["f0"])
         g.step(7)
         outs.append(g.download())

@@ -108,7 +108,7 @@ struct Ctx {
     // small grids (state in L2): the tile kernel instead of the warp-specialised one (vlasov_tile.cuh); KEY_TUNE_TILE:
     // 0 = by size, 1 = whenever its conditions hold, 2 = never
     bool tile = false;
-    int tune_tile = 0;
+    int tune_tile = 0, tile_nr = 16;
     int fnw() const { return tile ? 1 : FW_NTW; }  // rows of density partials per band of the one-pass kernel
     int fgran(size_t elem) const { return (int)(16 / elem); }  // lanes per column-block granule
     std::vector<int> h_srow;
@@ -389,9 +389,9 @@ int configure_fused() {
 
 // the tile kernel (vlasov_tile.cuh) for NST half shifts: fp64, periodic theta, integer shift not increasing with the row
 // and drifting by no more than the narrowest column block inside a tile's rows.  false: the grid does not qualify.
-template <int NST>
+template <int NST, int NR>
 bool configure_tile() {
-    using C = vl::TileCfg<NST>;
+    using C = vl::TileCfg<NST, NR>;
     const int np = G.np, nt = G.ntheta;
     for (int j = 1; j < np; ++j)
         if (G.h_srow[j] > G.h_srow[j - 1]) return false;
@@ -409,7 +409,7 @@ bool configure_tile() {
         const int ja = b * C::NR, jb = (b + 1) * C::NR < np ? (b + 1) * C::NR : np;
         if (NST * (G.h_srow[ja] - G.h_srow[jb - 1]) > wmin) return false;
     }
-    if (cudaFuncSetAttribute(vl::strang_tile_kernel<NST>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM_BYTES) !=
+    if (cudaFuncSetAttribute(vl::strang_tile_kernel<NST, NR>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM_BYTES) !=
         cudaSuccess) {
         cudaGetLastError();
         return false;
@@ -437,8 +437,9 @@ int configure_all() {
     G.tile = false;
     if (G.onepass && sizeof(T) == 8 && G.bc_x == vl::BC_PERIODIC && G.tune_tile != 2 &&
         (G.tune_tile == 1 || (double)G.ntheta * (double)G.np <= TILE_MAX_POINTS)) {
-        G.tile = true;  // (fnw() is read by the checks)
-        G.tile = configure_tile<1>() && configure_tile<2>();
+        G.tile = true;
+        G.tile_nr = (double)G.ntheta * (double)G.np <= 131072.0 ? 8 : 16;  // more, smaller tiles on the smallest grids
+        G.tile = G.tile_nr == 8 ? (configure_tile<1, 8>() && configure_tile<2, 8>()) : (configure_tile<1, 16>() && configure_tile<2, 16>());
     }
     if (G.onepass && !G.tile) {
         if ((rc = configure_fused<T, 1>()) != 0) return rc;
@@ -836,7 +837,10 @@ int launch_fused(bool want_colsums) {
     prof_begin(NST == 2 ? 4 : 5);
     if constexpr (sizeof(T) == 8) {
         if (G.tile) {
-            CU(launch_pdl(vl::strang_tile_kernel<NST>, grid, dim3(vl::TileCfg<NST>::NT), vl::TileCfg<NST>::SMEM_BYTES, a));
+            if (G.tile_nr == 8)
+                CU(launch_pdl(vl::strang_tile_kernel<NST, 8>, grid, dim3(vl::TileCfg<NST, 8>::NT), vl::TileCfg<NST, 8>::SMEM_BYTES, a));
+            else
+                CU(launch_pdl(vl::strang_tile_kernel<NST, 16>, grid, dim3(vl::TileCfg<NST, 16>::NT), vl::TileCfg<NST, 16>::SMEM_BYTES, a));
             prof_end(NST == 2 ? 4 : 5);
             LAUNCH_CHECK();
             G.cur ^= 1;

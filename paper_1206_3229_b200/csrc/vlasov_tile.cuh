@@ -4,7 +4,7 @@
 //
 // strang_fused_ws_kernel marches one CTA per SM down a long band through a three-deep ring: on a 256^2 or 1024^2 grid that
 // is a chain of latencies (first taps, two copy groups, three groups of twelve rows, ...) of about 19 us per pass whatever
-// the size.  Here a CTA owns a TILE of NR = 16 rows x (32 lanes x R = 7) output columns and does the pass in three short
+// the size.  Here a CTA owns a TILE of NR = 16 (or 8) rows x (32 lanes x R = 7) output columns and does the pass in three short
 // phases with two block-wide barriers; a grid of several hundred such CTAs covers the grid in one or two waves:
 //   p stage      thread = source column (TC + NTAP - 1 of them).  All NR + 9 taps of the column are loaded at once (they
 //                come from L2; adjacent lanes read adjacent columns), then NR outputs of ten FMAs each (eq (11))
@@ -23,9 +23,11 @@
 
 namespace vl {
 
-template <int NST>
+template <int NST, int NR_>
 struct TileCfg {
-    static constexpr int NR = 16;                  // rows per tile
+    static constexpr int NR = NR_;                 // rows per tile: 16, or 8 on the smallest grids (more CTAs: cfg 1 10.3 -> 9.3 us
+                                                   // per step; sweep of 8 / 16 / 24 / 32 in profiles/README.md)
+    static constexpr int MINB = 3;                 // CTAs per SM the register budget is set for (<= 85 registers)
     static constexpr int R = 7;                    // outputs per lane
     static constexpr int TC = 32 * R;              // output columns per tile (at most)
     static constexpr int NTAP = NST == 2 ? 19 : 10;
@@ -39,9 +41,9 @@ struct TileCfg {
     static_assert(NR % NW == 0, "");
 };
 
-template <int NST>
-__global__ void __launch_bounds__(TileCfg<NST>::NT) strang_tile_kernel(const FusedArgs<double> arg) {
-    using C = TileCfg<NST>;
+template <int NST, int NR_>
+__global__ void __launch_bounds__(TileCfg<NST, NR_>::NT, TileCfg<NST, NR_>::MINB) strang_tile_kernel(const FusedArgs<double> arg) {
+    using C = TileCfg<NST, NR_>;
     constexpr int NR = C::NR, R = C::R, NTAP = C::NTAP, NTA = C::NTA, GP = C::GP, WST = C::WST;
     extern __shared__ __align__(16) unsigned char tile_smem[];
     double* g = reinterpret_cast<double*>(tile_smem);          // [NR][GP] rows after the momentum shift, then the outputs

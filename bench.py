@@ -356,7 +356,10 @@ def run_cuda(args):
         gs = args.spline == "gs"
         traffic, traffic_src = committed_traffic(("gsrec_" if gs else "") + dom, nt, prec) if nt == npp else (None, None)
         step_frac = (step_bytes * pts * K / (ms * 1e-3) / 1e9) / peak
-        roofline = {"bound": "hbm", "kernel": (GS_KERNEL_NAMES if gs else KERNEL_NAMES).get(dom, dom),
+        kname = (GS_KERNEL_NAMES if gs else KERNEL_NAMES).get(dom, dom)
+        if g.info().get("onepass_tile") and dom in ("ptheta2", "ptheta1"):  # small grids: the tile kernel ran
+            kname = kname.replace("strang_fused_ws_kernel", "strang_tile_kernel")
+        roofline = {"bound": "hbm", "kernel": kname,
                     "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
                     "traffic": traffic, "traffic_source": traffic_src,
                     "peak_source": peak_src, "algorithmic_bytes_per_launch": 2 * eb * pts,

@@ -59,10 +59,10 @@ __global__ void __launch_bounds__(TileCfg<NST, NR_>::NT, TileCfg<NST, NR_>::MINB
     const unsigned pitch = (unsigned)ntheta;
 
     ptx::pdl_launch_dependents();
+    // weight rows of the tile: constants of the run, fetched while the density / force kernel this pass was launched behind
+    // still runs (programmatic dependent launch)
+    for (int e = tid; e < nrows * WST; e += C::NT) wsm[e] = __ldg(arg.wtab + (size_t)jA * WST + e);
     ptx::pdl_wait();  // the force and f are read from here on
-
-    // weight rows of the tile (the tables are padded beyond Np)
-    for (int e = tid; e < nrows * WST; e += C::NT) wsm[e] = arg.wtab[(size_t)jA * WST + e];
 
     // ---- p stage ----
     if (tid < NTA) {

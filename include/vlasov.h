@@ -206,7 +206,8 @@ int vlasov_kernel_times(double out[12]);
 /* Fill out[0..n) (host) with implementation facts for reports: {SM count, theta-kernel CTAs, p-kernel CTAs,
  * bands, warps per theta CTA (2-shift), warps per theta CTA (1-shift), theta1 CTAs, p segment length, p threads,
  * bulk-copy theta kernel in use, one-pass kernel in use (0/1), its CTAs, bands, rows per band, whether it is the tile
- * kernel of small grids (0/1)}; returns how many were written. */
+ * kernel of small grids (0/1), the largest thread-block cluster the density / force kernel of short theta axes may use (8 or
+ * 16)}; returns how many were written. */
 int vlasov_info(double* out, int n);
 
 void vlasov_free(void);

@@ -240,7 +240,7 @@ def vlasov_info() -> dict:
     n = _chk(load().vlasov_info(buf.ctypes.data_as(_dp), 16), "vlasov_info")
     names = ["sm_count", "theta2_ctas", "p_ctas", "theta2_bands", "theta2_warps", "theta1_warps", "theta1_ctas",
              "p_seg_len", "p_threads", "theta_bulk", "onepass", "onepass_ctas", "onepass_bands", "onepass_rows_per_band",
-             "onepass_tile"]
+             "onepass_tile", "max_cluster"]
     return {k: int(buf[i]) for i, k in enumerate(names[:n])}
 
 

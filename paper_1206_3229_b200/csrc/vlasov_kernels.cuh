@@ -12,6 +12,7 @@
 // are not needed): the theta shift runs along the contiguous axis through shared memory, the p shift lets
 // adjacent threads own adjacent columns and march down p with a register window.
 #pragma once
+#include <cooperative_groups.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
 
@@ -619,6 +620,93 @@ __global__ void __launch_bounds__(RR_COLS* RR_GROUPS)
     my = mp[32].y;
 #pragma unroll 8
     for (int k = tid; k < ntheta; k += RR_COLS * RR_GROUPS) force[k] = -sin_t[k] * mx + cos_t[k] * my;
+}
+
+// Short theta axes (Ntheta <= 1024: cfg 1, cfg 2), HMF model: density, Fourier moments and force by ONE THREAD-BLOCK CLUSTER
+// of up to eight CTAs, each with 128 columns.  rho_force_kernel above is a chain of six dependent round trips through L2
+// (partials, rho + fence, ticket, moment partials, tables, force) whatever the size: 5 us on a 256-column grid whose
+// whole pass takes 4.5 us.  Here thread (column c, group g) adds the partials of bands g, g + 8, ... of its column (all
+// loads in flight at once), the eight groups are added in order, the CTA adds its moments over a fixed tree, the CTAs
+// read one another's moment partials through distributed shared memory in rank order (one cluster barrier instead of a
+// ticket in global memory) and every CTA writes the force of its own columns.  eqs (10), (7)-(8) (L75-L78, L56-L63).
+constexpr int RC_COLS = 128, RC_GROUPS = 8;
+__global__ void __launch_bounds__(RC_COLS* RC_GROUPS)
+    rho_force_cluster_kernel(double* __restrict__ colpart, int nbands, int ntheta, double dp, double* __restrict__ rho,
+                             const double* __restrict__ cos_t, const double* __restrict__ sin_t, int zero_after,
+                             double dtheta, double* __restrict__ force) {
+    namespace cg = cooperative_groups;
+    cg::cluster_group cluster = cg::this_cluster();
+    __shared__ double part[RC_GROUPS][RC_COLS];
+    __shared__ double2 red[RC_COLS / 32];
+    __shared__ double2 mine;  // this CTA's (sum cos theta_i rho_i, sum sin theta_i rho_i)
+    ptx::pdl_launch_dependents();
+    const int tid = threadIdx.x, c = tid & (RC_COLS - 1), g = tid / RC_COLS, lane = tid & 31, warp = tid >> 5;
+    const int i = blockIdx.x * RC_COLS + c;
+    const bool in = i < ntheta;
+    const bool own = in && g == 0;
+    const double ct = own ? cos_t[i] : 0.0, st = own ? sin_t[i] : 0.0;  // constants of the run: fetched before the wait
+    ptx::pdl_wait();                                                    // the pass whose column sums are read has completed
+    double acc = 0.0;
+    if (in) {
+        constexpr int NB = 4;
+        for (int b0 = g; b0 < nbands; b0 += NB * RC_GROUPS) {
+            double v[NB];
+#pragma unroll
+            for (int k = 0; k < NB; ++k) {
+                const int b = b0 + k * RC_GROUPS;
+                v[k] = (b < nbands) ? __ldcg(colpart + (size_t)b * ntheta + i) : 0.0;
+            }
+            if (zero_after) {
+#pragma unroll
+                for (int k = 0; k < NB; ++k) {
+                    const int b = b0 + k * RC_GROUPS;
+                    if (b < nbands) __stcg(colpart + (size_t)b * ntheta + i, 0.0);
+                }
+            }
+#pragma unroll
+            for (int k = 0; k < NB; ++k) acc += v[k];
+        }
+    }
+    part[g][c] = acc;
+    __syncthreads();
+    double r = 0.0;
+    if (g == 0) {
+#pragma unroll
+        for (int q = 0; q < RC_GROUPS; ++q) r += part[q][c];
+        r *= dp;
+        if (in) rho[i] = r;
+    }
+    if (warp < RC_COLS / 32) {  // the warps of group 0
+        double cs = ct * r, ss = st * r;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            cs += __shfl_down_sync(0xffffffffu, cs, o);
+            ss += __shfl_down_sync(0xffffffffu, ss, o);
+        }
+        if (lane == 0) red[warp] = make_double2(cs, ss);
+    }
+    __syncthreads();
+    if (tid == 0) {
+        double2 t = red[0];
+#pragma unroll
+        for (int w = 1; w < RC_COLS / 32; ++w) {
+            t.x += red[w].x;
+            t.y += red[w].y;
+        }
+        mine = t;
+    }
+    cluster.sync();  // every CTA's partial is written
+    if (own) {
+        double mx = 0.0, my = 0.0;
+        const unsigned nb = cluster.num_blocks();
+        for (unsigned rk = 0; rk < nb; ++rk) {
+            const double2 t = *cluster.map_shared_rank(&mine, rk);
+            mx += t.x;
+            my += t.y;
+        }
+        force[i] = -st * (mx * dtheta) + ct * (my * dtheta);
+    }
+    cluster.sync();  // no CTA leaves while its shared memory may still be read
 }
 
 // HMF force from a density vector (eqs (7)-(8), L56-L63), one CTA: M = dtheta sum_i (cos, sin)(theta_i) rho_i over a fixed

@@ -294,6 +294,8 @@ def run_cuda(args):
         params["tune_fedge"] = args.fedge
     if args.tile > 0:
         params["tune_tile"] = args.tile
+    if args.rc > 0:
+        params["tune_rc"] = args.rc
     g = vb.Vlasov(c["model"], c["grid"], c["domain"], c["dt"], precision=prec, device="cuda:%d" % local_rank, **params)
     g.upload(f0)
     pts = float(nt) * float(npp)
@@ -686,6 +688,8 @@ def main():
     ap.add_argument("--fbands", type=int, default=0, help="bands of rows of the one-pass kernel (0 = automatic)")
     ap.add_argument("--tile", type=int, default=0, choices=[0, 1, 2],
                     help="one-pass step of small grids by the tile kernel: 0 by size (default), 1 wherever it applies, 2 never")
+    ap.add_argument("--rc", type=int, default=0, choices=[0, 2],
+                    help="HMF density / force of short theta axes by one thread-block cluster: 0 (default), 2 never (the ticketed kernel)")
     ap.add_argument("--fedge", type=int, default=0, help="zero-extended x: width (percent) of the two edge column blocks (0 = automatic)")
     ap.add_argument("--graph", type=int, default=1, choices=[0, 1],
                     help="1 (default): steady-state step pairs are launched as CUDA graphs, 0: plain launches")

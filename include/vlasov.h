@@ -88,7 +88,9 @@ extern "C" {
  *   110 TUNE_PDL                 0: ordinary launches instead of programmatic dependent launch (default 1)
  *   111 TUNE_TILE                one-pass step of small grids (fp64, periodic theta) by the tile kernel strang_tile_kernel instead of
  *                                the warp-specialised one: 0 by size (default: up to 4.5e6 grid points, i.e. 2048^2), 1 whenever its conditions
- *                                hold, 2 never                                                                         */
+ *                                hold, 2 never
+ *   112 TUNE_RC                  2: never rho_force_cluster_kernel (HMF density / moments / force of theta axes of up to 1024
+ *                                columns by one thread-block cluster); the ticketed rho_force_kernel on every grid instead   */
 
 /* sub-steps for vlasov_substep (parity tests of single stages; same kernels as vlasov_step) */
 #define VLASOV_SUB_THETA_HALF 0  /* eq (9)/(12): f(x - p dt/2, p), also leaves the column sums for the force */

@@ -46,7 +46,7 @@ constexpr int FW_NTW = VL_FW_NTW_;       // its theta warps = density partial ro
 constexpr int KEY_TUNE_GRAPH = 109, KEY_TUNE_PDL = 110, KEY_TUNE_FEDGE = 108;
 constexpr int FU_PAD = 12;       // rows of padding of the theta weight tables (the last phase of a band reads on)
 constexpr int NCLS = 6;          // profiled kernel classes: theta x1, theta x2, p, rho+force, p+theta x2, p+theta x1
-constexpr int KEY_TUNE_FBANDS = 107, KEY_TUNE_TILE = 111;
+constexpr int KEY_TUNE_FBANDS = 107, KEY_TUNE_TILE = 111, KEY_TUNE_RC = 112;
 constexpr double TILE_MAX_POINTS = 4.5e6;  // grids up to 2048^2 take the tile kernel (sweep in profiles/README.md: it wins up to there)
 constexpr int KEY_TUNE_NW1 = 101, KEY_TUNE_NW2 = 102, KEY_TUNE_BANDS = 103, KEY_TUNE_PSEG = 104,
               KEY_TUNE_PTX = 105, KEY_TUNE_GENERIC = 106;
@@ -108,6 +108,7 @@ struct Ctx {
     // small grids (state in L2): the tile kernel instead of the warp-specialised one (vlasov_tile.cuh); KEY_TUNE_TILE:
     // 0 = by size, 1 = whenever its conditions hold, 2 = never
     int rc_max_cluster = 8;  // largest cluster rho_force_cluster_kernel may be launched with (16 where the GPU can place it)
+    int tune_rc = 0;         // KEY_TUNE_RC: 2 = never the cluster kernel (the ticketed rho_force_kernel on every grid)
     bool tile = false;
     int tune_tile = 0, tile_nr = 16;
     int fnw() const { return tile ? 1 : FW_NTW; }  // rows of density partials per band of the one-pass kernel
@@ -891,9 +892,12 @@ int rho_from_colpart(int bands, double* rho_out, bool hmf_partials, double* colp
     const double dp = (G.pmax - G.pmin) / (double)G.np;
     const double dx = (G.xmax - G.xmin) / (double)G.ntheta;
     const bool sheet = fuse_force && G.model == VLASOV_MODEL_SHEET;
-    if (fuse_force && hmf_partials && G.ntheta <= vl::RC_COLS * G.rc_max_cluster && G.halo_lo + G.halo_hi == 0) {
-        // short theta axis (cfg 1, cfg 2; up to 2048 columns where the GPU takes clusters of 16), HMF: density, moments and
-        // force by one thread-block cluster instead of the ticketed kernel (cfg 1: 9.3 -> 7.5 us per step, cfg 2: 15.4 -> 14.4)
+    // (theta axes of up to 1024 columns: from 2048 on the ticketed kernel is faster -- 33.8 against 36.1 us per step at 2048^2,
+    // 259.3 against 264.6 at 8192^2 with four chunks of columns per CTA, profiles/README.md)
+    if (fuse_force && hmf_partials && G.tune_rc != 2 && G.ntheta <= 1024 && G.ntheta <= vl::RC_COLS * G.rc_max_cluster &&
+        G.halo_lo + G.halo_hi == 0) {
+        // short theta axis (cfg 1, cfg 2), HMF: density, moments and force by one thread-block cluster instead of the ticketed
+        // kernel (cfg 1: 9.3 -> 7.5 us per step, cfg 2: 15.4 -> 14.4)
         cudaLaunchConfig_t cfg = {};
         const unsigned ncta = (unsigned)cdiv(G.ntheta, vl::RC_COLS);
         cfg.gridDim = dim3(ncta);
@@ -1122,6 +1126,7 @@ int vlasov_set_param(int key, double value) {
             break;
         case KEY_TUNE_FBANDS: G.tune_fbands = (int)value; break;
         case KEY_TUNE_TILE: G.tune_tile = (int)value; break;
+        case KEY_TUNE_RC: G.tune_rc = (int)value; break;
         case KEY_TUNE_GRAPH: G.graphs = (value != 0.0); break;
         case KEY_TUNE_PDL: G.pdl = (value != 0.0); break;
         case KEY_TUNE_FEDGE: G.tune_fedge = (int)value; break;

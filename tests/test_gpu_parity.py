@@ -88,10 +88,13 @@ def test_p_sweep_with_given_force(grid, bc_p, amp):
 
 @pytest.mark.parametrize("model,dom", [(MODEL_HMF, (-PI, PI, -4.0, 4.0)), (MODEL_RING, (-PI, PI, -3.0, 3.0)),
                                        (MODEL_SHEET, (-10.0, 10.0, -4.0, 4.0)), (MODEL_FREE, (-PI, PI, -4.0, 4.0))])
-@pytest.mark.parametrize("grid", [(64, 48), (300, 129), (1500, 40), (2048, 64)])
-def test_density_force_and_moments(model, dom, grid):
+@pytest.mark.parametrize("grid", [(64, 48), (300, 129), (1024, 70), (1500, 40), (2048, 64)])
+@pytest.mark.parametrize("rc", [0, 2])
+def test_density_force_and_moments(model, dom, grid, rc):
+    """rc = 0: HMF on theta axes of up to 1024 columns takes the thread-block-cluster kernel (rho_force_cluster_kernel),
+    rc = 2 (TUNE_RC): the ticketed rho_force_kernel that every other grid and model takes."""
     f0 = smooth_state(grid[0], grid[1], dom, seed=4)
-    o, g = pair(model, grid, dom, 0.05, f0)
+    o, g = pair(model, grid, dom, 0.05, f0, gpu_params=dict(tune_rc=rc))
     g.substep(vb.SUB_FORCE)
     rho_o, F_o = o.density(), o.force()
     assert np.max(np.abs(g.density() - rho_o)) <= 1e-13 * np.max(np.abs(rho_o))
@@ -228,11 +231,16 @@ def test_100_steps_match_oracle(name, kw, fuse):
 
 @pytest.mark.parametrize("name,kw", [c for c in CASES if c[0] != "cfg4"])
 def test_100_steps_match_oracle_large_grid_kernel_on_small_grids(name, kw):
+    _run_100_steps_large_grid_kernels(name, kw)
+
+
+def _run_100_steps_large_grid_kernels(name, kw):
     """The default one-pass path of these grids is the tile kernel (test above, fuse = 2); the warp-specialised kernel that
-    the large grids take is held to the same bar on them (TUNE_TILE = 2).  (cfg 4 has a zero-extended x axis: always the
-    warp-specialised kernel.)"""
+    the large grids take is held to the same bar on them (TUNE_TILE = 2), and so is their density / force kernel (TUNE_RC = 2:
+    the ticketed kernel instead of the thread-block cluster).  (cfg 4 has a zero-extended x axis: always the warp-specialised
+    kernel.)"""
     c = inputs.config(name, **kw)
-    o, g = pair(c["model"], c["grid"], c["domain"], c["dt"], c["f0"], gpu_params=dict(fuse=2, tune_tile=2), **c["params"])
+    o, g = pair(c["model"], c["grid"], c["domain"], c["dt"], c["f0"], gpu_params=dict(fuse=2, tune_tile=2, tune_rc=2), **c["params"])
     assert g.info()["onepass"] == 1 and g.info()["onepass_tile"] == 0
     o.step(100)
     g.step(100)

@@ -22,7 +22,7 @@ def rel_err(a, b):
 
 @pytest.mark.parametrize("name,kw,params", [
     ("cfg1", dict(ntheta=353, npts=61), dict()),                       # one-pass step by the tile kernel (small grids)
-    ("cfg1", dict(ntheta=353, npts=61), dict(tune_tile=2)),            # warp-specialised one-pass kernel, ragged row (plain stores)
+    ("cfg1", dict(ntheta=353, npts=61), dict(tune_tile=2, tune_rc=2)), # warp-specialised one-pass kernel, ragged row (plain stores); ticketed density / force kernel
     ("cfg1", dict(ntheta=352, npts=60), dict(tune_tile=2)),            # warp-specialised one-pass kernel, bulk stores
     ("cfg1", dict(ntheta=352, npts=60), dict(precision=32)),           # fp32: difference form
     ("cfg1", dict(ntheta=128, npts=48), dict(fuse=1)),                 # theta x2 bulk kernel + p kernel
@@ -70,7 +70,7 @@ def test_small_md_matches_oracle():
 
 @pytest.mark.parametrize("name,kw,params", [
     ("cfg1", dict(ntheta=353, npts=61), dict()), ("cfg1", dict(ntheta=352, npts=60), dict(precision=32)),
-    ("cfg1", dict(ntheta=353, npts=61), dict(tune_tile=2)), ("cfg5", dict(ntheta=1100, npts=640), dict(tune_tile=2)),
+    ("cfg1", dict(ntheta=353, npts=61), dict(tune_tile=2, tune_rc=2)), ("cfg5", dict(ntheta=1100, npts=640), dict(tune_tile=2)),
     ("cfg5", dict(ntheta=1100, npts=640), dict()), ("cfg3", dict(ntheta=256, npts=48), dict(fuse=1)),
     ("cfg4", dict(ntheta=256, npts=64), dict()), ("cfg1", dict(ntheta=96, npts=64), dict(spline=1)),
     ("cfg1", dict(ntheta=131, npts=40), dict(fuse=0, order=4)), ("cfg1", dict(ntheta=128, npts=48), dict(halo_lo=7, halo_hi=9, fuse=0)),
@@ -86,7 +86,7 @@ def test_no_byte_is_written_outside_the_attached_buffers(name, kw, params):
     prec = params.get("precision", 64)
     vb.vlasov_init(c["model"], c["grid"], c["domain"], c["dt"])
     keys = {"precision": vb.KEY_PRECISION, "fuse": vb.KEY_FUSE, "spline": vb.KEY_SPLINE, "order": vb.KEY_ORDER,
-            "halo_lo": vb.KEY_HALO_LO, "halo_hi": vb.KEY_HALO_HI, "tune_tile": vb.KEY_TUNE_TILE}
+            "halo_lo": vb.KEY_HALO_LO, "halo_hi": vb.KEY_HALO_HI, "tune_tile": vb.KEY_TUNE_TILE, "tune_rc": vb.KEY_TUNE_RC}
     for k, v in params.items():
         vb.vlasov_set_param(keys[k], v)
     for k, v in c["params"].items():

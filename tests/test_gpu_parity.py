@@ -123,7 +123,7 @@ ONEPASS_GRIDS = [(64, 48), (352, 30), (353, 61), (1000, 137), (2233, 25), (31, 9
 @pytest.mark.parametrize("grid", ONEPASS_GRIDS)
 @pytest.mark.parametrize("bc_p", [BC_ZERO, BC_PERIODIC])
 @pytest.mark.parametrize("which,dt,amp", [(1, 0.1, 0.5), (2, 0.1, 0.5), (2, -0.37, 30.0), (1, 9.0, 2000.0),
-                                          (2, 9.0, 30.0), (2, 3.0, 0.0)])
+                                          (2, 9.0, 30.0), (2, 3.0, 0.0), (2, 0.1, 300.0), (1, 0.1, 7.0)])
 @pytest.mark.parametrize("tile", [1, 2])
 def test_one_pass_p_then_theta(grid, bc_p, which, dt, amp, tile):
     """p shift with a given force, then one or two half theta shifts, then density and force of the result:

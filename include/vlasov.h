@@ -90,7 +90,10 @@ extern "C" {
  *                                the warp-specialised one: 0 by size (default: up to 4.5e6 grid points, i.e. 2048^2), 1 whenever its conditions
  *                                hold, 2 never
  *   112 TUNE_RC                  2: never rho_force_cluster_kernel (HMF density / moments / force of theta axes of up to 1024
- *                                columns by one thread-block cluster); the ticketed rho_force_kernel on every grid instead   */
+ *                                columns by one thread-block cluster); the ticketed rho_force_kernel on every grid instead   
+ *   113 TUNE_HIST                2: HISTORY = 1 always by the separate passes (theta, p + theta, moments read pass per step);
+ *                                default: on small grids (tile kernel) with the HMF model the history is recorded on the
+ *                                one-pass path (history_rows_kernel)                                                   */
 
 /* sub-steps for vlasov_substep (parity tests of single stages; same kernels as vlasov_step) */
 #define VLASOV_SUB_THETA_HALF 0  /* eq (9)/(12): f(x - p dt/2, p), also leaves the column sums for the force */

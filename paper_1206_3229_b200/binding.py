@@ -19,7 +19,7 @@ from . import build as _build
 MODEL_FREE, MODEL_HMF, MODEL_RING, MODEL_SHEET = 0, 1, 2, 3
 KEY_EPS, KEY_PRECISION, KEY_BC_X, KEY_BC_P, KEY_HISTORY, KEY_FUSE, KEY_PROFILE, KEY_SPLINE, KEY_ORDER, KEY_HALO_LO, KEY_HALO_HI = 1, 2, 3, 4, 5, 6, 7, 8, 9, 10, 11
 SPLINE_FD, SPLINE_GS = 0, 1
-KEY_TUNE_NW1, KEY_TUNE_NW2, KEY_TUNE_BANDS, KEY_TUNE_PSEG, KEY_TUNE_PTX, KEY_TUNE_GENERIC, KEY_TUNE_FBANDS, KEY_TUNE_FEDGE, KEY_TUNE_GRAPH, KEY_TUNE_PDL, KEY_TUNE_TILE, KEY_TUNE_RC = 101, 102, 103, 104, 105, 106, 107, 108, 109, 110, 111, 112
+KEY_TUNE_NW1, KEY_TUNE_NW2, KEY_TUNE_BANDS, KEY_TUNE_PSEG, KEY_TUNE_PTX, KEY_TUNE_GENERIC, KEY_TUNE_FBANDS, KEY_TUNE_FEDGE, KEY_TUNE_GRAPH, KEY_TUNE_PDL, KEY_TUNE_TILE, KEY_TUNE_RC, KEY_TUNE_HIST = 101, 102, 103, 104, 105, 106, 107, 108, 109, 110, 111, 112, 113
 SUB_THETA_HALF, SUB_FORCE, SUB_P_FULL, SUB_THETA_TWICE, SUB_P_THETA_HALF, SUB_P_THETA_TWICE, SUB_RHO, SUB_FORCE_FROM_RHO = 0, 1, 2, 3, 4, 5, 6, 7
 VEC_RHO, VEC_FORCE = 0, 1
 OK, EINVAL, ENOTINIT, ECUDA, ENOMEM = 0, -1, -2, -3, -4
@@ -274,7 +274,7 @@ class Vlasov:
         keys = {"eps": KEY_EPS, "bc_x": KEY_BC_X, "bc_p": KEY_BC_P, "history": KEY_HISTORY, "fuse": KEY_FUSE, "profile": KEY_PROFILE, "spline": KEY_SPLINE, "order": KEY_ORDER, "halo_lo": KEY_HALO_LO, "halo_hi": KEY_HALO_HI,
                 "tune_nw1": KEY_TUNE_NW1, "tune_nw2": KEY_TUNE_NW2, "tune_bands": KEY_TUNE_BANDS,
                 "tune_pseg": KEY_TUNE_PSEG, "tune_ptx": KEY_TUNE_PTX, "tune_generic": KEY_TUNE_GENERIC,
-                "tune_fbands": KEY_TUNE_FBANDS, "tune_fedge": KEY_TUNE_FEDGE, "tune_graph": KEY_TUNE_GRAPH, "tune_pdl": KEY_TUNE_PDL, "tune_tile": KEY_TUNE_TILE, "tune_rc": KEY_TUNE_RC}
+                "tune_fbands": KEY_TUNE_FBANDS, "tune_fedge": KEY_TUNE_FEDGE, "tune_graph": KEY_TUNE_GRAPH, "tune_pdl": KEY_TUNE_PDL, "tune_tile": KEY_TUNE_TILE, "tune_rc": KEY_TUNE_RC, "tune_hist": KEY_TUNE_HIST}
         for k, v in params.items():
             vlasov_set_param(keys[k], float(v))
         self.f_dev = self.work_dev = None

@@ -46,7 +46,7 @@ constexpr int FW_NTW = VL_FW_NTW_;       // its theta warps = density partial ro
 constexpr int KEY_TUNE_GRAPH = 109, KEY_TUNE_PDL = 110, KEY_TUNE_FEDGE = 108;
 constexpr int FU_PAD = 12;       // rows of padding of the theta weight tables (the last phase of a band reads on)
 constexpr int NCLS = 6;          // profiled kernel classes: theta x1, theta x2, p, rho+force, p+theta x2, p+theta x1
-constexpr int KEY_TUNE_FBANDS = 107, KEY_TUNE_TILE = 111, KEY_TUNE_RC = 112;
+constexpr int KEY_TUNE_FBANDS = 107, KEY_TUNE_TILE = 111, KEY_TUNE_RC = 112, KEY_TUNE_HIST = 113;
 constexpr double TILE_MAX_POINTS = 4.5e6;  // grids up to 2048^2 take the tile kernel (sweep in profiles/README.md: it wins up to there)
 constexpr int KEY_TUNE_NW1 = 101, KEY_TUNE_NW2 = 102, KEY_TUNE_BANDS = 103, KEY_TUNE_PSEG = 104,
               KEY_TUNE_PTX = 105, KEY_TUNE_GENERIC = 106;
@@ -107,7 +107,11 @@ struct Ctx {
     int tune_fbands = 0;
     // small grids (state in L2): the tile kernel instead of the warp-specialised one (vlasov_tile.cuh); KEY_TUNE_TILE:
     // 0 = by size, 1 = whenever its conditions hold, 2 = never
+    // history on the one-pass path (history_rows_kernel): per-row sums of the tile kernel, 1 / T_j of every row
+    double *rowmom = nullptr, *hist_invT = nullptr;
+    bool want_rowmom = false;
     int rc_max_cluster = 8;  // largest cluster rho_force_cluster_kernel may be launched with (16 where the GPU can place it)
+    int tune_hist = 0;       // KEY_TUNE_HIST: 2 = history always by the separate passes (theta, p + theta, moments pass)
     int tune_rc = 0;         // KEY_TUNE_RC: 2 = never the cluster kernel (the ticketed rho_force_kernel on every grid)
     bool tile = false;
     int tune_tile = 0, tile_nr = 16;
@@ -194,13 +198,14 @@ int cdiv(int a, int b) { return (a + b - 1) / b; }
 void free_small() {
     void* ptrs[] = {G.srow, G.wrow, G.cos_t, G.sin_t, G.ringK, G.ringV, G.rho, G.force, G.rho_m,
                     G.phi,  G.mpart, G.pkpart, G.mom_dev, G.hist, G.wrow2, G.colpart_f, G.ticket, G.caspart, G.ringpart, G.ringtick,
-                    G.gsab, G.srow_sub[0], G.srow_sub[1], G.wrow_sub[0], G.wrow_sub[1]};
+                    G.gsab, G.srow_sub[0], G.srow_sub[1], G.wrow_sub[0], G.wrow_sub[1], G.rowmom, G.hist_invT};
     for (void* p : ptrs)
         if (p) cudaFree(p);
     G.srow = nullptr;
     G.wrow = G.cos_t = G.sin_t = G.ringK = G.ringV = G.rho = G.force = G.rho_m = G.phi = G.mpart = G.pkpart =
         G.mom_dev = G.hist = G.wrow2 = G.colpart_f = nullptr;
     G.ticket = nullptr;
+    G.rowmom = G.hist_invT = nullptr;
     G.gsab = nullptr;
     G.srow_sub[0] = G.srow_sub[1] = nullptr;
     G.wrow_sub[0] = G.wrow_sub[1] = nullptr;
@@ -663,6 +668,26 @@ int prepare_tables() {
     }
     CU(cudaMalloc(&G.pkpart, sizeof(double) * 2 * (size_t)G.mbands * cdiv(nt, 256)));
     CU(cudaMalloc(&G.caspart, sizeof(double) * 4 * ((size_t)G.mbands * cdiv(nt, 256) + 1)));
+    if (G.onepass && G.tile) {
+        // history on the one-pass path: 1 / T_j, T_j = e^{-i s_j dx} sum_m w_m e^{-i (m - 4) dx} (history_rows_kernel)
+        std::vector<double> inv((size_t)np * 2);
+        for (int j = 0; j < np; ++j) {
+            const double* w = &wrow[(size_t)j * vl::WROW_STRIDE];
+            double tr = 0.0, ti = 0.0;
+            for (int m = 0; m < 10; ++m) {
+                const double ph = -((double)srow[j] + (double)(m - 4)) * dx;
+                tr += w[m] * cos(ph);
+                ti += w[m] * sin(ph);
+            }
+            const double n2 = tr * tr + ti * ti;
+            inv[2 * j] = tr / n2;
+            inv[2 * j + 1] = -ti / n2;
+        }
+        CU(cudaMalloc(&G.hist_invT, sizeof(double) * inv.size()));
+        CU(cudaMemcpy(G.hist_invT, inv.data(), sizeof(double) * inv.size(), cudaMemcpyHostToDevice));
+        const size_t nblk = (size_t)(G.fcols[2] > G.fcols[1] ? G.fcols[2] : G.fcols[1]);
+        CU(cudaMalloc(&G.rowmom, sizeof(double) * 3 * nblk * np));
+    }
     if (G.onepass) {
         const size_t nb = (size_t)(G.fbands[2] > G.fbands[1] ? G.fbands[2] : G.fbands[1]) * G.fnw();
         CU(cudaMalloc(&G.colpart_f, sizeof(double) * nb * nt));
@@ -848,6 +873,9 @@ int launch_fused(bool want_colsums) {
     a.edge_w = NST == 2 ? G.fedge : 100;
     a.xw = G.fxw;
     a.colpart = want_colsums ? G.colpart_f : nullptr;
+    a.rowmom = (G.tile && G.want_rowmom) ? G.rowmom : nullptr;
+    a.cos_t = G.cos_t;
+    a.sin_t = G.sin_t;
     a.ntheta = G.ntheta;
     a.np = G.np;
     a.bc_p = G.bc_p;
@@ -1127,6 +1155,7 @@ int vlasov_set_param(int key, double value) {
         case KEY_TUNE_FBANDS: G.tune_fbands = (int)value; break;
         case KEY_TUNE_TILE: G.tune_tile = (int)value; break;
         case KEY_TUNE_RC: G.tune_rc = (int)value; break;
+        case KEY_TUNE_HIST: G.tune_hist = (int)value; break;
         case KEY_TUNE_GRAPH: G.graphs = (value != 0.0); break;
         case KEY_TUNE_PDL: G.pdl = (value != 0.0); break;
         case KEY_TUNE_FEDGE: G.tune_fedge = (int)value; break;
@@ -1247,6 +1276,30 @@ int vlasov_step(int n) {
         G.wrow = wrow0;
         G.dt_sub = G.dt;
         if (rc != 0) return rc;
+    } else if (G.onepass && G.history && G.tile && G.model == VLASOV_MODEL_HMF && G.rowmom != nullptr && G.tune_hist != 2 &&
+               fabs((G.xmax - G.xmin) - 6.283185307179586) < 1e-9) {
+        // HISTORY on the one-pass path (small grids, HMF): n + 1 passes as below; the tile kernel also leaves per-row sums of
+        // the state it stores and history_rows_kernel turns them into the moments of the end-of-step state (the half shift
+        // that opens the next step only multiplies a row's first Fourier sum by a known number)
+        const double dp = (G.pmax - G.pmin) / (double)G.np, dx = (G.xmax - G.xmin) / (double)G.ntheta;
+        if ((rc = theta_pass(1, true)) != 0) return rc;                           // eq (9)
+        G.want_rowmom = true;
+        for (int k = 0; k < n; ++k) {
+            const bool last = k + 1 == n;
+            if (k == 0) rc = rho_and_force(theta_bands(1), nullptr, false);              // eq (10)
+            else rc = rho_and_force(G.fbands[2] * G.fnw(), G.colpart_f, true);
+            if (rc == VLASOV_OK) rc = fused_pass(last ? 1 : 2, !last);                   // eqs (11), (12) [, (9)]
+            if (rc != VLASOV_OK) break;
+            vl::history_rows_kernel<<<1, 1024, 0, G.stream>>>(G.rowmom, G.fcols[last ? 1 : 2], G.np, G.hist_invT, last ? 1 : 0,
+                                                              G.pmin, dp, dx, G.t + (double)(k + 1) * G.dt,
+                                                              G.hist + 8 * (size_t)k);
+            G.launches++;
+            G.hist_count = k + 1;
+        }
+        G.want_rowmom = false;
+        if (rc != VLASOV_OK) return rc;
+        CU(cudaGetLastError());
+        G.t += (double)n * G.dt;
     } else if (G.onepass && !G.history) {
         // n + 1 passes: theta(dt/2), then per step ONE pass  p(dt) -> theta(dt/2) [-> theta(dt/2) of the next step]
         if ((rc = theta_pass(1, true)) != 0) return rc;                           // eq (9)

@@ -55,6 +55,10 @@ struct FusedArgs {
     int x0, xw;              // the column blocks tile the source positions [x0, x0 + xw): [0, Ntheta) on a periodic axis; on a
                              // zero-extended one (ZX) also what the rows drift beyond the ends (x0 <= 0, even)
     double dt, dp;
+    // tile kernel only (history on the one-pass path, vlasov_tile.cuh): per (column block, row) the sums of the output row and
+    // of the row times cos theta_i, sin theta_i -> rowmom[block][row][3]; null: not wanted
+    double* rowmom;
+    const double *cos_t, *sin_t;
 };
 
 namespace ptx {

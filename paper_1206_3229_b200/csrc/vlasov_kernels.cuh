@@ -816,6 +816,62 @@ __global__ void __launch_bounds__(256) moments_pass_kernel(const T* __restrict__
     }
 }
 
+// HISTORY on the one-pass path (HMF model, periodic theta axis of length 2 pi): the eight moments of the END-OF-STEP state
+// f^{n+1} from per-row sums of the state the one-pass path stores, h = theta(dt/2) f^{n+1} (the leading half shift of the
+// next step is already applied).  A half shift of a periodic row is a circular convolution, h_i = sum_m w_m f_{i+s+m-4},
+// so it multiplies the row's first Fourier sum by a number that depends on the row only:
+//     sum_i h_i e^{i theta_i} = T_j sum_l f_l e^{i theta_l},   T_j = e^{-i s_j dtheta} sum_m w_m e^{-i (m-4) dtheta},
+// and leaves the row's sum alone.  So with R0_j, Rc_j, Rs_j the sums of row j of h (times 1, cos theta_i, sin theta_i; from
+// strang_tile_kernel, per column block) and 1/T_j from the host:  mass, P, K from R0 (eq (6) discretised, D6), and
+// M_x + i M_y = dtheta dp sum_j (Rc_j + i Rs_j) / T_j (eq (8)); U = (m^2 - M^2) / 2 (D10).  ident = 1: the stored state IS
+// f^{n+1} (last pass of a call: one half shift only).  One CTA, fixed order.  out = {t, mass, P, K, U, Mx, My, E}
+__global__ void __launch_bounds__(1024) history_rows_kernel(const double* __restrict__ rowmom /* [nblk][np][3] */, int nblk, int np,
+                                                            const double* __restrict__ invT /* [np][2] */, int ident,
+                                                            double pmin, double dp, double dtheta, double t,
+                                                            double* __restrict__ out) {
+    __shared__ double red[32];
+    double m = 0.0, pp = 0.0, kk = 0.0, mx = 0.0, my = 0.0;
+    for (int j = threadIdx.x; j < np; j += 1024) {
+        double r0 = 0.0, rc = 0.0, rs = 0.0;
+        for (int b = 0; b < nblk; ++b) {
+            const double* rm = rowmom + ((size_t)b * np + j) * 3;
+            r0 += __ldcg(rm);
+            rc += __ldcg(rm + 1);
+            rs += __ldcg(rm + 2);
+        }
+        const double p = pmin + (double)j * dp;
+        m += r0;
+        pp = fma(p, r0, pp);
+        kk = fma(0.5 * p * p, r0, kk);
+        if (ident) {
+            mx += rc;
+            my += rs;
+        } else {  // (rc + i rs) (a + i b), a + i b = 1 / T_j
+            const double a = invT[2 * j], b = invT[2 * j + 1];
+            mx += rc * a - rs * b;
+            my += rc * b + rs * a;
+        }
+    }
+    const double M = block_sum<1024>(m, red);
+    const double PP = block_sum<1024>(pp, red);
+    const double KK = block_sum<1024>(kk, red);
+    const double MX = block_sum<1024>(mx, red);
+    const double MY = block_sum<1024>(my, red);
+    if (threadIdx.x == 0) {
+        const double w = dtheta * dp;
+        const double mass = M * w, Mx = MX * w, My = MY * w, K = KK * w;
+        const double U = 0.5 * (mass * mass - Mx * Mx - My * My);
+        out[0] = t;
+        out[1] = mass;
+        out[2] = PP * w;
+        out[3] = K;
+        out[4] = U;
+        out[5] = Mx;
+        out[6] = My;
+        out[7] = K + U;
+    }
+}
+
 // final: one CTA.  rho must already hold dp * column sums; phi (ring / sheet potential) may be null.
 // out = {t, mass, P, K, U, Mx, My, E}
 __global__ void __launch_bounds__(1024) moments_final_kernel(const double* __restrict__ rho,

@@ -130,13 +130,34 @@ __global__ void __launch_bounds__(TileCfg<NST, NR_>::NT, TileCfg<NST, NR_>::MINB
         __syncwarp();
         const int base = wrap_index(i0 - S, ntheta);
         double* orow = arg.fout + (size_t)(jA + r) * pitch;
+        double r0 = 0.0, rc = 0.0, rs = 0.0;
 #pragma unroll
         for (int k = 0; k < R; ++k) {
             const int q = lane + 32 * k;
             if (q < qmax) {
                 int i = base + q;
                 if (i >= ntheta) i -= ntheta;
-                orow[i] = grow[q];
+                const double v = grow[q];
+                orow[i] = v;
+                if (arg.rowmom != nullptr) {  // history on the one-pass path: the row's sum and first Fourier sums
+                    r0 += v;
+                    rc = fma(v, __ldg(arg.cos_t + i), rc);
+                    rs = fma(v, __ldg(arg.sin_t + i), rs);
+                }
+            }
+        }
+        if (arg.rowmom != nullptr) {
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) {
+                r0 += __shfl_down_sync(0xffffffffu, r0, o);
+                rc += __shfl_down_sync(0xffffffffu, rc, o);
+                rs += __shfl_down_sync(0xffffffffu, rs, o);
+            }
+            if (lane == 0) {
+                double* rm = arg.rowmom + ((size_t)blockIdx.x * (size_t)np + (size_t)(jA + r)) * 3;
+                rm[0] = r0;
+                rm[1] = rc;
+                rm[2] = rs;
             }
         }
     }

@@ -275,9 +275,15 @@ def test_tile_kernel_and_large_grid_kernel_agree_bit_for_bit(grid, bc_p, which):
     assert np.max(np.abs(rhos[0] - rhos[1])) <= 1e-13 * np.max(np.abs(rhos[1]))
 
 
-def test_history_records_every_step_and_matches_oracle():
-    c = inputs.config("cfg1", n=128)
-    o, g = pair(c["model"], c["grid"], c["domain"], c["dt"], c["f0"], gpu_params=dict(history=1))
+@pytest.mark.parametrize("name,kw", [("cfg1", dict(n=128)), ("cfg1", dict()), ("cfg2", dict(ntheta=320, npts=256)),
+                                     ("cfg5", dict(ntheta=700, npts=260)), ("cfg3", dict(ntheta=320, npts=256))])
+@pytest.mark.parametrize("hist", [0, 2])
+def test_history_records_every_step_and_matches_oracle(name, kw, hist):
+    """HISTORY = 1: the eight moments after EVERY step against the oracle's.  hist = 0: on small grids with the HMF model the
+    history comes off the one-pass path (per-row sums of the stored, half-shifted state and the row's Fourier factor,
+    history_rows_kernel); hist = 2 (TUNE_HIST) and the ring model: the separate passes with a moments read pass per step."""
+    c = inputs.config(name, **kw)
+    o, g = pair(c["model"], c["grid"], c["domain"], c["dt"], c["f0"], gpu_params=dict(history=1, tune_hist=hist), **c["params"])
     g.step(20)
     h = g.history(20)
     assert h.shape == (20, 8)
@@ -285,6 +291,11 @@ def test_history_records_every_step_and_matches_oracle():
         o.step(1)
         mo = o.moments()
         assert np.max(np.abs(h[k] - mo)) <= TOL * max(1.0, np.max(np.abs(mo))), k
+    assert rel_err(g.download(), o.download()) <= TOL
+    g.step(3)  # a second call: the history restarts, the clock does not
+    o.step(3)
+    h = g.history(3)
+    assert abs(h[2][0] - 23 * c["dt"]) < 1e-12 and np.max(np.abs(h[2] - o.moments())) <= TOL * max(1.0, np.max(np.abs(o.moments())))
     g.close()
 
 

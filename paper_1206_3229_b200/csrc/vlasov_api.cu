@@ -110,6 +110,7 @@ struct Ctx {
     // history on the one-pass path (history_rows_kernel): per-row sums of the tile kernel, 1 / T_j of every row
     double *rowmom = nullptr, *hist_invT = nullptr;
     bool want_rowmom = false;
+    vl::HistArgs hist_pending = {};  // history of the step that just ended, to ride along with the next density / force launch
     int rc_max_cluster = 8;  // largest cluster rho_force_cluster_kernel may be launched with (16 where the GPU can place it)
     int tune_hist = 0;       // KEY_TUNE_HIST: 2 = history always by the separate passes (theta, p + theta, moments pass)
     int tune_rc = 0;         // KEY_TUNE_RC: 2 = never the cluster kernel (the ticketed rho_force_kernel on every grid)
@@ -927,7 +928,13 @@ int rho_from_colpart(int bands, double* rho_out, bool hmf_partials, double* colp
         // short theta axis (cfg 1, cfg 2), HMF: density, moments and force by one thread-block cluster instead of the ticketed
         // kernel (cfg 1: 9.3 -> 7.5 us per step, cfg 2: 15.4 -> 14.4)
         cudaLaunchConfig_t cfg = {};
-        const unsigned ncta = (unsigned)cdiv(G.ntheta, vl::RC_COLS);
+        vl::HistArgs ha = {};
+        unsigned ncta = (unsigned)cdiv(G.ntheta, vl::RC_COLS);
+        if (G.hist_pending.rowmom != nullptr && (int)ncta + 1 <= G.rc_max_cluster) {  // one more CTA writes the pending history entry
+            ha = G.hist_pending;
+            G.hist_pending.rowmom = nullptr;
+            ncta += 1;
+        }
         cfg.gridDim = dim3(ncta);
         cfg.blockDim = dim3(vl::RC_COLS * vl::RC_GROUPS);
         cfg.stream = G.stream;
@@ -941,7 +948,7 @@ int rho_from_colpart(int bands, double* rho_out, bool hmf_partials, double* colp
         cfg.attrs = attr;
         cfg.numAttrs = G.pdl ? 2 : 1;
         CU(cudaLaunchKernelEx(&cfg, vl::rho_force_cluster_kernel, colpart ? colpart : G.colpart, bands, G.ntheta, dp, rho_out,
-                              (const double*)G.cos_t, (const double*)G.sin_t, zero_after ? 1 : 0, dx, G.force));
+                              (const double*)G.cos_t, (const double*)G.sin_t, zero_after ? 1 : 0, dx, G.force, ha));
         LAUNCH_CHECK();
         return VLASOV_OK;
     }
@@ -1284,18 +1291,34 @@ int vlasov_step(int n) {
         const double dp = (G.pmax - G.pmin) / (double)G.np, dx = (G.xmax - G.xmin) / (double)G.ntheta;
         if ((rc = theta_pass(1, true)) != 0) return rc;                           // eq (9)
         G.want_rowmom = true;
+        // the history entry of step k rides along with the density / force launch of step k + 1 (one more CTA of its cluster);
+        // where that kernel is not the cluster kernel, and after the last step, history_rows_kernel writes it
+        auto flush_history = [&]() {
+            if (G.hist_pending.rowmom == nullptr) return;
+            const vl::HistArgs h = G.hist_pending;
+            G.hist_pending.rowmom = nullptr;
+            vl::history_rows_kernel<<<1, 1024, 0, G.stream>>>(h.rowmom, h.nblk, h.np, h.invT, h.ident, h.pmin, dp, dx, h.t, h.out);
+            G.launches++;
+        };
+        G.hist_pending.rowmom = nullptr;
         for (int k = 0; k < n; ++k) {
             const bool last = k + 1 == n;
             if (k == 0) rc = rho_and_force(theta_bands(1), nullptr, false);              // eq (10)
             else rc = rho_and_force(G.fbands[2] * G.fnw(), G.colpart_f, true);
+            flush_history();                                                             // (if the launch above did not take it)
             if (rc == VLASOV_OK) rc = fused_pass(last ? 1 : 2, !last);                   // eqs (11), (12) [, (9)]
             if (rc != VLASOV_OK) break;
-            vl::history_rows_kernel<<<1, 1024, 0, G.stream>>>(G.rowmom, G.fcols[last ? 1 : 2], G.np, G.hist_invT, last ? 1 : 0,
-                                                              G.pmin, dp, dx, G.t + (double)(k + 1) * G.dt,
-                                                              G.hist + 8 * (size_t)k);
-            G.launches++;
+            G.hist_pending.rowmom = G.rowmom;
+            G.hist_pending.invT = G.hist_invT;
+            G.hist_pending.out = G.hist + 8 * (size_t)k;
+            G.hist_pending.nblk = G.fcols[last ? 1 : 2];
+            G.hist_pending.np = G.np;
+            G.hist_pending.ident = last ? 1 : 0;
+            G.hist_pending.pmin = G.pmin;
+            G.hist_pending.t = G.t + (double)(k + 1) * G.dt;
             G.hist_count = k + 1;
         }
+        flush_history();
         G.want_rowmom = false;
         if (rc != VLASOV_OK) return rc;
         CU(cudaGetLastError());

@@ -629,11 +629,23 @@ __global__ void __launch_bounds__(RR_COLS* RR_GROUPS)
 // loads in flight at once), the eight groups are added in order, the CTA adds its moments over a fixed tree, the CTAs
 // read one another's moment partials through distributed shared memory in rank order (one cluster barrier instead of a
 // ticket in global memory) and every CTA writes the force of its own columns.  eqs (10), (7)-(8) (L75-L78, L56-L63).
+// With HISTORY = 1 on the one-pass path the cluster has one more CTA, the last, which meanwhile turns the per-row sums of the pass
+// that just ended into the moments of that step (history_rows_body below): the history costs no launch of its own.
+struct HistArgs {
+    const double* rowmom;  // null: no history CTA
+    const double* invT;
+    double* out;
+    int nblk, np, ident;
+    double pmin, t;
+};
+__device__ __forceinline__ void history_rows_body(const double* __restrict__ rowmom, int nblk, int np, const double* __restrict__ invT,
+                                                  int ident, double pmin, double dp, double dtheta, double t,
+                                                  double* __restrict__ out, double* red);
 constexpr int RC_COLS = 128, RC_GROUPS = 8;
 __global__ void __launch_bounds__(RC_COLS* RC_GROUPS)
     rho_force_cluster_kernel(double* __restrict__ colpart, int nbands, int ntheta, double dp, double* __restrict__ rho,
                              const double* __restrict__ cos_t, const double* __restrict__ sin_t, int zero_after,
-                             double dtheta, double* __restrict__ force) {
+                             double dtheta, double* __restrict__ force, const HistArgs hist) {
     namespace cg = cooperative_groups;
     cg::cluster_group cluster = cg::this_cluster();
     __shared__ double part[RC_GROUPS][RC_COLS];
@@ -641,6 +653,14 @@ __global__ void __launch_bounds__(RC_COLS* RC_GROUPS)
     __shared__ double2 mine;  // this CTA's (sum cos theta_i rho_i, sum sin theta_i rho_i)
     ptx::pdl_launch_dependents();
     const int tid = threadIdx.x, c = tid & (RC_COLS - 1), g = tid / RC_COLS, lane = tid & 31, warp = tid >> 5;
+    const unsigned ndens = gridDim.x - (hist.rowmom != nullptr ? 1u : 0u);  // CTAs that own columns
+    if (blockIdx.x >= ndens) {  // the history CTA: no columns, but it keeps the cluster's two barriers
+        ptx::pdl_wait();
+        history_rows_body(hist.rowmom, hist.nblk, hist.np, hist.invT, hist.ident, hist.pmin, dp, dtheta, hist.t, hist.out, &part[0][0]);
+        cluster.sync();
+        cluster.sync();
+        return;
+    }
     const int i = blockIdx.x * RC_COLS + c;
     const bool in = i < ntheta;
     const bool own = in && g == 0;
@@ -698,8 +718,7 @@ __global__ void __launch_bounds__(RC_COLS* RC_GROUPS)
     cluster.sync();  // every CTA's partial is written
     if (own) {
         double mx = 0.0, my = 0.0;
-        const unsigned nb = cluster.num_blocks();
-        for (unsigned rk = 0; rk < nb; ++rk) {
+        for (unsigned rk = 0; rk < ndens; ++rk) {
             const double2 t = *cluster.map_shared_rank(&mine, rk);
             mx += t.x;
             my += t.y;
@@ -825,11 +844,10 @@ __global__ void __launch_bounds__(256) moments_pass_kernel(const T* __restrict__
 // strang_tile_kernel, per column block) and 1/T_j from the host:  mass, P, K from R0 (eq (6) discretised, D6), and
 // M_x + i M_y = dtheta dp sum_j (Rc_j + i Rs_j) / T_j (eq (8)); U = (m^2 - M^2) / 2 (D10).  ident = 1: the stored state IS
 // f^{n+1} (last pass of a call: one half shift only).  One CTA, fixed order.  out = {t, mass, P, K, U, Mx, My, E}
-__global__ void __launch_bounds__(1024) history_rows_kernel(const double* __restrict__ rowmom /* [nblk][np][3] */, int nblk, int np,
-                                                            const double* __restrict__ invT /* [np][2] */, int ident,
-                                                            double pmin, double dp, double dtheta, double t,
-                                                            double* __restrict__ out) {
-    __shared__ double red[32];
+__device__ __forceinline__ void history_rows_body(const double* __restrict__ rowmom /* [nblk][np][3] */, int nblk, int np,
+                                                  const double* __restrict__ invT /* [np][2] */, int ident, double pmin,
+                                                  double dp, double dtheta, double t, double* __restrict__ out,
+                                                  double* red /* 32 doubles of shared memory */) {
     double m = 0.0, pp = 0.0, kk = 0.0, mx = 0.0, my = 0.0;
     for (int j = threadIdx.x; j < np; j += 1024) {
         double r0 = 0.0, rc = 0.0, rs = 0.0;
@@ -870,6 +888,13 @@ __global__ void __launch_bounds__(1024) history_rows_kernel(const double* __rest
         out[6] = My;
         out[7] = K + U;
     }
+}
+
+__global__ void __launch_bounds__(1024) history_rows_kernel(const double* __restrict__ rowmom, int nblk, int np,
+                                                            const double* __restrict__ invT, int ident, double pmin, double dp,
+                                                            double dtheta, double t, double* __restrict__ out) {
+    __shared__ double red[32];
+    history_rows_body(rowmom, nblk, np, invT, ident, pmin, dp, dtheta, t, out, red);
 }
 
 // final: one CTA.  rho must already hold dp * column sums; phi (ring / sheet potential) may be null.

@@ -51,7 +51,8 @@ extern "C" {
 #define VLASOV_KEY_PRECISION 2 /* storage precision of f: 64 (default) or 32; arithmetic of sums is fp64    */
 #define VLASOV_KEY_BC_X 3      /* 0 periodic (paper, L113; default for FREE/HMF/RING), 1 zero extension     */
 #define VLASOV_KEY_BC_P 4      /* 0 periodic (paper, L113), 1 zero extension "f = 0 beyond" (default)       */
-#define VLASOV_KEY_HISTORY 5   /* 1: vlasov_step records the 8 moments after every step (no a6 fusion)      */
+#define VLASOV_KEY_HISTORY 5   /* 1: vlasov_step records the 8 moments after every step (HMF model: still on the
+                                  one-pass path, history_rows_kernel; ring and sheet: separate passes)        */
 #define VLASOV_KEY_FUSE 6      /* passes over f per step in vlasov_step(n): 0: three (theta, p, theta); 1: two (the
                                   adjacent half theta shifts of steps k, k+1 share a pass); 2 (default): ONE
                                   (p shift, both half theta shifts and the density of the next step share a pass;
@@ -92,7 +93,7 @@ extern "C" {
  *   112 TUNE_RC                  2: never rho_force_cluster_kernel (HMF density / moments / force of theta axes of up to 1024
  *                                columns by one thread-block cluster); the ticketed rho_force_kernel on every grid instead   
  *   113 TUNE_HIST                2: HISTORY = 1 always by the separate passes (theta, p + theta, moments read pass per step);
- *                                default: on small grids (tile kernel) with the HMF model the history is recorded on the
+ *                                default: with the HMF model (theta axis of length 2 pi) the history is recorded on the
  *                                one-pass path (history_rows_kernel)                                                   */
 
 /* sub-steps for vlasov_substep (parity tests of single stages; same kernels as vlasov_step) */
@@ -158,7 +159,9 @@ int vlasov_download(void* f_host);
  * (default; periodic x, shift of a half step below one domain length) everything inside the brackets plus the
  * density of the next force is ONE kernel and the two adjacent half shifts of a row are applied as one 19-tap
  * filter (the convolution of the ten weights with themselves: the same map up to rounding order); with FUSE = 1
- * they are evaluated one after the other inside one kernel; FUSE = 0 or HISTORY = 1: separate passes.
+ * they are evaluated one after the other inside one kernel; FUSE = 0: separate passes.  HISTORY = 1: the HMF model on a
+ * theta axis of length 2 pi keeps the one-pass path (the moments of the end-of-step state follow from per-row sums of the
+ * stored state, which already carries the next step's leading half shift); the other models take separate passes.
  * Errors: EINVAL (n <= 0), ENOTINIT, ECUDA.
  */
 int vlasov_step(int n);

@@ -550,6 +550,21 @@ int prepare_tables() {
     std::vector<double> wrow((size_t)(np + FU_PAD) * vl::WROW_STRIDE, 0.0);  // FU_PAD rows of padding
     row_tables(tau, srow, wrow);
     G.h_srow = srow;
+    // (from the plain weights, before the fp32 tables go to difference form)
+    // history on the one-pass path: 1 / T_j, T_j = e^{-i s_j dx} sum_m w_m e^{-i (m - 4) dx} (history_rows_kernel)
+    std::vector<double> inv((size_t)np * 2);
+    for (int j = 0; j < np; ++j) {
+        const double* w = &wrow[(size_t)j * vl::WROW_STRIDE];
+        double tr = 0.0, ti = 0.0;
+        for (int m = 0; m < 10; ++m) {
+            const double ph = -((double)srow[j] + (double)(m - 4)) * dx;
+            tr += w[m] * cos(ph);
+            ti += w[m] * sin(ph);
+        }
+        const double n2 = tr * tr + ti * ti;
+        inv[2 * j] = tr / n2;
+        inv[2 * j + 1] = -ti / n2;
+    }
     // composite weights of two equal half shifts, W = w * w (19 taps): the one-pass kernel applies both at once
     const int W2 = G.bc_x == vl::BC_PERIODIC ? 20 : 32;  // FusedWsCfg<T, 2, ..., ZX>::WST
     std::vector<double> wrow2((size_t)(np + FU_PAD) * W2, 0.0);
@@ -669,24 +684,11 @@ int prepare_tables() {
     }
     CU(cudaMalloc(&G.pkpart, sizeof(double) * 2 * (size_t)G.mbands * cdiv(nt, 256)));
     CU(cudaMalloc(&G.caspart, sizeof(double) * 4 * ((size_t)G.mbands * cdiv(nt, 256) + 1)));
-    if (G.onepass && G.tile) {
-        // history on the one-pass path: 1 / T_j, T_j = e^{-i s_j dx} sum_m w_m e^{-i (m - 4) dx} (history_rows_kernel)
-        std::vector<double> inv((size_t)np * 2);
-        for (int j = 0; j < np; ++j) {
-            const double* w = &wrow[(size_t)j * vl::WROW_STRIDE];
-            double tr = 0.0, ti = 0.0;
-            for (int m = 0; m < 10; ++m) {
-                const double ph = -((double)srow[j] + (double)(m - 4)) * dx;
-                tr += w[m] * cos(ph);
-                ti += w[m] * sin(ph);
-            }
-            const double n2 = tr * tr + ti * ti;
-            inv[2 * j] = tr / n2;
-            inv[2 * j + 1] = -ti / n2;
-        }
+    if (G.onepass && G.bc_x == vl::BC_PERIODIC) {
         CU(cudaMalloc(&G.hist_invT, sizeof(double) * inv.size()));
         CU(cudaMemcpy(G.hist_invT, inv.data(), sizeof(double) * inv.size(), cudaMemcpyHostToDevice));
-        const size_t nblk = (size_t)(G.fcols[2] > G.fcols[1] ? G.fcols[2] : G.fcols[1]);
+        // (the tile kernel leaves the row sums per column block; on the large grids a read pass leaves one set per row)
+        const size_t nblk = G.tile ? (size_t)(G.fcols[2] > G.fcols[1] ? G.fcols[2] : G.fcols[1]) : 1;
         CU(cudaMalloc(&G.rowmom, sizeof(double) * 3 * nblk * np));
     }
     if (G.onepass) {
@@ -1283,11 +1285,12 @@ int vlasov_step(int n) {
         G.wrow = wrow0;
         G.dt_sub = G.dt;
         if (rc != 0) return rc;
-    } else if (G.onepass && G.history && G.tile && G.model == VLASOV_MODEL_HMF && G.rowmom != nullptr && G.tune_hist != 2 &&
+    } else if (G.onepass && G.history && G.model == VLASOV_MODEL_HMF && G.rowmom != nullptr && G.tune_hist != 2 &&
                fabs((G.xmax - G.xmin) - 6.283185307179586) < 1e-9) {
-        // HISTORY on the one-pass path (small grids, HMF): n + 1 passes as below; the tile kernel also leaves per-row sums of
-        // the state it stores and history_rows_kernel turns them into the moments of the end-of-step state (the half shift
-        // that opens the next step only multiplies a row's first Fourier sum by a known number)
+        // HISTORY on the one-pass path (HMF): n + 1 passes as below; the tile kernel also leaves per-row sums of the state it
+        // stores (on the large grids a read pass, row_moments_kernel, takes them) and history_rows_kernel turns them into the
+        // moments of the end-of-step state (the half shift that opens the next step only multiplies a row's first Fourier
+        // sum by a known number)
         const double dp = (G.pmax - G.pmin) / (double)G.np, dx = (G.xmax - G.xmin) / (double)G.ntheta;
         if ((rc = theta_pass(1, true)) != 0) return rc;                           // eq (9)
         G.want_rowmom = true;
@@ -1308,10 +1311,19 @@ int vlasov_step(int n) {
             flush_history();                                                             // (if the launch above did not take it)
             if (rc == VLASOV_OK) rc = fused_pass(last ? 1 : 2, !last);                   // eqs (11), (12) [, (9)]
             if (rc != VLASOV_OK) break;
+            if (!G.tile) {  // large grids: the row sums by a read pass over the state the pass has just written
+                if (G.prec == 32)
+                    vl::row_moments_kernel<float><<<cdiv(G.np, 8), 256, 0, G.stream>>>(static_cast<const float*>(G.f[G.cur]), G.ntheta, G.np,
+                                                                                       G.cos_t, G.sin_t, G.rowmom);
+                else
+                    vl::row_moments_kernel<double><<<cdiv(G.np, 8), 256, 0, G.stream>>>(static_cast<const double*>(G.f[G.cur]), G.ntheta,
+                                                                                        G.np, G.cos_t, G.sin_t, G.rowmom);
+                G.launches++;
+            }
             G.hist_pending.rowmom = G.rowmom;
             G.hist_pending.invT = G.hist_invT;
             G.hist_pending.out = G.hist + 8 * (size_t)k;
-            G.hist_pending.nblk = G.fcols[last ? 1 : 2];
+            G.hist_pending.nblk = G.tile ? G.fcols[last ? 1 : 2] : 1;
             G.hist_pending.np = G.np;
             G.hist_pending.ident = last ? 1 : 0;
             G.hist_pending.pmin = G.pmin;

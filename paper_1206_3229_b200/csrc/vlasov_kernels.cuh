@@ -890,6 +890,48 @@ __device__ __forceinline__ void history_rows_body(const double* __restrict__ row
     }
 }
 
+// the three sums of every row of f (times 1, cos theta_i, sin theta_i) by a read pass: what strang_tile_kernel leaves behind on
+// small grids, for the grids of the warp-specialised kernel (HISTORY = 1 on the one-pass path at any size).  One warp per row.
+template <typename T>
+__global__ void __launch_bounds__(256) row_moments_kernel(const T* __restrict__ f, int ntheta, int np,
+                                                          const double* __restrict__ cos_t, const double* __restrict__ sin_t,
+                                                          double* __restrict__ rowmom /* [np][3] */) {
+    const int lane = threadIdx.x & 31;
+    const int j = (int)blockIdx.x * 8 + (int)(threadIdx.x >> 5);
+    if (j >= np) return;  // whole warp
+    const T* __restrict__ row = f + (size_t)j * ntheta;
+    double r0 = 0.0, rc = 0.0, rs = 0.0;
+    int i = lane;
+    for (; i + 7 * 32 < ntheta; i += 8 * 32) {  // eight loads in flight per lane; the order of the additions is fixed
+        double v[8];
+#pragma unroll
+        for (int k = 0; k < 8; ++k) v[k] = (double)__ldcs(row + i + 32 * k);
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+            r0 += v[k];
+            rc = fma(v[k], __ldg(cos_t + i + 32 * k), rc);
+            rs = fma(v[k], __ldg(sin_t + i + 32 * k), rs);
+        }
+    }
+    for (; i < ntheta; i += 32) {
+        const double v = (double)__ldcs(row + i);
+        r0 += v;
+        rc = fma(v, __ldg(cos_t + i), rc);
+        rs = fma(v, __ldg(sin_t + i), rs);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        r0 += __shfl_down_sync(0xffffffffu, r0, o);
+        rc += __shfl_down_sync(0xffffffffu, rc, o);
+        rs += __shfl_down_sync(0xffffffffu, rs, o);
+    }
+    if (lane == 0) {
+        rowmom[3 * (size_t)j + 0] = r0;
+        rowmom[3 * (size_t)j + 1] = rc;
+        rowmom[3 * (size_t)j + 2] = rs;
+    }
+}
+
 __global__ void __launch_bounds__(1024) history_rows_kernel(const double* __restrict__ rowmom, int nblk, int np,
                                                             const double* __restrict__ invT, int ident, double pmin, double dp,
                                                             double dtheta, double t, double* __restrict__ out) {

@@ -277,13 +277,15 @@ def test_tile_kernel_and_large_grid_kernel_agree_bit_for_bit(grid, bc_p, which):
 
 @pytest.mark.parametrize("name,kw", [("cfg1", dict(n=128)), ("cfg1", dict()), ("cfg2", dict(ntheta=320, npts=256)),
                                      ("cfg5", dict(ntheta=700, npts=260)), ("cfg3", dict(ntheta=320, npts=256))])
-@pytest.mark.parametrize("hist", [0, 2])
-def test_history_records_every_step_and_matches_oracle(name, kw, hist):
-    """HISTORY = 1: the eight moments after EVERY step against the oracle's.  hist = 0: on small grids with the HMF model the
-    history comes off the one-pass path (per-row sums of the stored, half-shifted state and the row's Fourier factor,
-    history_rows_kernel); hist = 2 (TUNE_HIST) and the ring model: the separate passes with a moments read pass per step."""
+@pytest.mark.parametrize("hist,tile", [(0, 0), (0, 2), (2, 0)])
+def test_history_records_every_step_and_matches_oracle(name, kw, hist, tile):
+    """HISTORY = 1: the eight moments after EVERY step against the oracle's.  hist = 0: with the HMF model the history comes off
+    the one-pass path (per-row sums of the stored, half-shifted state and the row's Fourier factor, history_rows_kernel; the
+    sums from the tile kernel itself on small grids, tile = 0, from a read pass behind the warp-specialised kernel of the large
+    grids, tile = 2); hist = 2 (TUNE_HIST) and the ring model: the separate passes with a moments read pass per step."""
     c = inputs.config(name, **kw)
-    o, g = pair(c["model"], c["grid"], c["domain"], c["dt"], c["f0"], gpu_params=dict(history=1, tune_hist=hist), **c["params"])
+    o, g = pair(c["model"], c["grid"], c["domain"], c["dt"], c["f0"],
+                gpu_params=dict(history=1, tune_hist=hist, tune_tile=tile), **c["params"])
     g.step(20)
     h = g.history(20)
     assert h.shape == (20, 8)
@@ -461,6 +463,21 @@ def test_errors():
         vb.vlasov_step(0)
     assert e.value.code == vb.EINVAL
     vb.vlasov_free()
+
+
+def test_history_fp32_state_on_the_one_pass_path():
+    """fp32 storage: the history off the one-pass path (row sums by the read pass, Fourier factors from the fp64 weights)."""
+    c = inputs.config("cfg1", n=192)
+    o = Oracle(c["model"], c["grid"], c["domain"], c["dt"], threads=8)
+    o.upload(c["f0"])
+    g = vb.Vlasov(c["model"], c["grid"], c["domain"], c["dt"], precision=32, history=1)
+    g.upload(c["f0"].astype(np.float32))
+    g.step(12)
+    h = g.history(12)
+    for k in range(12):
+        o.step(1)
+        assert np.max(np.abs(h[k] - o.moments())) <= 1e-4, k
+    g.close()
 
 
 def test_fp32_path_matches_oracle_to_1e_4():

@@ -397,13 +397,13 @@ int configure_fused() {
 
 // the tile kernel (vlasov_tile.cuh) for NST half shifts: fp64, periodic theta, integer shift not increasing with the row
 // and drifting by no more than the narrowest column block inside a tile's rows.  false: the grid does not qualify.
-template <int NST, int NR>
+template <typename T, int NST, int NR>
 bool configure_tile() {
-    using C = vl::TileCfg<NST, NR>;
+    using C = vl::TileCfg<T, NST, NR>;
     const int np = G.np, nt = G.ntheta;
     for (int j = 1; j < np; ++j)
         if (G.h_srow[j] > G.h_srow[j - 1]) return false;
-    const int gran = G.fgran(sizeof(double));
+    const int gran = G.fgran(sizeof(T));
     const int cols = vl::fused_block_cols(nt, C::R, gran, 100);
     int wmin = nt;
     for (int c = 0; c < cols; ++c) {
@@ -417,7 +417,7 @@ bool configure_tile() {
         const int ja = b * C::NR, jb = (b + 1) * C::NR < np ? (b + 1) * C::NR : np;
         if (NST * (G.h_srow[ja] - G.h_srow[jb - 1]) > wmin) return false;
     }
-    if (cudaFuncSetAttribute(vl::strang_tile_kernel<NST, NR>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM_BYTES) !=
+    if (cudaFuncSetAttribute(vl::strang_tile_kernel<T, NST, NR>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM_BYTES) !=
         cudaSuccess) {
         cudaGetLastError();
         return false;
@@ -462,11 +462,12 @@ int configure_all() {
     }
     G.onepass = (G.fuse >= 2) && (G.halo_lo + G.halo_hi == 0);
     G.tile = false;
-    if (G.onepass && sizeof(T) == 8 && G.bc_x == vl::BC_PERIODIC && G.tune_tile != 2 &&
+    if (G.onepass && G.bc_x == vl::BC_PERIODIC && G.tune_tile != 2 &&
         (G.tune_tile == 1 || (double)G.ntheta * (double)G.np <= TILE_MAX_POINTS)) {
         G.tile = true;
         G.tile_nr = (double)G.ntheta * (double)G.np <= 131072.0 ? 8 : 16;  // more, smaller tiles on the smallest grids
-        G.tile = G.tile_nr == 8 ? (configure_tile<1, 8>() && configure_tile<2, 8>()) : (configure_tile<1, 16>() && configure_tile<2, 16>());
+        G.tile = G.tile_nr == 8 ? (configure_tile<T, 1, 8>() && configure_tile<T, 2, 8>())
+                                : (configure_tile<T, 1, 16>() && configure_tile<T, 2, 16>());
     }
     if (G.onepass && !G.tile) {
         if ((rc = configure_fused<T, 1>()) != 0) return rc;
@@ -887,17 +888,15 @@ int launch_fused(bool want_colsums) {
     a.dp = (G.pmax - G.pmin) / (double)G.np;
     dim3 grid(G.fcols[NST], G.fbands[NST]);
     prof_begin(NST == 2 ? 4 : 5);
-    if constexpr (sizeof(T) == 8) {
-        if (G.tile) {
-            if (G.tile_nr == 8)
-                CU(launch_pdl(vl::strang_tile_kernel<NST, 8>, grid, dim3(vl::TileCfg<NST, 8>::NT), vl::TileCfg<NST, 8>::SMEM_BYTES, a));
-            else
-                CU(launch_pdl(vl::strang_tile_kernel<NST, 16>, grid, dim3(vl::TileCfg<NST, 16>::NT), vl::TileCfg<NST, 16>::SMEM_BYTES, a));
-            prof_end(NST == 2 ? 4 : 5);
-            LAUNCH_CHECK();
-            G.cur ^= 1;
-            return VLASOV_OK;
-        }
+    if (G.tile) {
+        if (G.tile_nr == 8)
+            CU(launch_pdl(vl::strang_tile_kernel<T, NST, 8>, grid, dim3(vl::TileCfg<T, NST, 8>::NT), vl::TileCfg<T, NST, 8>::SMEM_BYTES, a));
+        else
+            CU(launch_pdl(vl::strang_tile_kernel<T, NST, 16>, grid, dim3(vl::TileCfg<T, NST, 16>::NT), vl::TileCfg<T, NST, 16>::SMEM_BYTES, a));
+        prof_end(NST == 2 ? 4 : 5);
+        LAUNCH_CHECK();
+        G.cur ^= 1;
+        return VLASOV_OK;
     }
     if (G.bc_x == vl::BC_PERIODIC)
         CU(launch_pdl(vl::strang_fused_ws_kernel<T, NST, FU_R<T>, FW_NSTG, FW_NTW, false>, grid, dim3(CW::NT), CW::SMEM_BYTES, a));

@@ -17,13 +17,13 @@
 //                sum to colpart[band][column] (red.global.add: at most two tiles touch an entry, onto zero, so the result
 //                does not depend on the order; eq (10)).
 // The arithmetic of both shifts is the same sequence of operations as in strang_fused_ws_kernel (the results agree bit
-// for bit); only periodic theta axes and fp64 are built.
+// for bit, fp32 in difference form included); only periodic theta axes are built.
 #pragma once
 #include "vlasov_fused.cuh"
 
 namespace vl {
 
-template <int NST, int NR_>
+template <typename T, int NST, int NR_>
 struct TileCfg {
     static constexpr int NR = NR_;                 // rows per tile: 16, or 8 on the smallest grids (more CTAs: cfg 1 10.3 -> 9.3 us
                                                    // per step; sweep of 8 / 16 / 24 / 32 in profiles/README.md)
@@ -36,18 +36,19 @@ struct TileCfg {
     static constexpr int NW = NT / 32;
     static constexpr int GP = NTA | 1;             // row pitch of the tile in shared memory
     static constexpr int WST = NST == 2 ? 20 : WROW_STRIDE;
-    static constexpr size_t SMEM_BYTES = (size_t)NR * GP * sizeof(double) + (size_t)NR * WST * sizeof(double);
+    static constexpr size_t W_OFF = ((size_t)NR * GP * sizeof(T) + 15) / 16 * 16;  // weight rows behind the tile
+    static constexpr size_t SMEM_BYTES = W_OFF + (size_t)NR * WST * sizeof(double);
     static_assert(NTA <= NT, "one thread per source column");
     static_assert(NR % NW == 0, "");
 };
 
-template <int NST, int NR_>
-__global__ void __launch_bounds__(TileCfg<NST, NR_>::NT, TileCfg<NST, NR_>::MINB) strang_tile_kernel(const FusedArgs<double> arg) {
-    using C = TileCfg<NST, NR_>;
+template <typename T, int NST, int NR_>
+__global__ void __launch_bounds__(TileCfg<T, NST, NR_>::NT, TileCfg<T, NST, NR_>::MINB) strang_tile_kernel(const FusedArgs<T> arg) {
+    using C = TileCfg<T, NST, NR_>;
     constexpr int NR = C::NR, R = C::R, NTAP = C::NTAP, NTA = C::NTA, GP = C::GP, WST = C::WST;
     extern __shared__ __align__(16) unsigned char tile_smem[];
-    double* g = reinterpret_cast<double*>(tile_smem);          // [NR][GP] rows after the momentum shift, then the outputs
-    double* wsm = g + (size_t)NR * GP;                         // [NR][WST] weight rows
+    T* g = reinterpret_cast<T*>(tile_smem);                    // [NR][GP] rows after the momentum shift, then the outputs
+    double* wsm = reinterpret_cast<double*>(tile_smem + C::W_OFF);  // [NR][WST] weight rows
     __shared__ int delta[NR];                                  // S_first - S_r
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -79,25 +80,49 @@ __global__ void __launch_bounds__(TileCfg<NST, NR_>::NT, TileCfg<NST, NR_>::MINB
             const double lim = (double)np + 64.0;
             s = (int)fmin(fmax(sf, -lim), lim);
         }
-        double w[10];
-        spline_fd8_weights(a, w);
-        const double* col = arg.fin + c;
+        double wd[10];
+        spline_fd8_weights(a, wd);
+        T w[10];
+        if constexpr (sizeof(T) == 4) {  // fp32 arithmetic: difference form (diff_form_weights), as in the big kernel
+            double U[9];
+            diff_form_weights(wd, 10, FD_C, U);
+#pragma unroll
+            for (int m = 0; m < 9; ++m) w[m] = (T)U[m];
+            w[9] = T(0);
+        } else {
+#pragma unroll
+            for (int m = 0; m < 10; ++m) w[m] = (T)wd[m];
+        }
+        const T* col = arg.fin + c;
         int rn = jA + s - 4;
         if (p_periodic) rn = wrap_index(rn, np);
-        double v[NR + 9];
+        T v[NR + 9];
 #pragma unroll
         for (int m = 0; m < NR + 9; ++m) {
             const bool ok = p_periodic || (unsigned)rn < (unsigned)np;
-            v[m] = ok ? __ldg(col + (size_t)rn * pitch) : 0.0;
+            v[m] = ok ? __ldg(col + (size_t)rn * pitch) : T(0);
             ++rn;
             if (p_periodic && rn >= np) rn = 0;
         }
+        if constexpr (sizeof(T) == 4) {
+            T e[NR + 8];
 #pragma unroll
-        for (int r = 0; r < NR; ++r) {
-            double acc = w[0] * v[r];
+            for (int m = 0; m < NR + 8; ++m) e[m] = v[m + 1] - v[m];
 #pragma unroll
-            for (int m = 1; m < 10; ++m) acc = fma(w[m], v[r + m], acc);
-            g[r * GP + tid] = acc;
+            for (int r = 0; r < NR; ++r) {
+                T acc = v[r + FD_C];
+#pragma unroll
+                for (int m = 0; m < 9; ++m) acc = fma(w[m], e[r + m], acc);
+                g[r * GP + tid] = acc;
+            }
+        } else {
+#pragma unroll
+            for (int r = 0; r < NR; ++r) {
+                T acc = w[0] * v[r];
+#pragma unroll
+                for (int m = 1; m < 10; ++m) acc = fma(w[m], v[r + m], acc);
+                g[r * GP + tid] = acc;
+            }
         }
     }
     __syncthreads();
@@ -106,21 +131,36 @@ __global__ void __launch_bounds__(TileCfg<NST, NR_>::NT, TileCfg<NST, NR_>::MINB
     const int S0 = (int)wsm[NTAP];  // shift of the first row (the largest: S does not increase with the row)
     for (int r = warp; r < nrows; r += C::NW) {
         const double* Wr = wsm + r * WST;
-        double* grow = g + r * GP;
-        double x[R + NTAP - 1];
+        T* grow = g + r * GP;
+        T x[R + NTAP - 1];
 #pragma unroll
         for (int k = 0; k < R + NTAP - 1; ++k) x[k] = grow[lane * R + k];
-        double out[R];
-        {
-            const double W0 = Wr[0];
+        T out[R];
+        if constexpr (sizeof(T) == 4) {  // difference form: the table holds U_0 .. U_{NTAP-2}, centre tap CT
+            constexpr int CT = NST == 2 ? 2 * FD_C + 1 : FD_C;
+            T d[R + NTAP - 2];
 #pragma unroll
-            for (int q = 0; q < R; ++q) out[q] = W0 * x[q];
-        }
+            for (int k = 0; k < R + NTAP - 2; ++k) d[k] = x[k + 1] - x[k];
 #pragma unroll
-        for (int n = 1; n < NTAP; ++n) {
-            const double Wn = Wr[n];
+            for (int q = 0; q < R; ++q) out[q] = x[q + CT];
 #pragma unroll
-            for (int q = 0; q < R; ++q) out[q] = fma(Wn, x[q + n], out[q]);
+            for (int n = 0; n < NTAP - 1; ++n) {
+                const T Wn = (T)Wr[n];
+#pragma unroll
+                for (int q = 0; q < R; ++q) out[q] = fma(Wn, d[q + n], out[q]);
+            }
+        } else {
+            {
+                const T W0 = (T)Wr[0];
+#pragma unroll
+                for (int q = 0; q < R; ++q) out[q] = W0 * x[q];
+            }
+#pragma unroll
+            for (int n = 1; n < NTAP; ++n) {
+                const T Wn = (T)Wr[n];
+#pragma unroll
+                for (int q = 0; q < R; ++q) out[q] = fma(Wn, x[q + n], out[q]);
+            }
         }
         const int S = (int)Wr[NTAP];
         __syncwarp();  // every lane has its window
@@ -129,7 +169,7 @@ __global__ void __launch_bounds__(TileCfg<NST, NR_>::NT, TileCfg<NST, NR_>::MINB
         if (lane == 0) delta[r] = S0 - S;
         __syncwarp();
         const int base = wrap_index(i0 - S, ntheta);
-        double* orow = arg.fout + (size_t)(jA + r) * pitch;
+        T* orow = arg.fout + (size_t)(jA + r) * pitch;
         double r0 = 0.0, rc = 0.0, rs = 0.0;
 #pragma unroll
         for (int k = 0; k < R; ++k) {
@@ -137,8 +177,9 @@ __global__ void __launch_bounds__(TileCfg<NST, NR_>::NT, TileCfg<NST, NR_>::MINB
             if (q < qmax) {
                 int i = base + q;
                 if (i >= ntheta) i -= ntheta;
-                const double v = grow[q];
-                orow[i] = v;
+                const T vo = grow[q];
+                orow[i] = vo;
+                const double v = (double)vo;
                 if (arg.rowmom != nullptr) {  // history on the one-pass path: the row's sum and first Fourier sums
                     r0 += v;
                     rc = fma(v, __ldg(arg.cos_t + i), rc);
@@ -172,7 +213,7 @@ __global__ void __launch_bounds__(TileCfg<NST, NR_>::NT, TileCfg<NST, NR_>::MINB
         double acc = 0.0;
         for (int r = 0; r < nrows; ++r) {
             const int q = u - delta[r];
-            if (q >= 0 && q < qmax) acc += g[r * GP + q];
+            if (q >= 0 && q < qmax) acc += (double)g[r * GP + q];
         }
         ptx::red_add_f64(cp + wrap_index(cb + u, ntheta), acc);
     }

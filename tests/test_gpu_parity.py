@@ -253,18 +253,19 @@ def _run_100_steps_large_grid_kernels(name, kw):
 @pytest.mark.parametrize("grid", [(256, 256), (1000, 137), (353, 61), (2048, 96)])
 @pytest.mark.parametrize("bc_p", [BC_ZERO, BC_PERIODIC])
 @pytest.mark.parametrize("which", [1, 2])
-def test_tile_kernel_and_large_grid_kernel_agree_bit_for_bit(grid, bc_p, which):
+@pytest.mark.parametrize("precision", [64, 32])
+def test_tile_kernel_and_large_grid_kernel_agree_bit_for_bit(grid, bc_p, which, precision):
     """Both one-pass kernels apply the same sequence of floating-point operations to every grid point (ten FMAs of the
-    momentum shift, 10 or 19 of the theta weights): with the same force, f after the pass is the same bits; the density
-    differs only in the order of its column sums."""
+    momentum shift, 10 or 19 of the theta weights; fp32: the same difference form): with the same force, f after the pass
+    is the same bits; the density differs only in the order of its column sums."""
     dom = (-PI, PI, -4.0, 4.0)
     f0 = smooth_state(grid[0], grid[1], dom, seed=11)
     th = inputs.nodes(dom[0], dom[1], grid[0])
     F = 0.8 * np.sin(th + 0.3) + 0.1
     outs, rhos = [], []
     for tile in (1, 2):
-        g = vb.Vlasov(MODEL_HMF, grid, dom, 0.1, bc_p=bc_p, tune_tile=tile)
-        g.upload(f0)
+        g = vb.Vlasov(MODEL_HMF, grid, dom, 0.1, bc_p=bc_p, tune_tile=tile, precision=precision)
+        g.upload(f0.astype(np.float32) if precision == 32 else f0)
         assert g.info()["onepass"] == 1 and g.info()["onepass_tile"] == (1 if tile == 1 else 0)
         g.set_force(F)
         g.substep(vb.SUB_P_THETA_TWICE if which == 2 else vb.SUB_P_THETA_HALF)
@@ -465,12 +466,14 @@ def test_errors():
     vb.vlasov_free()
 
 
-def test_history_fp32_state_on_the_one_pass_path():
-    """fp32 storage: the history off the one-pass path (row sums by the read pass, Fourier factors from the fp64 weights)."""
+@pytest.mark.parametrize("tile", [0, 2])
+def test_history_fp32_state_on_the_one_pass_path(tile):
+    """fp32 storage: the history off the one-pass path (row sums from the tile kernel, tile = 0, or by the read pass behind the
+    warp-specialised kernel, tile = 2; Fourier factors from the fp64 weights)."""
     c = inputs.config("cfg1", n=192)
     o = Oracle(c["model"], c["grid"], c["domain"], c["dt"], threads=8)
     o.upload(c["f0"])
-    g = vb.Vlasov(c["model"], c["grid"], c["domain"], c["dt"], precision=32, history=1)
+    g = vb.Vlasov(c["model"], c["grid"], c["domain"], c["dt"], precision=32, history=1, tune_tile=tile)
     g.upload(c["f0"].astype(np.float32))
     g.step(12)
     h = g.history(12)
@@ -480,13 +483,17 @@ def test_history_fp32_state_on_the_one_pass_path():
     g.close()
 
 
-def test_fp32_path_matches_oracle_to_1e_4():
+@pytest.mark.parametrize("tile", [1, 2])
+def test_fp32_path_matches_oracle_to_1e_4(tile):
+    """tile = 1: the tile kernel of small grids, tile = 2: the warp-specialised kernel of the large ones (fp32: both in
+    difference form)."""
     c = inputs.config("cfg5", ntheta=600, npts=280)
     o = Oracle(c["model"], c["grid"], c["domain"], c["dt"], threads=8)
     o.upload(c["f0"])
     o.step(100)
-    g = vb.Vlasov(c["model"], c["grid"], c["domain"], c["dt"], precision=32)
+    g = vb.Vlasov(c["model"], c["grid"], c["domain"], c["dt"], precision=32, tune_tile=tile)
     g.upload(c["f0"])
+    assert g.info()["onepass_tile"] == (1 if tile == 1 else 0)
     g.step(100)
     assert rel_err(g.download().astype(np.float64), o.download()) <= 1e-4
     g.close()

@@ -466,6 +466,26 @@ def test_errors():
     vb.vlasov_free()
 
 
+@pytest.mark.parametrize("grid", [(353, 61), (64, 48), (1000, 137)])
+@pytest.mark.parametrize("bc_p", [BC_ZERO, BC_PERIODIC])
+@pytest.mark.parametrize("tile", [0, 2])
+def test_history_single_steps_and_ragged_grids(grid, bc_p, tile):
+    """The history off the one-pass path on ragged grids, with either momentum boundary, in calls of one, two and three steps
+    (a call of one step is a single pass with one half shift: its stored state IS the end-of-step state)."""
+    dom = (-PI, PI, -4.0, 4.0)
+    f0 = smooth_state(grid[0], grid[1], dom, seed=9)
+    o, g = pair(MODEL_HMF, grid, dom, 0.1, f0, bc_p=bc_p, gpu_params=dict(history=1, tune_tile=tile))
+    for n in (1, 2, 3, 1):
+        g.step(n)
+        h = g.history(n)
+        for k in range(n):
+            o.step(1)
+            mo = o.moments()
+            assert np.max(np.abs(h[k] - mo)) <= TOL * max(1.0, np.max(np.abs(mo))), (n, k)
+    assert rel_err(g.download(), o.download()) <= TOL
+    g.close()
+
+
 @pytest.mark.parametrize("tile", [0, 2])
 def test_history_fp32_state_on_the_one_pass_path(tile):
     """fp32 storage: the history off the one-pass path (row sums from the tile kernel, tile = 0, or by the read pass behind the

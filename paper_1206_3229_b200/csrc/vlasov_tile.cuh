@@ -97,12 +97,18 @@ __global__ void __launch_bounds__(TileCfg<T, NST, NR_>::NT, TileCfg<T, NST, NR_>
         int rn = jA + s - 4;
         if (p_periodic) rn = wrap_index(rn, np);
         T v[NR + 9];
+        if (rn >= 0 && rn + NR + 9 <= np) {  // all taps exist and do not wrap (the usual column): no per-row tests
+            const T* p0 = col + (size_t)rn * pitch;
 #pragma unroll
-        for (int m = 0; m < NR + 9; ++m) {
-            const bool ok = p_periodic || (unsigned)rn < (unsigned)np;
-            v[m] = ok ? __ldg(col + (size_t)rn * pitch) : T(0);
-            ++rn;
-            if (p_periodic && rn >= np) rn = 0;
+            for (int m = 0; m < NR + 9; ++m) v[m] = __ldg(p0 + (size_t)((unsigned)m * pitch));
+        } else {
+#pragma unroll
+            for (int m = 0; m < NR + 9; ++m) {
+                const bool ok = p_periodic || (unsigned)rn < (unsigned)np;
+                v[m] = ok ? __ldg(col + (size_t)rn * pitch) : T(0);
+                ++rn;
+                if (p_periodic && rn >= np) rn = 0;
+            }
         }
         if constexpr (sizeof(T) == 4) {
             T e[NR + 8];
@@ -129,6 +135,11 @@ __global__ void __launch_bounds__(TileCfg<T, NST, NR_>::NT, TileCfg<T, NST, NR_>
 
     // ---- theta stage ----
     const int S0 = (int)wsm[NTAP];  // shift of the first row (the largest: S does not increase with the row)
+    double* const rowmom = arg.rowmom;
+    const double* const cos_t = arg.cos_t;
+    const double* const sin_t = arg.sin_t;
+    T* const fout = arg.fout;
+    int base0 = wrap_index(i0 - S0, ntheta);  // output column of q = 0 in the first row; later rows: + (S0 - S)
     for (int r = warp; r < nrows; r += C::NW) {
         const double* Wr = wsm + r * WST;
         T* grow = g + r * GP;
@@ -168,8 +179,9 @@ __global__ void __launch_bounds__(TileCfg<T, NST, NR_>::NT, TileCfg<T, NST, NR_>
         for (int q = 0; q < R; ++q) grow[lane * R + q] = out[q];
         if (lane == 0) delta[r] = S0 - S;
         __syncwarp();
-        const int base = wrap_index(i0 - S, ntheta);
-        T* orow = arg.fout + (size_t)(jA + r) * pitch;
+        int base = base0 + (S0 - S);  // = wrap(i0 - S): S0 - S >= 0 stays below one turn inside a tile (configure_tile)
+        if (base >= ntheta) base -= ntheta;
+        T* orow = fout + (size_t)(jA + r) * pitch;
         double r0 = 0.0, rc = 0.0, rs = 0.0;
 #pragma unroll
         for (int k = 0; k < R; ++k) {
@@ -180,14 +192,14 @@ __global__ void __launch_bounds__(TileCfg<T, NST, NR_>::NT, TileCfg<T, NST, NR_>
                 const T vo = grow[q];
                 orow[i] = vo;
                 const double v = (double)vo;
-                if (arg.rowmom != nullptr) {  // history on the one-pass path: the row's sum and first Fourier sums
+                if (rowmom != nullptr) {  // history on the one-pass path: the row's sum and first Fourier sums
                     r0 += v;
-                    rc = fma(v, __ldg(arg.cos_t + i), rc);
-                    rs = fma(v, __ldg(arg.sin_t + i), rs);
+                    rc = fma(v, __ldg(cos_t + i), rc);
+                    rs = fma(v, __ldg(sin_t + i), rs);
                 }
             }
         }
-        if (arg.rowmom != nullptr) {
+        if (rowmom != nullptr) {
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1) {
                 r0 += __shfl_down_sync(0xffffffffu, r0, o);
@@ -195,7 +207,7 @@ __global__ void __launch_bounds__(TileCfg<T, NST, NR_>::NT, TileCfg<T, NST, NR_>
                 rs += __shfl_down_sync(0xffffffffu, rs, o);
             }
             if (lane == 0) {
-                double* rm = arg.rowmom + ((size_t)blockIdx.x * (size_t)np + (size_t)(jA + r)) * 3;
+                double* rm = rowmom + ((size_t)blockIdx.x * (size_t)np + (size_t)(jA + r)) * 3;
                 rm[0] = r0;
                 rm[1] = rc;
                 rm[2] = rs;

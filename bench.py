@@ -296,6 +296,10 @@ def run_cuda(args):
         params["tune_tile"] = args.tile
     if args.rc > 0:
         params["tune_rc"] = args.rc
+    if args.history > 0:
+        params["history"] = 1
+        if args.history == 2:
+            params["tune_hist"] = 2
     g = vb.Vlasov(c["model"], c["grid"], c["domain"], c["dt"], precision=prec, device="cuda:%d" % local_rank, **params)
     g.upload(f0)
     pts = float(nt) * float(npp)
@@ -412,7 +416,7 @@ def run_cuda(args):
                          "oracle/vlasov_oracle.c with OpenMP over lines" % (done, nt, npp, el)}
 
     # `config` is the same object in both arms (the driver compares them); what is particular to this run sits in `run`
-    run = {"passes_per_step": passes / K, "fuse": args.fuse, "pdl": args.pdl, "graph": args.graph,
+    run = {"passes_per_step": passes / K, "fuse": args.fuse, "pdl": args.pdl, "graph": args.graph, "history": args.history,
            "parallelism": "replicas x%d" % world if world > 1 else "single GPU"}
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
@@ -688,6 +692,9 @@ def main():
     ap.add_argument("--fbands", type=int, default=0, help="bands of rows of the one-pass kernel (0 = automatic)")
     ap.add_argument("--tile", type=int, default=0, choices=[0, 1, 2],
                     help="one-pass step of small grids by the tile kernel: 0 by size (default), 1 wherever it applies, 2 never")
+    ap.add_argument("--history", type=int, default=0, choices=[0, 1, 2],
+                    help="1: HISTORY = 1 (the eight moments recorded after every step; HMF: still on the one-pass path), 2: the same "
+                         "by the separate passes (TUNE_HIST = 2)")
     ap.add_argument("--rc", type=int, default=0, choices=[0, 2],
                     help="HMF density / force of short theta axes by one thread-block cluster: 0 (default), 2 never (the ticketed kernel)")
     ap.add_argument("--fedge", type=int, default=0, help="zero-extended x: width (percent) of the two edge column blocks (0 = automatic)")

@@ -397,9 +397,9 @@ int configure_fused() {
 
 // the tile kernel (vlasov_tile.cuh) for NST half shifts: fp64, periodic theta, integer shift not increasing with the row
 // and drifting by no more than the narrowest column block inside a tile's rows.  false: the grid does not qualify.
-template <typename T, int NST, int NR>
+template <typename T, int NST, int NR, int R>
 bool configure_tile() {
-    using C = vl::TileCfg<T, NST, NR>;
+    using C = vl::TileCfg<T, NST, NR, R>;
     const int np = G.np, nt = G.ntheta;
     for (int j = 1; j < np; ++j)
         if (G.h_srow[j] > G.h_srow[j - 1]) return false;
@@ -417,7 +417,7 @@ bool configure_tile() {
         const int ja = b * C::NR, jb = (b + 1) * C::NR < np ? (b + 1) * C::NR : np;
         if (NST * (G.h_srow[ja] - G.h_srow[jb - 1]) > wmin) return false;
     }
-    if (cudaFuncSetAttribute(vl::strang_tile_kernel<T, NST, NR>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM_BYTES) !=
+    if (cudaFuncSetAttribute(vl::strang_tile_kernel<T, NST, NR, R>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM_BYTES) !=
         cudaSuccess) {
         cudaGetLastError();
         return false;
@@ -465,9 +465,13 @@ int configure_all() {
     if (G.onepass && G.bc_x == vl::BC_PERIODIC && G.tune_tile != 2 &&
         (G.tune_tile == 1 || (double)G.ntheta * (double)G.np <= TILE_MAX_POINTS)) {
         G.tile = true;
-        G.tile_nr = (double)G.ntheta * (double)G.np <= 131072.0 ? 8 : 16;  // more, smaller tiles on the smallest grids
-        G.tile = G.tile_nr == 8 ? (configure_tile<T, 1, 8>() && configure_tile<T, 2, 8>())
-                                : (configure_tile<T, 1, 16>() && configure_tile<T, 2, 16>());
+        // tile shape by size (sweeps in profiles/README.md): 8 rows x 224 columns on the smallest grids (more CTAs), 12 x 352 (384
+        // threads) around 1024^2 (fp64; fewer, larger tiles), 16 x 224 beyond
+        const double npts = (double)G.ntheta * (double)G.np;
+        G.tile_nr = npts <= 131072.0 ? 8 : (sizeof(T) == 8 && npts >= 9.5e5 && npts <= 1.2e6 ? 12 : 16);
+        G.tile = G.tile_nr == 8    ? (configure_tile<T, 1, 8, 7>() && configure_tile<T, 2, 8, 7>())
+                 : G.tile_nr == 12 ? (configure_tile<T, 1, 12, 11>() && configure_tile<T, 2, 12, 11>())
+                                   : (configure_tile<T, 1, 16, 7>() && configure_tile<T, 2, 16, 7>());
     }
     if (G.onepass && !G.tile) {
         if ((rc = configure_fused<T, 1>()) != 0) return rc;
@@ -890,9 +894,12 @@ int launch_fused(bool want_colsums) {
     prof_begin(NST == 2 ? 4 : 5);
     if (G.tile) {
         if (G.tile_nr == 8)
-            CU(launch_pdl(vl::strang_tile_kernel<T, NST, 8>, grid, dim3(vl::TileCfg<T, NST, 8>::NT), vl::TileCfg<T, NST, 8>::SMEM_BYTES, a));
+            CU(launch_pdl(vl::strang_tile_kernel<T, NST, 8, 7>, grid, dim3(vl::TileCfg<T, NST, 8, 7>::NT), vl::TileCfg<T, NST, 8, 7>::SMEM_BYTES, a));
+        else if (G.tile_nr == 12)
+            CU(launch_pdl(vl::strang_tile_kernel<T, NST, 12, 11>, grid, dim3(vl::TileCfg<T, NST, 12, 11>::NT),
+                          vl::TileCfg<T, NST, 12, 11>::SMEM_BYTES, a));
         else
-            CU(launch_pdl(vl::strang_tile_kernel<T, NST, 16>, grid, dim3(vl::TileCfg<T, NST, 16>::NT), vl::TileCfg<T, NST, 16>::SMEM_BYTES, a));
+            CU(launch_pdl(vl::strang_tile_kernel<T, NST, 16, 7>, grid, dim3(vl::TileCfg<T, NST, 16, 7>::NT), vl::TileCfg<T, NST, 16, 7>::SMEM_BYTES, a));
         prof_end(NST == 2 ? 4 : 5);
         LAUNCH_CHECK();
         G.cur ^= 1;

@@ -4,7 +4,7 @@
 //
 // strang_fused_ws_kernel marches one CTA per SM down a long band through a three-deep ring: on a 256^2 or 1024^2 grid that
 // is a chain of latencies (first taps, two copy groups, three groups of twelve rows, ...) of about 19 us per pass whatever
-// the size.  Here a CTA owns a TILE of NR = 16 (or 8) rows x (32 lanes x R = 7) output columns and does the pass in three short
+// the size.  Here a CTA owns a TILE of NR = 16 (or 8, or 12) rows x (32 lanes x R = 7 (or 11)) output columns and does the pass in three short
 // phases with two block-wide barriers; a grid of several hundred such CTAs covers the grid in one or two waves:
 //   p stage      thread = source column (TC + NTAP - 1 of them).  All NR + 9 taps of the column are loaded at once (they
 //                come from L2; adjacent lanes read adjacent columns), then NR outputs of ten FMAs each (eq (11))
@@ -23,28 +23,29 @@
 
 namespace vl {
 
-template <typename T, int NST, int NR_>
+template <typename T, int NST, int NR_, int R_>
 struct TileCfg {
     static constexpr int NR = NR_;                 // rows per tile: 16, or 8 on the smallest grids (more CTAs: cfg 1 10.3 -> 9.3 us
                                                    // per step; sweep of 8 / 16 / 24 / 32 in profiles/README.md)
-    static constexpr int MINB = 3;                 // CTAs per SM the register budget is set for (<= 85 registers)
-    static constexpr int R = 7;                    // outputs per lane
+    static constexpr int MINB = R_ <= 7 ? 3 : 2;   // CTAs per SM the register budget is set for (256 threads x 3, 384 x 2: <= 85 registers)
+    static constexpr int R = R_;                   // outputs per lane: 7 (256 threads), or 11 (384 threads) on grids of about 1024^2,
+                                                   // where fewer, larger tiles win (cfg 2 14.4 -> 13.4 us per step; 2048^2: 35.1 against 32.8)
     static constexpr int TC = 32 * R;              // output columns per tile (at most)
     static constexpr int NTAP = NST == 2 ? 19 : 10;
     static constexpr int NTA = TC + NTAP - 1;      // source columns
-    static constexpr int NT = 256;                 // threads
+    static constexpr int NT = (TC + NTAP - 1 + 31) / 32 * 32;  // threads: one per source column (256 for R = 7)
     static constexpr int NW = NT / 32;
     static constexpr int GP = NTA | 1;             // row pitch of the tile in shared memory
     static constexpr int WST = NST == 2 ? 20 : WROW_STRIDE;
     static constexpr size_t W_OFF = ((size_t)NR * GP * sizeof(T) + 15) / 16 * 16;  // weight rows behind the tile
     static constexpr size_t SMEM_BYTES = W_OFF + (size_t)NR * WST * sizeof(double);
     static_assert(NTA <= NT, "one thread per source column");
-    static_assert(NR % NW == 0, "");
+    // (NR need not be a multiple of NW: warps beyond the rows idle in the theta stage)
 };
 
-template <typename T, int NST, int NR_>
-__global__ void __launch_bounds__(TileCfg<T, NST, NR_>::NT, TileCfg<T, NST, NR_>::MINB) strang_tile_kernel(const FusedArgs<T> arg) {
-    using C = TileCfg<T, NST, NR_>;
+template <typename T, int NST, int NR_, int R_>
+__global__ void __launch_bounds__(TileCfg<T, NST, NR_, R_>::NT, TileCfg<T, NST, NR_, R_>::MINB) strang_tile_kernel(const FusedArgs<T> arg) {
+    using C = TileCfg<T, NST, NR_, R_>;
     constexpr int NR = C::NR, R = C::R, NTAP = C::NTAP, NTA = C::NTA, GP = C::GP, WST = C::WST;
     extern __shared__ __align__(16) unsigned char tile_smem[];
     T* g = reinterpret_cast<T*>(tile_smem);                    // [NR][GP] rows after the momentum shift, then the outputs

@@ -117,7 +117,7 @@ def test_density_after_theta_sweep_epilogue():
 
 
 # ----------------------------------------------------------------------------- one-pass kernel (p + theta)
-ONEPASS_GRIDS = [(64, 48), (352, 30), (353, 61), (1000, 137), (2233, 25), (31, 9), (1, 5), (7, 1), (720, 700)]
+ONEPASS_GRIDS = [(64, 48), (352, 30), (353, 61), (1000, 137), (2233, 25), (31, 9), (1, 5), (7, 1), (720, 700), (1023, 1001)]
 
 
 @pytest.mark.parametrize("grid", ONEPASS_GRIDS)
@@ -250,7 +250,7 @@ def _run_100_steps_large_grid_kernels(name, kw):
     g.close()
 
 
-@pytest.mark.parametrize("grid", [(256, 256), (1000, 137), (353, 61), (2048, 96)])
+@pytest.mark.parametrize("grid", [(256, 256), (1000, 137), (353, 61), (2048, 96), (1024, 960)])  # the three tile shapes
 @pytest.mark.parametrize("bc_p", [BC_ZERO, BC_PERIODIC])
 @pytest.mark.parametrize("which", [1, 2])
 @pytest.mark.parametrize("precision", [64, 32])

@@ -466,9 +466,9 @@ int configure_all() {
         (G.tune_tile == 1 || (double)G.ntheta * (double)G.np <= TILE_MAX_POINTS)) {
         G.tile = true;
         // tile shape by size (sweeps in profiles/README.md): 8 rows x 224 columns on the smallest grids (more CTAs), 12 x 352 (384
-        // threads) around 1024^2 (fp64; fewer, larger tiles), 16 x 224 beyond
+        // threads) around 1024^2 (fewer, larger tiles), 16 x 224 beyond
         const double npts = (double)G.ntheta * (double)G.np;
-        G.tile_nr = npts <= 131072.0 ? 8 : (sizeof(T) == 8 && npts >= 9.5e5 && npts <= 1.2e6 ? 12 : 16);
+        G.tile_nr = npts <= 131072.0 ? 8 : (npts >= 9.5e5 && npts <= 1.2e6 ? 12 : 16);
         G.tile = G.tile_nr == 8    ? (configure_tile<T, 1, 8, 7>() && configure_tile<T, 2, 8, 7>())
                  : G.tile_nr == 12 ? (configure_tile<T, 1, 12, 11>() && configure_tile<T, 2, 12, 11>())
                                    : (configure_tile<T, 1, 16, 7>() && configure_tile<T, 2, 16, 7>());
